@@ -1,0 +1,129 @@
+/*
+ * tatrg.h -- C-ABI of libtatrg: Triad-ATRG coarse-graining of the 4D Ising tensor network
+ * on one NVIDIA B200 (sm_100a), FP64.
+ *
+ * The calls follow the paper's statement of the problem (arXiv:2412.14104,
+ * /root/reference/PAPER.md): the model is fixed by the inverse temperature beta
+ * (Eqs. 15-17), the method by the bond dimension chi and the oversampling
+ * parameter r, the number q of RSVD iterations (Table 1) and the
+ * coarse-graining direction ("coarse-graining step along the 1^ direction");
+ * the output is the free energy.
+ *
+ * Conventions
+ *   - One process-global context; not thread safe.  All device work is enqueued on the
+ *     stream given by tatrg_set_stream (default: the legacy default stream).
+ *   - The library allocates no device memory: every device buffer lives in the workspace
+ *     the caller passes to tatrg_set_workspace (e.g. a torch tensor).  The caller keeps it
+ *     alive and unchanged until tatrg_destroy or the next tatrg_set_workspace.
+ *   - Status: 0 = OK, negative = error, message via tatrg_last_error().  Errors never abort
+ *     the process.  A failed coarse_grain leaves the renormalised tensor (Phi, Psi), the
+ *     step count and the ln Z accumulator of the previous step intact.
+ *   - "host" / "device" is stated for every pointer.
+ */
+#ifndef TATRG_H
+#define TATRG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TATRG_OK 0
+#define TATRG_EINVAL (-22)   /* bad argument */
+#define TATRG_ENOMEM (-12)   /* workspace too small */
+#define TATRG_ESTATE (-1)    /* called before init / before a workspace was set */
+#define TATRG_ECUDA (-5)     /* CUDA runtime error (message has the CUDA error string) */
+#define TATRG_ENUM (-34)     /* numerical failure (non-finite value, no convergence) */
+
+/* Initial tensor of the 4D Ising model, Eqs. 16-17:
+ *   T_{i1..i4 j1..j4} = sum_a e^{beta h s_a} prod_mu W_{a i_mu} prod_mu W_{a j_mu},
+ *   W = ((sqrt cosh b, sqrt sinh b), (sqrt cosh b, -sqrt sinh b))  (square roots restored so
+ *   that W W^T = e^{beta s s'}; reading G1; field term: reading G2),
+ * kept factorised as T = sum_g Phi_{i,g} Psi_{j,g} (bond 2), normalised to |Phi|=|Psi|=1.
+ * Resets the step count and the ln Z accumulator.  beta must be finite and > 0, h finite. */
+int init_ising_tensor(double beta, double h);
+
+/* One Triad-ATRG coarse-graining step along `direction` (1..4): canonical form
+ * A sigma D, RSVD bond swap to Gamma = A X sigma Y D (Eq. 1), oversampled
+ * isometries U^A..U^D by RSVD (Eqs. 2-3), triad tensors E..L (Eqs. 4-11), squeezers
+ * M^(mu), N^(mu) (Eq. 12), contraction to Phi, Psi (Eqs. 13-14), normalisation.
+ *   chi >= 1 bond dimension, r >= 1 oversampling (internal lines r*chi), q >= 0 RSVD
+ *   iterations, seed: master seed of the Gaussian sketches (sub-seeds per SURVEY.md 8(d);
+ *   sketches are generated on the host by the shared seeded generator and uploaded inside
+ *   this call unless tatrg_set_sketch supplied them). */
+int coarse_grain(int direction, int chi, int r, int q, uint64_t seed);
+
+/* Same step without the triad decomposition: plain ATRG with bond swapping, O(chi^9)
+ * contraction (Table 1); r and q act on the bond-swap RSVD only. */
+int coarse_grain_atrg(int direction, int chi, int r, int q, uint64_t seed);
+
+/* ln Z / V = sum_m 2^-m ln c_m + 2^-n ln tTr T^(n)  (Eq. 15 closed periodically
+ * after n steps; reading O8).  NaN before init or if the trace is not positive.
+ * One device reduction and one scalar device->host copy. */
+double log_Z_per_site(void);
+
+/* ---- plumbing (PyTorch owns memory and streams) ------------------------------------- */
+int tatrg_set_stream(void *cuda_stream);                     /* cudaStream_t; NULL = default */
+int tatrg_set_workspace(void *dev_ptr, size_t bytes);        /* device; 256-byte aligned */
+size_t tatrg_workspace_bytes(int chi, int r);                /* upper bound, steady state */
+
+/* Caller-supplied Gaussian inputs for the NEXT coarse_grain call (consumed by it).
+ * which: 0 swap sketch [(beta,J), l]; 1..4 isometry sketches A,X,Y,D [(p,q), k];
+ *        5 gauge reference for A/D [(i0..i3), a]; 6..8 gauge references of the squeezers.
+ * data: n doubles, row-major in the rotated frame;
+ * on_device != 0: device pointer, must stay valid until coarse_grain returns;
+ * on_device == 0: host pointer, copied (H2D) inside the next coarse_grain. */
+int tatrg_set_sketch(int which, const double *data, size_t n, int on_device);
+/* Shape the next coarse_grain(direction, chi, r) will ask for input `which`
+ * (rows, cols; 0,0 if unused).  For which = 0,5 the bond after canonicalisation is assumed
+ * equal to the current bond (true whenever Phi Psi^T has full numerical rank). */
+int tatrg_sketch_shape(int which, int direction, int chi, int r, int64_t *rows, int64_t *cols);
+
+/* Spectra of the LAST step, descending, copied to host_out (host, capacity cap doubles).
+ * which: 0 sigma^T (canonical form), 1 sigma (bond swap), 2..5 S^A,S^X,S^Y,S^D (Eq. 3;
+ * count 0 when U is the identity), 6..8 squeezer singular values s^(t1..t3), 9: ln c of the
+ * step (1 value).  Returns the count (<= cap) or a negative status. */
+int tatrg_get_spectrum(int which, double *host_out, int cap);
+
+/* dims_out[0..3] = leg dimensions d1..d4, dims_out[4] = bond, dims_out[5] = step count. */
+int tatrg_get_dims(int dims_out[6]);
+
+/* Copy the current renormalised tensors to the host: phi_out, psi_out each
+ * d1*d2*d3*d4*bond doubles, row-major [i1,i2,i3,i4,g] (host).  For tests. */
+int tatrg_get_tensors(double *phi_out, double *psi_out, size_t cap_each);
+
+/* Order parameter X^(m) = (Tr A)^2 / Tr(A^2), A_kl = sum T_{i1 i2 i3 k; i1 i2 i3 l}
+ * (PAPER.md:177); `leg` = 1..4 is the direction left open (the paper: 4). NaN on error. */
+double tatrg_order_parameter(int leg);
+
+/* Per-stage device milliseconds of the last step (CUDA events): out[0..n) for the stages
+ * named by tatrg_stage_name(i).  Returns the number of stages. */
+int tatrg_get_stage_ms(double *host_out, int cap);
+const char *tatrg_stage_name(int i);
+/* Number of kernel launches this library has enqueued since the last call (and reset). */
+long long tatrg_launch_count(int reset);
+/* FP64 flops of the tensor-GEMM launches since the last reset (2*M*N*K*batch each). */
+double tatrg_gemm_flops(int reset);
+
+/* Measured FP64 peak of this GPU: register-resident loop of mode 0: DMMA.8x8x4 (tensor
+ * pipe), 1: DFMA (vector pipe), 2: both interleaved.  Runs `iters` outer iterations per
+ * warp, returns TFLOP/s (device-timed), <0 on error. */
+double tatrg_probe_fp64_peak(int mode, int iters);
+
+/* Stand-alone tensor-GEMM entry (the contraction kernel the path is built from), for tests
+ * and roofline measurement:  C[b][cm(m)+cn(n)] = alpha * sum_k A[b][am(m)+ak(k)] B[b][bk(k)+bn(n)].
+ * Every index map is two-level: idx -> (idx % n0)*s0 + (idx / n0)*s1, given as
+ * {n0, s0, s1} int64 triples in `maps` in the order am, ak, bk, bn, cm, cn (18 values);
+ * bs = batch strides of A, B, C.  All pointers device. */
+int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N, int K, int batch,
+                      const int64_t *maps, const int64_t *bs, double alpha);
+
+const char *tatrg_last_error(void);
+void tatrg_destroy(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TATRG_H */
