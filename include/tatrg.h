@@ -112,13 +112,39 @@ double tatrg_gemm_flops(int reset);
  * warp, returns TFLOP/s (device-timed), <0 on error. */
 double tatrg_probe_fp64_peak(int mode, int iters);
 
-/* Stand-alone tensor-GEMM entry (the contraction kernel the path is built from), for tests
- * and roofline measurement:  C[b][cm(m)+cn(n)] = alpha * sum_k A[b][am(m)+ak(k)] B[b][bk(k)+bn(n)].
- * Every index map is two-level: idx -> (idx % n0)*s0 + (idx / n0)*s1, given as
- * {n0, s0, s1} int64 triples in `maps` in the order am, ak, bk, bn, cm, cn (18 values);
- * bs = batch strides of A, B, C.  All pointers device. */
+/* Stand-alone tensor-GEMM entry (the one contraction kernel the path is built from; PAPER.md:58-67
+ * Eqs. 4-7, :90 Eqs. 13-14 are all instances), for tests and roofline measurement:
+ *   C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)].
+ * Every index map is mixed radix over up to four tensor legs:
+ *   idx = d0 + n0*(d1 + n1*(d2 + n2*d3))  ->  d0*s0 + d1*s1 + d2*s2 + d3*s3   (element offsets),
+ * given as 7 int64 {n0, n1, n2, s0, s1, s2, s3} (radix <= 0 = unused level) in `maps` (host), in
+ * the order am, ak, bk, bn, cm, cn, ab, bb, cb (63 values; the last three map the batch index).
+ * A, B, C: device.  accumulate != 0: C += .  M, N >= 0, K >= 1, batch in 1..65535. */
 int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N, int K, int batch,
-                      const int64_t *maps, const int64_t *bs, double alpha);
+                      const int64_t *maps, double alpha, int accumulate);
+
+/* Thin QR with R_ii >= 0 of the row-major m x n matrix Y (device; m >= n, n <= 64): Q overwrites
+ * Y, R (n x n row-major upper triangular) goes to R (device).  The "QR decomposition in the RSVD"
+ * of PAPER.md:106 / the canonical form of PAPER.md:37 (Householder TSQR, robust to rank deficiency). */
+int tatrg_qr_pos(double *Y, int64_t m, int n, double *R);
+
+/* One-sided Jacobi SVD of the column-major m x n matrix G (device, ld = m): on exit G = U diag(s)
+ * with orthogonal columns sorted by decreasing norm, V (n x n column-major, device) such that
+ * G_in V = G_out, s (device, n) the singular values.  Also the symmetric PSD eigensolver
+ * (G symmetric: V = eigenvectors, s = eigenvalues).  PAPER.md:25 (RSVD core), Eq. 3, Eq. 12. */
+int tatrg_jacobi_svd(double *G, int m, int n, double *V, double *s);
+
+/* Norm / trace reductions of the normalisation and of tTr T = <Phi,Psi> (Eq. 15):
+ * out_dev[0] = sum x^2, resp. sum x*y; x *= 1/sqrt(*sumsq_dev).  All pointers device. */
+int tatrg_sumsq(const double *x, int64_t n, double *out_dev);
+int tatrg_dot(const double *x, const double *y, int64_t n, double *out_dev);
+int tatrg_scale_by_rsqrt(double *x, int64_t n, const double *sumsq_dev);
+
+/* Relative gaps (s[k-1]-s[k])/s[0] at the truncation cuts of the last step: bond swap,
+ * squeezers t1..t3 (inf when nothing was cut).  A cut through a degenerate cluster shows here. */
+int tatrg_get_gaps(double out[4]);
+/* High-water mark of workspace use in bytes since tatrg_set_workspace. */
+size_t tatrg_workspace_peak(void);
 
 const char *tatrg_last_error(void);
 void tatrg_destroy(void);

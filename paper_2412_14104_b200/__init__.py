@@ -1,0 +1,284 @@
+"""paper_2412_14104_b200 -- Triad-ATRG coarse-graining of the 4D Ising tensor network on one
+NVIDIA B200 (sm_100a), FP64.
+
+Thin ctypes binding of libtatrg.so (C-ABI: include/tatrg.h).  Argument marshalling only: every
+step of the path runs in the library's CUDA kernels.  PyTorch is used for device memory and
+streams.  There is no CPU fallback: importing works without a GPU (so that the symbols can be
+checked), but every compute call needs the CUDA library and a device, and fails loudly otherwise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtatrg.so")
+
+EXPORTS = [
+    "init_ising_tensor", "coarse_grain", "coarse_grain_atrg", "log_Z_per_site",
+    "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_peak",
+    "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
+    "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
+    "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
+    "tatrg_qr_pos", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
+    "tatrg_last_error", "tatrg_destroy",
+]
+
+SPECTRA = {"sigmaT": 0, "sigma_swap": 1, "SA": 2, "SX": 3, "SY": 4, "SD": 5, "s1": 6, "s2": 7, "s3": 8,
+           "ln_c": 9}
+
+_lib = None
+_keep = {}     # keeps the workspace / sketch tensors alive while the library points into them
+
+
+class TatrgError(RuntimeError):
+    pass
+
+
+def lib():
+    """Loads libtatrg.so (built in-tree by build.py / __graft_entry__.build()); no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise TatrgError("libtatrg.so is missing: run `python paper_2412_14104_b200/build.py` "
+                             "(there is no CPU fallback)")
+        L = ctypes.CDLL(_SO)
+        c_d, c_i, c_vp, c_sz = ctypes.c_double, ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t
+        c_i64, c_u64 = ctypes.c_int64, ctypes.c_uint64
+        sig = {
+            "init_ising_tensor": (c_i, [c_d, c_d]),
+            "coarse_grain": (c_i, [c_i, c_i, c_i, c_i, c_u64]),
+            "coarse_grain_atrg": (c_i, [c_i, c_i, c_i, c_i, c_u64]),
+            "log_Z_per_site": (c_d, []),
+            "tatrg_set_stream": (c_i, [c_vp]),
+            "tatrg_set_workspace": (c_i, [c_vp, c_sz]),
+            "tatrg_workspace_bytes": (c_sz, [c_i, c_i]),
+            "tatrg_workspace_peak": (c_sz, []),
+            "tatrg_set_sketch": (c_i, [c_i, c_vp, c_sz, c_i]),
+            "tatrg_sketch_shape": (c_i, [c_i, c_i, c_i, c_i, ctypes.POINTER(c_i64), ctypes.POINTER(c_i64)]),
+            "tatrg_get_spectrum": (c_i, [c_i, c_vp, c_i]),
+            "tatrg_get_gaps": (c_i, [c_vp]),
+            "tatrg_get_dims": (c_i, [c_vp]),
+            "tatrg_get_tensors": (c_i, [c_vp, c_vp, c_sz]),
+            "tatrg_order_parameter": (c_d, [c_i]),
+            "tatrg_get_stage_ms": (c_i, [c_vp, c_i]),
+            "tatrg_stage_name": (ctypes.c_char_p, [c_i]),
+            "tatrg_launch_count": (ctypes.c_longlong, [c_i]),
+            "tatrg_gemm_flops": (c_d, [c_i]),
+            "tatrg_probe_fp64_peak": (c_d, [c_i, c_i]),
+            "tatrg_tensor_gemm": (c_i, [c_vp, c_vp, c_vp, c_i, c_i, c_i, c_i, c_vp, c_d, c_i]),
+            "tatrg_qr_pos": (c_i, [c_vp, c_i64, c_i, c_vp]),
+            "tatrg_jacobi_svd": (c_i, [c_vp, c_i, c_i, c_vp, c_vp]),
+            "tatrg_sumsq": (c_i, [c_vp, c_i64, c_vp]),
+            "tatrg_dot": (c_i, [c_vp, c_vp, c_i64, c_vp]),
+            "tatrg_scale_by_rsqrt": (c_i, [c_vp, c_i64, c_vp]),
+            "tatrg_last_error": (ctypes.c_char_p, []),
+            "tatrg_destroy": (None, []),
+        }
+        for name, (res, args) in sig.items():
+            f = getattr(L, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        raise TatrgError("libtatrg error %d: %s" % (rc, lib().tatrg_last_error().decode()))
+
+
+def _require_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        raise TatrgError("no CUDA device: libtatrg has no CPU fallback")
+    return torch
+
+
+# ------------------------------------------------------------------ plumbing
+def set_workspace(nbytes: int | None = None, chi: int | None = None, r: int = 2, device="cuda:0"):
+    """Allocates the workspace as a torch tensor (PyTorch owns device memory) and hands it over."""
+    torch = _require_cuda()
+    if nbytes is None:
+        nbytes = int(lib().tatrg_workspace_bytes(int(chi), int(r)))
+    buf = torch.empty((nbytes + 255) // 256 * 32, dtype=torch.float64, device=device)
+    _keep["ws"] = buf
+    _check(lib().tatrg_set_workspace(buf.data_ptr(), buf.numel() * 8))
+    return buf
+
+
+def set_stream(stream=None):
+    torch = _require_cuda()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    _keep["stream"] = s
+    _check(lib().tatrg_set_stream(ctypes.c_void_p(s.cuda_stream)))
+
+
+def workspace_bytes(chi, r):
+    return int(lib().tatrg_workspace_bytes(int(chi), int(r)))
+
+
+def workspace_peak():
+    return int(lib().tatrg_workspace_peak())
+
+
+# ------------------------------------------------------------------ the three calls of the path
+def init_ising_tensor(beta: float, h: float = 0.0):
+    _require_cuda()
+    _check(lib().init_ising_tensor(float(beta), float(h)))
+
+
+def coarse_grain(direction: int, chi: int, r: int, q: int, seed: int):
+    _require_cuda()
+    _check(lib().coarse_grain(int(direction), int(chi), int(r), int(q), int(seed) & (2**64 - 1)))
+    for k in [k for k in _keep if isinstance(k, tuple)]:
+        del _keep[k]
+
+
+def coarse_grain_atrg(direction: int, chi: int, r: int, q: int, seed: int):
+    _require_cuda()
+    _check(lib().coarse_grain_atrg(int(direction), int(chi), int(r), int(q), int(seed) & (2**64 - 1)))
+    for k in [k for k in _keep if isinstance(k, tuple)]:
+        del _keep[k]
+
+
+def log_Z_per_site() -> float:
+    _require_cuda()
+    return float(lib().log_Z_per_site())
+
+
+# ------------------------------------------------------------------ inputs / outputs
+def set_sketch(which: int, data):
+    """data: torch CUDA float64 tensor (device pointer) or C-contiguous numpy / pinned CPU torch
+    tensor (host pointer, copied inside the next coarse_grain)."""
+    if isinstance(data, np.ndarray):
+        assert data.dtype == np.float64 and data.flags.c_contiguous
+        ptr, n, dev = data.ctypes.data, data.size, 0
+    else:
+        import torch
+        assert data.dtype == torch.float64 and data.is_contiguous()
+        ptr, n, dev = data.data_ptr(), data.numel(), int(data.is_cuda)
+    _keep[("sketch", which)] = data
+    _check(lib().tatrg_set_sketch(int(which), ctypes.c_void_p(ptr), n, dev))
+
+
+def sketch_shape(which, direction, chi, r):
+    rows, cols = ctypes.c_int64(0), ctypes.c_int64(0)
+    _check(lib().tatrg_sketch_shape(int(which), int(direction), int(chi), int(r),
+                                    ctypes.byref(rows), ctypes.byref(cols)))
+    return rows.value, cols.value
+
+
+def get_spectrum(which) -> np.ndarray:
+    w = SPECTRA[which] if isinstance(which, str) else int(which)
+    out = np.empty(8192)
+    n = lib().tatrg_get_spectrum(w, out.ctypes.data, out.size)
+    if n < 0:
+        _check(n)
+    return out[:n].copy()
+
+
+def get_gaps() -> np.ndarray:
+    out = np.empty(4)
+    _check(lib().tatrg_get_gaps(out.ctypes.data))
+    return out
+
+
+def get_dims():
+    out = np.zeros(6, dtype=np.int32)
+    _check(lib().tatrg_get_dims(out.ctypes.data))
+    return tuple(int(v) for v in out)
+
+
+def get_tensors():
+    d = get_dims()
+    shape = d[:5]
+    n = int(np.prod(shape))
+    phi, psi = np.empty(n), np.empty(n)
+    _check(lib().tatrg_get_tensors(phi.ctypes.data, psi.ctypes.data, n))
+    return phi.reshape(shape), psi.reshape(shape)
+
+
+def order_parameter(leg: int = 4) -> float:
+    return float(lib().tatrg_order_parameter(int(leg)))
+
+
+def stage_ms() -> dict:
+    out = np.zeros(16)
+    n = lib().tatrg_get_stage_ms(out.ctypes.data, out.size)
+    return {lib().tatrg_stage_name(i).decode(): float(out[i]) for i in range(n)}
+
+
+def launch_count(reset=False) -> int:
+    return int(lib().tatrg_launch_count(int(reset)))
+
+
+def gemm_flops(reset=False) -> float:
+    return float(lib().tatrg_gemm_flops(int(reset)))
+
+
+def probe_fp64_peak(mode: int, iters: int = 4096) -> float:
+    _require_cuda()
+    v = float(lib().tatrg_probe_fp64_peak(int(mode), int(iters)))
+    if v < 0:
+        raise TatrgError(lib().tatrg_last_error().decode())
+    return v
+
+
+# ------------------------------------------------------------------ stand-alone kernels
+def make_map(levels):
+    """levels: list of (size, stride), fastest first, at most 4.  -> 7 int64."""
+    assert 0 < len(levels) <= 4
+    n = [0, 0, 0]
+    s = [0, 0, 0, 0]
+    for i, (size, stride) in enumerate(levels):
+        s[i] = int(stride)
+        if i < 3 and i + 1 < len(levels):
+            n[i] = int(size)
+    return n + s
+
+
+def tensor_gemm(A, B, C, M, N, K, maps, batch=1, alpha=1.0, accumulate=False):
+    """maps: dict with keys am, ak, bk, bn, cm, cn (and optionally ab, bb, cb), each a list of
+    (size, stride) levels.  A, B, C: torch CUDA float64 tensors."""
+    _require_cuda()
+    flat = []
+    for key in ("am", "ak", "bk", "bn", "cm", "cn", "ab", "bb", "cb"):
+        flat += make_map(maps.get(key, [(1, 0)]))
+    arr = np.asarray(flat, dtype=np.int64)
+    _check(lib().tatrg_tensor_gemm(A.data_ptr(), B.data_ptr(), C.data_ptr(), int(M), int(N), int(K),
+                                   int(batch), arr.ctypes.data, float(alpha), int(accumulate)))
+
+
+def qr_pos(Y, R):
+    """In place: Y (m x n row-major CUDA tensor) <- Q; R (n x n) <- R with R_ii >= 0."""
+    _require_cuda()
+    m, n = Y.shape
+    _check(lib().tatrg_qr_pos(Y.data_ptr(), int(m), int(n), R.data_ptr()))
+
+
+def jacobi_svd(G, V, s):
+    """G: torch tensor holding a column-major m x n matrix as shape (n, m) row-major (row j = column j).
+    In place G <- U diag(s); V shape (n, n), row k = k-th right singular vector."""
+    _require_cuda()
+    n, m = G.shape
+    _check(lib().tatrg_jacobi_svd(G.data_ptr(), int(m), int(n), V.data_ptr(), s.data_ptr()))
+
+
+def sumsq(x, out):
+    _check(lib().tatrg_sumsq(x.data_ptr(), x.numel(), out.data_ptr()))
+
+
+def dot(x, y, out):
+    _check(lib().tatrg_dot(x.data_ptr(), y.data_ptr(), x.numel(), out.data_ptr()))
+
+
+def scale_by_rsqrt(x, ss):
+    _check(lib().tatrg_scale_by_rsqrt(x.data_ptr(), x.numel(), ss.data_ptr()))
+
+
+def destroy():
+    lib().tatrg_destroy()
+    _keep.clear()

@@ -1,0 +1,376 @@
+// api.cpp -- the C-ABI of libtatrg (include/tatrg.h): argument checking, the process-global
+// context, the caller-owned workspace (bump allocator), error reporting.
+#include <math.h>
+#include <stdarg.h>
+#include <string.h>
+
+#include "../../include/tatrg.h"
+#include "ctx.h"
+
+namespace tatrg {
+
+Ctx &ctx()
+{
+    static Ctx c;
+    return c;
+}
+
+cudaStream_t stream() { return ctx().stream; }
+void count_launch(int n) { ctx().launches += n; }
+void count_flops(double f) { ctx().flops += f; }
+
+int set_error(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    ctx().err = buf;
+    return code;
+}
+
+void fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof(buf), fmt, ap);
+    va_end(ap);
+    ctx().err = buf;
+    throw Err{code};
+}
+
+void *ws_alloc(size_t bytes)
+{
+    Ctx &c = ctx();
+    if (!c.ws) fail(TATRG_ESTATE, "no workspace set (tatrg_set_workspace)");
+    size_t b = (bytes + 255) & ~(size_t)255;
+    if (c.lo + b > c.hi)
+        fail(TATRG_ENOMEM, "workspace too small: need %zu more bytes (scratch %zu of %zu in use)", b, c.lo,
+             c.ws_bytes);
+    void *p = c.ws + c.lo;
+    c.lo += b;
+    size_t used = c.lo + (c.ws_bytes - c.hi);
+    if (used > c.peak) c.peak = used;
+    return p;
+}
+
+double *ws_doubles(long long n) { return (double *)ws_alloc(sizeof(double) * (size_t)(n > 0 ? n : 1)); }
+size_t ws_mark() { return ctx().lo; }
+void ws_release(size_t mark) { ctx().lo = mark; }
+
+namespace {
+
+// scratch region for the stand-alone entry points (tests, roofline measurements)
+void scratch_begin()
+{
+    Ctx &c = ctx();
+    if (!c.ws) fail(TATRG_ESTATE, "no workspace set (tatrg_set_workspace)");
+    if (c.inited) {
+        c.lo = c.state_low ? c.state_bytes : 0;
+        c.hi = c.state_low ? c.ws_bytes : c.ws_bytes - c.state_bytes;
+    } else {
+        c.lo = 0;
+        c.hi = c.ws_bytes;
+    }
+}
+
+template <class F>
+int guarded(F f)
+{
+    try {
+        f();
+        return TATRG_OK;
+    } catch (const Err &e) {
+        cudaGetLastError();
+        return e.code;
+    } catch (const std::exception &e) {
+        return set_error(TATRG_ENUM, "exception: %s", e.what());
+    }
+}
+
+Map4 map_from(const int64_t *m)
+{
+    Map4 r;
+    r.n0 = m[0] > 0 ? (unsigned)m[0] : TATRG_RADIX_INF;
+    r.n1 = m[1] > 0 ? (unsigned)m[1] : TATRG_RADIX_INF;
+    r.n2 = m[2] > 0 ? (unsigned)m[2] : TATRG_RADIX_INF;
+    r.pad = 0;
+    r.s0 = m[3];
+    r.s1 = m[4];
+    r.s2 = m[5];
+    r.s3 = m[6];
+    return r;
+}
+
+}  // namespace
+}  // namespace tatrg
+
+using namespace tatrg;
+
+extern "C" {
+
+int init_ising_tensor(double beta, double h)
+{
+    return guarded([&] { do_init(beta, h); });
+}
+
+int coarse_grain(int direction, int chi, int r, int q, uint64_t seed)
+{
+    int rc = guarded([&] { do_coarse_grain(direction, chi, r, q, seed, 0); });
+    for (auto &i : ctx().in) i = Input();
+    return rc;
+}
+
+int coarse_grain_atrg(int direction, int chi, int r, int q, uint64_t seed)
+{
+    int rc = guarded([&] { do_coarse_grain(direction, chi, r, q, seed, 1); });
+    for (auto &i : ctx().in) i = Input();
+    return rc;
+}
+
+double log_Z_per_site(void)
+{
+    double v = NAN;
+    guarded([&] { v = do_log_z(); });
+    return v;
+}
+
+int tatrg_set_stream(void *cuda_stream)
+{
+    ctx().stream = (cudaStream_t)cuda_stream;
+    return TATRG_OK;
+}
+
+int tatrg_set_workspace(void *dev_ptr, size_t bytes)
+{
+    Ctx &c = ctx();
+    if (!dev_ptr || ((uintptr_t)dev_ptr & 255) || bytes < 4096) return set_error(TATRG_EINVAL, "workspace must be a 256-byte aligned device buffer of >= 4096 bytes");
+    c.ws = (char *)dev_ptr;
+    c.ws_bytes = bytes & ~(size_t)255;
+    c.lo = 0;
+    c.hi = c.ws_bytes;
+    c.inited = false;   // the state lived in the old workspace
+    c.peak = 0;
+    return TATRG_OK;
+}
+
+size_t tatrg_workspace_bytes(int chi, int r)
+{
+    if (chi < 1 || r < 1) return 0;
+    // steady state, all legs = chi: a generous count of the live chi^5-sized tensors
+    // (state x2 generations, Q_Phi, Q_Psi, A, D, X, Y, Xs, Ys, G_ref, sketch + 3 RSVD blocks of
+    // r chi^5, TSQR stacks, P of r^2 chi^5, EM of r chi^5) plus the chi^4-sized Gram intermediates.
+    double c5 = pow((double)chi, 5), c4 = pow((double)chi, 4);
+    double doubles = c5 * (4 + 9 + 5.0 * r + 2.0 * r * r) + c4 * (16.0 * r * r + 64) + (1 << 22);
+    return (size_t)(doubles * 8.0 * 1.1) + ((size_t)64 << 20);
+}
+
+size_t tatrg_workspace_peak(void) { return ctx().peak; }
+
+int tatrg_set_sketch(int which, const double *data, size_t n, int on_device)
+{
+    if (which < 0 || which > 8) return set_error(TATRG_EINVAL, "tatrg_set_sketch: which must be 0..8");
+    Input &i = ctx().in[which];
+    i.ptr = data;
+    i.n = data ? n : 0;
+    i.on_device = on_device;
+    return TATRG_OK;
+}
+
+int tatrg_sketch_shape(int which, int direction, int chi, int r, int64_t *rows, int64_t *cols)
+{
+    Ctx &c = ctx();
+    if (!c.inited || which < 0 || which > 8 || direction < 1 || direction > 4 || !rows || !cols)
+        return set_error(TATRG_EINVAL, "tatrg_sketch_shape: bad arguments or not initialised");
+    int perm[4];
+    perm[0] = direction - 1;
+    for (int i = 0, j = 1; i < 4; ++i)
+        if (i != direction - 1) perm[j++] = i;
+    int64_t n0 = c.dims[perm[0]], n1 = c.dims[perm[1]], n2 = c.dims[perm[2]], n3 = c.dims[perm[3]];
+    int64_t a = c.bond, nT = n1 * n2 * n3, rc = (int64_t)r * chi;
+    *rows = *cols = 0;
+    if (which == 0) {
+        *rows = a * nT;
+        *cols = rc < a * nT ? rc : a * nT;
+    } else if (which <= 4) {
+        if (rc < n1 * n2) {
+            *rows = n1 * n2;
+            *cols = rc;
+        }
+    } else if (which == 5) {
+        *rows = n0 * nT;
+        *cols = a;
+    } else {
+        int64_t nn = which == 6 ? n1 : which == 7 ? n2 : n3;
+        *rows = nn * nn;
+        *cols = chi < nn * nn ? chi : nn * nn;
+    }
+    return TATRG_OK;
+}
+
+int tatrg_get_spectrum(int which, double *host_out, int cap)
+{
+    if (which < 0 || which > 9 || !host_out) return set_error(TATRG_EINVAL, "tatrg_get_spectrum: bad arguments");
+    const std::vector<double> &s = ctx().spec[which];
+    int n = (int)s.size() < cap ? (int)s.size() : cap;
+    for (int i = 0; i < n; ++i) host_out[i] = s[i];
+    return n;
+}
+
+int tatrg_get_gaps(double out[4])
+{
+    for (int i = 0; i < 4; ++i) out[i] = ctx().gaps[i];
+    return TATRG_OK;
+}
+
+int tatrg_get_dims(int dims_out[6])
+{
+    Ctx &c = ctx();
+    if (!c.inited) return set_error(TATRG_ESTATE, "not initialised");
+    for (int i = 0; i < 4; ++i) dims_out[i] = c.dims[i];
+    dims_out[4] = c.bond;
+    dims_out[5] = c.step;
+    return TATRG_OK;
+}
+
+int tatrg_get_tensors(double *phi_out, double *psi_out, size_t cap_each)
+{
+    Ctx &c = ctx();
+    if (!c.inited) return set_error(TATRG_ESTATE, "not initialised");
+    size_t n = (size_t)c.dims[0] * c.dims[1] * c.dims[2] * c.dims[3] * c.bond;
+    if (cap_each < n) return set_error(TATRG_EINVAL, "tatrg_get_tensors: need %zu doubles each", n);
+    return guarded([&] {
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(phi_out, c.phi, n * 8, cudaMemcpyDeviceToHost, c.stream));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(psi_out, c.psi, n * 8, cudaMemcpyDeviceToHost, c.stream));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(c.stream));
+    });
+}
+
+double tatrg_order_parameter(int leg)
+{
+    double v = NAN;
+    guarded([&] { v = do_order_parameter(leg); });
+    return v;
+}
+
+static const char *kStageNames[ST_COUNT] = {"canonical_form", "bond_swap",  "isometries", "triad_tensors",
+                                            "gram_chains",    "squeezers",  "contraction", "normalise"};
+
+int tatrg_get_stage_ms(double *host_out, int cap)
+{
+    int n = ST_COUNT < cap ? ST_COUNT : cap;
+    for (int i = 0; i < n; ++i) host_out[i] = ctx().stage_ms[i];
+    return ST_COUNT;
+}
+
+const char *tatrg_stage_name(int i) { return (i >= 0 && i < ST_COUNT) ? kStageNames[i] : ""; }
+
+long long tatrg_launch_count(int reset)
+{
+    long long v = ctx().launches;
+    if (reset) ctx().launches = 0;
+    return v;
+}
+
+double tatrg_gemm_flops(int reset)
+{
+    double v = ctx().flops;
+    if (reset) ctx().flops = 0;
+    return v;
+}
+
+double tatrg_probe_fp64_peak(int mode, int iters)
+{
+    double v = -1.0;
+    guarded([&] {
+        if (mode < 0 || mode > 2 || iters < 1) fail(TATRG_EINVAL, "tatrg_probe_fp64_peak: bad arguments");
+        scratch_begin();
+        v = probe_fp64_peak(mode, iters);
+    });
+    return v;
+}
+
+int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N, int K, int batch,
+                      const int64_t *maps, double alpha, int accumulate)
+{
+    return guarded([&] {
+        if (!A || !B || !C || !maps || M < 0 || N < 0 || K < 1 || batch < 1) fail(TATRG_EINVAL, "tatrg_tensor_gemm: bad arguments");
+        scratch_begin();
+        GemmParams p;
+        memset(&p, 0, sizeof(p));
+        p.A = A;
+        p.B = B;
+        p.C = C;
+        p.M = M;
+        p.N = N;
+        p.K = K;
+        p.batch = batch;
+        p.am = map_from(maps + 0);
+        p.ak = map_from(maps + 7);
+        p.bk = map_from(maps + 14);
+        p.bn = map_from(maps + 21);
+        p.cm = map_from(maps + 28);
+        p.cn = map_from(maps + 35);
+        p.ab = map_from(maps + 42);
+        p.bb = map_from(maps + 49);
+        p.cb = map_from(maps + 56);
+        p.alpha = alpha;
+        p.accumulate = accumulate;
+        p.a_kfast = llabs(p.ak.s0) < llabs(p.am.s0) || p.am.s0 == 0;
+        p.b_kfast = llabs(p.bk.s0) < llabs(p.bn.s0) || p.bn.s0 == 0;
+        tensor_gemm(p);
+    });
+}
+
+int tatrg_qr_pos(double *Y, int64_t m, int n, double *R)
+{
+    return guarded([&] {
+        if (!Y || !R || m < n) fail(TATRG_EINVAL, "tatrg_qr_pos: need m >= n >= 1");
+        scratch_begin();
+        tsqr(Y, m, n, R);
+    });
+}
+
+int tatrg_jacobi_svd(double *G, int m, int n, double *V, double *s)
+{
+    return guarded([&] {
+        if (!G || !V || !s) fail(TATRG_EINVAL, "tatrg_jacobi_svd: null pointer");
+        scratch_begin();
+        jacobi_svd(G, m, n, V, s, 1, 0, 0, 0);
+    });
+}
+
+int tatrg_sumsq(const double *x, int64_t n, double *out_dev)
+{
+    return guarded([&] {
+        scratch_begin();
+        sumsq(x, n, out_dev);
+    });
+}
+
+int tatrg_dot(const double *x, const double *y, int64_t n, double *out_dev)
+{
+    return guarded([&] {
+        scratch_begin();
+        dot(x, y, n, out_dev);
+    });
+}
+
+int tatrg_scale_by_rsqrt(double *x, int64_t n, const double *sumsq_dev)
+{
+    return guarded([&] { scale_by_rsqrt(x, n, sumsq_dev); });
+}
+
+const char *tatrg_last_error(void) { return ctx().err.c_str(); }
+
+void tatrg_destroy(void)
+{
+    Ctx &c = ctx();
+    if (c.ev_ok)
+        for (auto &e : c.ev) cudaEventDestroy(e);
+    c = Ctx();
+}
+
+}  // extern "C"

@@ -8,46 +8,60 @@
 
 namespace tatrg {
 
-// Two-level index map: idx -> (idx % n0) * s0 + (idx / n0) * s1   (element offsets).
-// Every leg permutation / leg grouping of the path's contractions is expressed with these,
-// so no transpose kernel ever runs.
-struct Map2 {
-    long long n0, s0, s1;
+// Mixed-radix index map: idx = d0 + n0*(d1 + n1*(d2 + n2*d3)) -> d0*s0 + d1*s1 + d2*s2 + d3*s3
+// (element offsets).  Every leg permutation / leg grouping of the path's contractions is
+// expressed with these, so no transpose kernel ever runs.
+// An unused level has radix RADIX_INF (its quotient is always 0).
+#define TATRG_RADIX_INF 0x7fffffffu
+struct Map4 {
+    unsigned n0, n1, n2, pad;
+    long long s0, s1, s2, s3;
 };
-__host__ __device__ inline long long map2(const Map2 &m, long long i)
-{
-    return (i % m.n0) * m.s0 + (i / m.n0) * m.s1;
-}
-// one-level map (stride s)
-inline Map2 M1(long long s) { return Map2{1LL << 40, s, 0}; }
-// two-level map: hi index (size irrelevant) stride s_hi, lo index of size n_lo stride s_lo
-inline Map2 M2(long long s_hi, long long n_lo, long long s_lo) { return Map2{n_lo, s_lo, s_hi}; }
 
+__host__ __device__ __forceinline__ long long map_off(const Map4 &m, unsigned i)
+{
+    unsigned q0 = i / m.n0;
+    long long off = (long long)(i - q0 * m.n0) * m.s0;
+    if (q0) {
+        unsigned q1 = q0 / m.n1;
+        off += (long long)(q0 - q1 * m.n1) * m.s1;
+        if (q1) {
+            unsigned q2 = q1 / m.n2;
+            off += (long long)(q1 - q2 * m.n2) * m.s2 + (long long)q2 * m.s3;
+        }
+    }
+    return off;
+}
+
+inline Map4 map1(long long s) { return Map4{TATRG_RADIX_INF, TATRG_RADIX_INF, TATRG_RADIX_INF, 0, s, 0, 0, 0}; }
+
+// C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)]
 struct GemmParams {
     const double *A;
     const double *B;
     double *C;
     int M, N, K, batch;
-    Map2 am, ak, bk, bn, cm, cn;
-    long long a_bs, b_bs, c_bs;
+    Map4 am, ak, bk, bn, cm, cn;
+    Map4 ab, bb, cb;       // batch index maps of A, B, C
     double alpha;
+    int accumulate;        // C += instead of C =
+    int a_kfast, b_kfast;  // loader thread order: 1 = consecutive threads walk k (k is the contiguous index)
     int ksplit;            // >1: partial sums go to `partial`, reduced by a second kernel
     int ktiles_per_split;  // in units of BK
     double *partial;       // [ksplit][batch][M][N]
 };
 
 // ---- context -------------------------------------------------------------------------
-struct Ctx;
-Ctx &ctx();
 cudaStream_t stream();
 void count_launch(int n = 1);
 void count_flops(double f);
 int set_error(int code, const char *fmt, ...);
-void *ws_alloc(size_t bytes);          // bump allocation from the caller's workspace (throws)
+void *ws_alloc(size_t bytes);          // bump allocation from the caller's workspace (throws Err)
+double *ws_doubles(long long n);
 size_t ws_mark();
 void ws_release(size_t mark);
 
-struct WsError {
+struct Err {
     int code;
 };
 
@@ -57,20 +71,41 @@ struct WsError {
         if (_e != cudaSuccess) {                                                       \
             ::tatrg::set_error(-5, "CUDA error %s at %s:%d", cudaGetErrorString(_e),   \
                                __FILE__, __LINE__);                                    \
-            throw ::tatrg::WsError{-5};                                                \
+            throw ::tatrg::Err{-5};                                                    \
         }                                                                              \
     } while (0)
+#define TATRG_LAUNCH_CHECK() TATRG_CUDA_CHECK(cudaGetLastError())
+
+[[noreturn]] void fail(int code, const char *fmt, ...);
 
 // ---- kernels (host launchers) ----------------------------------------------------------
 // gemm.cu
 void tensor_gemm(GemmParams p);
 double probe_fp64_peak(int mode, int iters);
-// small.cu
-void jacobi_svd(double *G, int ldg, int m, int n, double *V, int ldv, double *s, int *sweeps_out);
+// qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
+// Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).
+void tsqr(double *Y, long long m, int n, double *Rout);
+// jacobi.cu : one-sided Jacobi SVD of `batch` column-major m x n matrices (ld = m), m >= n.
+// On exit G = U*diag(s) (columns orthogonal, sorted by decreasing norm), V (n x n, column
+// major) accumulates the rotations (G_in * V = G_out), s[n] = column norms (descending).
+void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long long strideG,
+                long long strideV, long long strideS);
 // reduce.cu
 void sumsq(const double *x, long long n, double *out);                       // out[0] = sum x^2
 void dot(const double *x, const double *y, long long n, double *out);        // out[0] = sum x y
 void scale_by_rsqrt(double *x, long long n, const double *sumsq_dev);        // x *= 1/sqrt(*sumsq)
-void scale_cols(double *x, long long rows, int cols, const double *v, int inv); // x[r,c] *= v[c]
+// x[i, c] *= f(v[c]) for a row-major (rows x cols) array; mode 0: v, 1: 1/v, 2: sqrt(v), 3: 1/sqrt(v), 4: v^2
+void scale_cols(double *x, long long rows, int cols, const double *v, int mode);
+// x[r, c] *= f(v[r])
+void scale_rows(double *x, long long rows, long long cols, const double *v, int mode);
+// x[i] *= f(v[(i / inner) % n]) : scales a tensor along one leg (inner = its stride, n = its size);
+// mode 5: v^-3/2
+void scale_leg(double *x, long long total, long long inner, long long n, const double *v, int mode);
+void symmetrize(double *x, int n);                                            // x = (x + x^T)/2
+void fill_identity(double *x, int n);
+void fill_zero(double *x, long long n);
+void transpose_small(const double *in, double *out, int rows, int cols);      // out[c,r] = in[r,c]
+// gauge.cu
+void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);
 
 }  // namespace tatrg

@@ -1,0 +1,262 @@
+// qr.cu -- thin QR with R_ii >= 0 ("qr+", reading O9) of a tall row-major matrix,
+// as a communication-avoiding Householder TSQR: the "iterations of the QR decomposition in the
+// RSVD" of PAPER.md:106 and the canonical form of PAPER.md:37.
+//
+// Level 0 splits the m rows into blocks of RB rows; every CTA factors its RB x n block with
+// Householder reflections in shared memory (robust for rank-deficient blocks: tau = 0), leaves
+// the reflectors V in place of the block (stored transposed, [n][rows], so that the apply pass
+// reads v_j coalesced) and emits its n x n R.  The stacked R's are the next level's matrix.
+// Q is formed top-down: block b of level l applies its reflectors to [C_b; 0], C_b being rows
+// [b n, (b+1) n) of the level above; the top starts from diag(sign(R_jj)) so that R_ii >= 0.
+#include "common.h"
+
+namespace tatrg {
+
+namespace {
+
+constexpr int RB = 256;      // rows per block
+constexpr int QR_NT = 256;   // threads per CTA
+
+__device__ __forceinline__ double block_sum256(double v, double *sh)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    double r = 0.0;
+#pragma unroll
+    for (int i = 0; i < QR_NT / 32; ++i) r += sh[i];
+    return r;  // all threads
+}
+
+// X: rows x n row-major. Block b: rows [b*RB, ...).  Outputs: V^T in place ([n][rb]),
+// tau[b*n + j], Rst[b*n*n + i*n + c].
+template <int CW>
+__global__ void __launch_bounds__(QR_NT) tsqr_factor_kernel(double *__restrict__ X, long long rows, int n,
+                                                           double *__restrict__ tau,
+                                                           double *__restrict__ Rst)
+{
+    extern __shared__ double sm[];
+    const int ld = n | 1;
+    double *S = sm;                 // [RB][ld]
+    double *vbuf = S + RB * ld;     // [RB]
+    double *red = vbuf + RB;        // [QR_NT/CW][CW]
+    double *sc = red + QR_NT;       // scalars + reduction scratch [16]
+    constexpr int RG = QR_NT / CW;
+
+    const int t = threadIdx.x;
+    const long long r0 = (long long)blockIdx.x * RB;
+    const int rb = (int)min((long long)RB, rows - r0);
+    double *Xb = X + r0 * n;
+
+    for (int i = t; i < RB * n; i += QR_NT) {
+        int r = i / n, c = i - r * n;
+        S[r * ld + c] = (r < rb) ? Xb[i] : 0.0;
+    }
+    __syncthreads();
+
+    const int c = t % CW, rg = t / CW;
+    for (int j = 0; j < n; ++j) {
+        // (a) norm of the column below the diagonal
+        double x = (t > j) ? S[t * ld + j] : 0.0;
+        double xn2 = block_sum256(x * x, sc + 4);
+        double alpha = S[j * ld + j];
+        double beta, tj, scal;
+        if (xn2 == 0.0) {
+            beta = alpha;
+            tj = 0.0;
+            scal = 0.0;
+        } else {
+            beta = -copysign(sqrt(alpha * alpha + xn2), alpha);
+            tj = (beta - alpha) / beta;
+            scal = 1.0 / (alpha - beta);
+        }
+        __syncthreads();
+        // (c) reflector
+        {
+            double v = (t > j) ? x * scal : (t == j ? 1.0 : 0.0);
+            vbuf[t] = v;
+            if (t > j) S[t * ld + j] = v;
+            if (t == j) {
+                S[j * ld + j] = beta;
+                tau[(long long)blockIdx.x * n + j] = tj;
+            }
+        }
+        __syncthreads();
+        // (d) w = v^T S[:, j+1:]
+        const bool act = (c > j) && (c < n);
+        double part = 0.0;
+        if (act && tj != 0.0) {
+            for (int r = j + ((rg - j) % RG + RG) % RG; r < RB; r += RG) part = fma(vbuf[r], S[r * ld + c], part);
+        }
+        red[rg * CW + c] = part;
+        __syncthreads();
+        if (act && tj != 0.0) {
+            double w = 0.0;
+#pragma unroll
+            for (int g = 0; g < RG; ++g) w += red[g * CW + c];
+            w *= tj;
+            for (int r = j + ((rg - j) % RG + RG) % RG; r < RB; r += RG) S[r * ld + c] = fma(-vbuf[r], w, S[r * ld + c]);
+        }
+        __syncthreads();
+    }
+    // R block (upper triangle), then V^T over the block's own storage
+    double *Rb = Rst + (long long)blockIdx.x * n * n;
+    for (int i = t; i < n * n; i += QR_NT) {
+        int r = i / n, cc = i - r * n;
+        Rb[i] = (r <= cc) ? S[r * ld + cc] : 0.0;
+    }
+    for (int i = t; i < n * rb; i += QR_NT) {
+        int j = i / rb, r = i - j * rb;
+        Xb[i] = (r < j) ? 0.0 : (r == j ? 1.0 : S[r * ld + j]);
+    }
+}
+
+// Forms Q of one level in place of its V^T blocks.  Cup: the level above (row-major, n columns),
+// block b uses rows [b*n, (b+1)*n); if Cup == nullptr the block starts from diag(dsign).
+template <int CW>
+__global__ void __launch_bounds__(QR_NT) tsqr_apply_kernel(double *__restrict__ X, long long rows, int n,
+                                                          const double *__restrict__ tau,
+                                                          const double *__restrict__ Cup,
+                                                          const double *__restrict__ dsign)
+{
+    extern __shared__ double sm[];
+    const int ld = n | 1;
+    double *W = sm;                 // [RB][ld]
+    double *vbuf = W + RB * ld;     // [RB]
+    double *red = vbuf + RB;        // [RG][CW]
+    constexpr int RG = QR_NT / CW;
+
+    const int t = threadIdx.x;
+    const long long r0 = (long long)blockIdx.x * RB;
+    const int rb = (int)min((long long)RB, rows - r0);
+    double *Xb = X + r0 * n;
+
+    for (int i = t; i < RB * n; i += QR_NT) {
+        int r = i / n, cc = i - r * n;
+        double v = 0.0;
+        if (r < n) {
+            if (Cup)
+                v = Cup[(long long)blockIdx.x * n * n + i];
+            else
+                v = (r == cc) ? dsign[r] : 0.0;
+        }
+        W[r * ld + cc] = v;
+    }
+    const int c = t % CW, rg = t / CW;
+    const bool act = c < n;
+    for (int j = n - 1; j >= 0; --j) {
+        __syncthreads();
+        vbuf[t] = (t < rb) ? Xb[(long long)j * rb + t] : 0.0;
+        const double tj = tau[(long long)blockIdx.x * n + j];
+        __syncthreads();
+        if (tj == 0.0) continue;   // uniform across the block
+        double part = 0.0;
+        if (act)
+            for (int r = j + ((rg - j) % RG + RG) % RG; r < RB; r += RG) part = fma(vbuf[r], W[r * ld + c], part);
+        red[rg * CW + c] = part;
+        __syncthreads();
+        if (act) {
+            double w = 0.0;
+#pragma unroll
+            for (int g = 0; g < RG; ++g) w += red[g * CW + c];
+            w *= tj;
+            for (int r = j + ((rg - j) % RG + RG) % RG; r < RB; r += RG) W[r * ld + c] = fma(-vbuf[r], w, W[r * ld + c]);
+        }
+    }
+    __syncthreads();
+    for (int i = t; i < rb * n; i += QR_NT) {
+        int r = i / n, cc = i - r * n;
+        Xb[i] = W[r * ld + cc];
+    }
+}
+
+// dsign[j] = R_jj >= 0 ? 1 : -1 ; R <- diag(dsign) R
+__global__ void sign_fix_kernel(double *R, int n, double *dsign)
+{
+    __shared__ double d[128];
+    int t = threadIdx.x;
+    if (t < n) {
+        d[t] = (R[t * n + t] < 0.0) ? -1.0 : 1.0;
+        dsign[t] = d[t];
+    }
+    __syncthreads();
+    for (int i = t; i < n * n; i += blockDim.x) R[i] *= d[i / n];
+}
+
+size_t smem_for(int n) { return ((size_t)RB * (n | 1) + RB + QR_NT + 16) * sizeof(double); }
+
+template <int CW>
+void set_attrs()
+{
+    static bool done = false;
+    if (done) return;
+    TATRG_CUDA_CHECK(cudaFuncSetAttribute(tsqr_factor_kernel<CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)smem_for(CW)));
+    TATRG_CUDA_CHECK(cudaFuncSetAttribute(tsqr_apply_kernel<CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)smem_for(CW)));
+    done = true;
+}
+
+template <int CW>
+void tsqr_impl(double *Y, long long m, int n, double *Rout)
+{
+    set_attrs<CW>();
+    size_t mark = ws_mark();
+    struct Level {
+        double *X;
+        long long rows;
+        long long nb;
+        double *tau;
+        double *Rst;
+    };
+    std::vector<Level> lv;
+    double *X = Y;
+    long long rows = m;
+    const size_t smem = smem_for(n);
+    while (true) {
+        Level L;
+        L.X = X;
+        L.rows = rows;
+        L.nb = (rows + RB - 1) / RB;
+        L.tau = ws_doubles(L.nb * n);
+        L.Rst = ws_doubles(L.nb * n * n);
+        tsqr_factor_kernel<CW><<<(unsigned)L.nb, QR_NT, smem, stream()>>>(L.X, L.rows, n, L.tau, L.Rst);
+        TATRG_LAUNCH_CHECK();
+        count_launch();
+        lv.push_back(L);
+        if (L.nb == 1) break;
+        X = L.Rst;
+        rows = L.nb * n;
+    }
+    double *dsign = ws_doubles(n);
+    Level &top = lv.back();
+    sign_fix_kernel<<<1, 128, 0, stream()>>>(top.Rst, n, dsign);
+    count_launch();
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(Rout, top.Rst, sizeof(double) * n * n, cudaMemcpyDeviceToDevice, stream()));
+    for (int l = (int)lv.size() - 1; l >= 0; --l) {
+        Level &L = lv[l];
+        const double *Cup = (l == (int)lv.size() - 1) ? nullptr : lv[l + 1].X;
+        tsqr_apply_kernel<CW><<<(unsigned)L.nb, QR_NT, smem, stream()>>>(L.X, L.rows, n, L.tau, Cup, dsign);
+        TATRG_LAUNCH_CHECK();
+        count_launch();
+    }
+    ws_release(mark);
+}
+
+}  // namespace
+
+void tsqr(double *Y, long long m, int n, double *Rout)
+{
+    if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");
+    if (n > 64) fail(-22, "tsqr: n = %d > 64 not supported yet", n);
+    if (n > 32)
+        tsqr_impl<64>(Y, m, n, Rout);
+    else if (n > 16)
+        tsqr_impl<32>(Y, m, n, Rout);
+    else
+        tsqr_impl<16>(Y, m, n, Rout);
+}
+
+}  // namespace tatrg

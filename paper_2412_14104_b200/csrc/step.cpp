@@ -1,0 +1,664 @@
+// step.cpp -- host orchestration of one Triad-ATRG coarse-graining step (arXiv:2412.14104,
+// /root/reference/PAPER.md Sec. 2): which kernels run, on which strided views, in which order.
+// All arithmetic on tensors runs in the CUDA kernels (gemm.cu, qr.cu, jacobi.cu, reduce.cu,
+// gauge.cu); the host takes the rank / cluster decisions on downloaded spectra (O(chi) scalars)
+// and keeps the ln Z bookkeeping.
+//
+// Rotated frame (reading G8): legs (0 | 1, 2 | 3) = (coarse-graining direction |
+// grouped transverse pair | lone transverse leg).  Leg letters used in the contractions below:
+//   x,c  direction-0 legs        p,q / P,Q  pair legs of the upper / lower site
+//   t / T  lone leg upper / lower   a,b  canonical bonds alpha, beta   g,d  swap bond gamma
+//   k,l  oversampled internal lines (r chi)   m,n,w  renormalised legs   z  sketch columns
+#include <math.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "ctx.h"
+
+extern "C" {
+uint64_t si_subseed(uint64_t seed, uint64_t step, uint64_t which);
+void si_fill_gauss(double *out, uint64_t n, uint64_t subseed, uint64_t offset);
+}
+
+namespace tatrg {
+
+namespace {
+
+constexpr double RANK_TOL = 1e-14;     // reading G9
+constexpr double CLUSTER_TOL = 1e-8;   // reading G12
+
+std::vector<double> d2h(const double *p, long long n)
+{
+    std::vector<double> v((size_t)n);
+    if (n > 0) {
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(v.data(), p, sizeof(double) * n, cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    }
+    return v;
+}
+
+void h2d(double *dst, const double *src, long long n)
+{
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(dst, src, sizeof(double) * n, cudaMemcpyHostToDevice, stream()));
+}
+
+void d2d(double *dst, const double *src, long long n)
+{
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(dst, src, sizeof(double) * n, cudaMemcpyDeviceToDevice, stream()));
+}
+
+int num_rank(const std::vector<double> &s, int cap)
+{
+    if (s.empty() || !(s[0] > 0)) return 0;
+    int k = 0;
+    for (double v : s) k += (v > RANK_TOL * s[0]);
+    return cap >= 0 ? std::min(cap, k) : k;
+}
+
+double rel_gap(const std::vector<double> &s, int cut)
+{
+    if (cut <= 0 || cut >= (int)s.size()) return INFINITY;
+    return (s[cut - 1] - s[cut]) / s[0];
+}
+
+// cluster boundaries of the first k values of the descending s
+std::vector<int> cluster_bounds(const std::vector<double> &s, int k)
+{
+    std::vector<int> b{0};
+    for (int i = 1; i < k; ++i)
+        if (s[i - 1] - s[i] > CLUSTER_TOL * s[0]) b.push_back(i);
+    b.push_back(k);
+    return b;
+}
+
+// W (k x k, row-major, device) = blockdiag of qr+ of the diagonal cluster blocks of P (k x k)
+Ten gauge_rotation(const Ten &P, const std::vector<double> &s, int k)
+{
+    std::vector<int> b = cluster_bounds(s, k);
+    for (size_t i = 0; i + 1 < b.size(); ++i)
+        if (b[i + 1] - b[i] > 32) fail(-34, "gauge fixing: degenerate cluster of %d values (max 32)", b[i + 1] - b[i]);
+    int *bd = (int *)ws_alloc(sizeof(int) * b.size());
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(bd, b.data(), sizeof(int) * b.size(), cudaMemcpyHostToDevice, stream()));
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));  // b is a local
+    Ten W = ws_tensor("ab", {k, k});
+    cluster_qr(P.p, k, W.p, k, bd, (int)b.size() - 1);
+    return W;
+}
+
+struct StepCfg {
+    uint64_t seed;
+    int step;
+};
+
+// Seeded Gaussian input `which` (rows x cols, row-major): the caller's buffer if one of the right
+// size was set, else generated here with the shared generator (sub-seed recipe of DESIGN.md).
+Ten get_input(int which, long long rows, long long cols, const StepCfg &cfg, const char *names2)
+{
+    Ctx &c = ctx();
+    long long n = rows * cols;
+    Ten t;
+    Input &in = c.in[which];
+    if (in.ptr && in.n == (size_t)n) {
+        if (in.on_device) {
+            t = Ten::make(const_cast<double *>(in.ptr), names2, {rows, cols});
+        } else {
+            t = ws_tensor(names2, {rows, cols});
+            h2d(t.p, in.ptr, n);
+        }
+        return t;
+    }
+    std::vector<double> host((size_t)n);
+    uint64_t st = (which >= 5) ? 0 : (uint64_t)cfg.step;   // gauge references are step independent
+    si_fill_gauss(host.data(), (uint64_t)n, si_subseed(cfg.seed, st, (uint64_t)which), 0);
+    t = ws_tensor(names2, {rows, cols});
+    h2d(t.p, host.data(), n);
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    return t;
+}
+
+void stage_mark(int i)
+{
+    Ctx &c = ctx();
+    if (!c.ev_ok) {
+        for (auto &e : c.ev) TATRG_CUDA_CHECK(cudaEventCreate(&e));
+        c.ev_ok = true;
+    }
+    TATRG_CUDA_CHECK(cudaEventRecord(c.ev[i], c.stream));
+}
+
+// Symmetric PSD eigenproblem of the n x n matrix S (overwritten): on exit the rows of Vt
+// (row-major n x n) are the eigenvectors, lam (device, n) descending; returns lam on the host.
+std::vector<double> sym_eig(double *S, int n, double *Vt, double *lam)
+{
+    symmetrize(S, n);
+    jacobi_svd(S, n, n, Vt, lam, 1, 0, 0, 0);
+    return d2h(lam, n);
+}
+
+// ---------------------------------------------------------------------------------------
+// RSVD by subspace iteration (reading O9).  apply / apply_t map a
+// (cols x z) block to (rows x z) and back.  Returns Q u[:, :k], s, Q_B v[:, :k].
+struct RsvdOut {
+    int k;
+    std::vector<double> s_full;
+    double *s_dev;
+};
+
+template <class F1, class F2>
+RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long cols, int ell, int q, int keep,
+             double *left, double *right)
+{
+    double *Rtmp = ws_doubles((long long)ell * ell);
+    Ten Yb = ws_tensor("rz", {rows, ell});
+    Ten Yt = ws_tensor("rz", {cols, ell});
+    apply(omega.p, Yb.p);
+    tsqr(Yb.p, rows, ell, Rtmp);
+    for (int it = 0; it < q; ++it) {
+        apply_t(Yb.p, Yt.p);
+        tsqr(Yt.p, cols, ell, Rtmp);
+        apply(Yt.p, Yb.p);
+        tsqr(Yb.p, rows, ell, Rtmp);
+    }
+    apply_t(Yb.p, Yt.p);             // B^T = Op^T Q
+    double *Rb = ws_doubles((long long)ell * ell);
+    tsqr(Yt.p, cols, ell, Rb);       // B^T = Q_B R_B; the row-major R_B buffer is R_B^T column-major
+    double *V = ws_doubles((long long)ell * ell);
+    double *s = ws_doubles(ell);
+    jacobi_svd(Rb, ell, ell, V, s, 1, 0, 0, 0);   // R_B^T V = U diag(s)
+    RsvdOut out;
+    out.s_full = d2h(s, ell);
+    out.s_dev = s;
+    out.k = num_rank(out.s_full, keep);
+    const int k = out.k;
+    if (k < 1) fail(-34, "rsvd: operator is numerically zero");
+    scale_leg(Rb, (long long)k * ell, ell, k, s, 1);   // columns of U
+    Ten U = Ten::make(Rb, "gz", {ell, ell});           // [g][z] = U[z, g]
+    Ten Vv = Ten::make(V, "gz", {ell, ell});
+    Ten Uk = U, Vk = Vv;
+    Uk.legs[0].n = k;
+    Vk.legs[0].n = k;
+    contract(Yb, Uk, Ten::make(left, "rg", {rows, k}));
+    contract(Yt, Vk, Ten::make(right, "rg", {cols, k}));
+    return out;
+}
+
+}  // namespace
+
+// =======================================================================================
+void do_init(double beta, double h)
+{
+    Ctx &c = ctx();
+    if (!(beta > 0) || !std::isfinite(beta) || !std::isfinite(h)) fail(-22, "init_ising_tensor: beta must be finite and > 0, h finite");
+    if (!c.ws) fail(-1, "init_ising_tensor: no workspace set");
+    // PAPER.md:128-137 Eqs. 16-17, readings G1 (square roots) and G2 (field weight)
+    double W[2][2];
+    const double sgn[2] = {1.0, -1.0};
+    for (int a = 0; a < 2; ++a) {
+        W[a][0] = sqrt(cosh(beta));
+        W[a][1] = sgn[a] * sqrt(sinh(beta));
+    }
+    std::vector<double> phi(32), psi(32);
+    for (int i = 0; i < 16; ++i)
+        for (int a = 0; a < 2; ++a) {
+            double v = 1.0;
+            for (int mu = 0; mu < 4; ++mu) v *= W[a][(i >> (3 - mu)) & 1];
+            phi[i * 2 + a] = v;
+            psi[i * 2 + a] = v * exp(beta * h * sgn[a]);
+        }
+    c.lo = 0;
+    c.hi = c.ws_bytes;
+    c.state_low = true;
+    c.state_bytes = 512;
+    if (c.ws_bytes < 4096) fail(-12, "workspace too small");
+    c.phi = (double *)c.ws;
+    c.psi = c.phi + 32;
+    h2d(c.phi, phi.data(), 32);
+    h2d(c.psi, psi.data(), 32);
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    for (int i = 0; i < 4; ++i) c.dims[i] = 2;
+    c.bond = 2;
+    c.step = 0;
+    c.log_acc = 0.0;
+    c.beta = beta;
+    c.h = h;
+    // normalise (reading O8): c_0 = |Phi||Psi|
+    c.lo = c.state_bytes;
+    double *ss = ws_doubles(2);
+    sumsq(c.phi, 32, ss);
+    sumsq(c.psi, 32, ss + 1);
+    scale_by_rsqrt(c.phi, 32, ss);
+    scale_by_rsqrt(c.psi, 32, ss + 1);
+    std::vector<double> v = d2h(ss, 2);
+    c.log_acc = 0.5 * (log(v[0]) + log(v[1]));
+    for (auto &s : c.spec) s.clear();
+    for (auto &i : c.in) i = Input();
+    c.inited = true;
+}
+
+double do_log_z()
+{
+    Ctx &c = ctx();
+    if (!c.inited) return NAN;
+    c.lo = c.state_low ? c.state_bytes : 0;
+    c.hi = c.state_low ? c.ws_bytes : c.ws_bytes - c.state_bytes;
+    long long n = (long long)c.dims[0] * c.dims[1] * c.dims[2] * c.dims[3] * c.bond;
+    double *o = ws_doubles(1);
+    dot(c.phi, c.psi, n, o);
+    double t = d2h(o, 1)[0];
+    if (!(t > 0)) return NAN;
+    return c.log_acc + ldexp(1.0, -c.step) * log(t);
+}
+
+// X^(m) = (Tr A)^2 / Tr(A^2), A_kl = sum T_{..k..;..l..}
+double do_order_parameter(int leg)
+{
+    Ctx &c = ctx();
+    if (!c.inited || leg < 1 || leg > 4) return NAN;
+    c.lo = c.state_low ? c.state_bytes : 0;
+    c.hi = c.state_low ? c.ws_bytes : c.ws_bytes - c.state_bytes;
+    const char *names[4] = {"kuvwg", "ukvwg", "uvkwg", "uvwkg"};
+    const char *namel[4] = {"luvwg", "ulvwg", "uvlwg", "uvwlg"};
+    Ten phi = Ten::make(c.phi, names[leg - 1], {c.dims[0], c.dims[1], c.dims[2], c.dims[3], c.bond});
+    Ten psi = Ten::make(c.psi, namel[leg - 1], {c.dims[0], c.dims[1], c.dims[2], c.dims[3], c.bond});
+    int n = c.dims[leg - 1];
+    Ten Am = ws_tensor("kl", {n, n});
+    contract(phi, psi, Am);
+    Ten A2 = ws_tensor("km", {n, n});
+    contract(Am, Am.as("lm"), A2);
+    std::vector<double> a = d2h(Am.p, (long long)n * n), a2 = d2h(A2.p, (long long)n * n);
+    double tr = 0, tr2 = 0;
+    for (int i = 0; i < n; ++i) {
+        tr += a[(size_t)i * n + i];
+        tr2 += a2[(size_t)i * n + i];
+    }
+    return tr * tr / tr2;
+}
+
+// =======================================================================================
+void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mode)
+{
+    Ctx &c = ctx();
+    if (!c.inited) fail(-1, "coarse_grain: call init_ising_tensor first");
+    if (direction < 1 || direction > 4 || chi < 1 || r < 1 || q < 0) fail(-22, "coarse_grain: bad arguments");
+    if ((long long)r * chi > 64) fail(-22, "coarse_grain: r*chi = %d > 64 not supported yet", r * chi);
+    StepCfg cfg{seed, c.step};
+
+    // ---- frames (reading G8)
+    int perm[4];
+    perm[0] = direction - 1;
+    for (int i = 0, j = 1; i < 4; ++i)
+        if (i != direction - 1) perm[j++] = i;
+    long long sd[4];   // strides of the standard layout [d1,d2,d3,d4,bond]
+    const int g0 = c.bond;
+    sd[3] = g0;
+    for (int i = 2; i >= 0; --i) sd[i] = sd[i + 1] * c.dims[i + 1];
+    const long long n0 = c.dims[perm[0]], n1 = c.dims[perm[1]], n2 = c.dims[perm[2]], n3 = c.dims[perm[3]];
+    const long long R = n0 * n1 * n2 * n3, nT = n1 * n2 * n3, n12 = n1 * n2;
+    auto rot_view = [&](double *p, long long bond) {
+        Ten t;
+        t.p = p;
+        for (int i = 0; i < 4; ++i) t.legs.push_back(Leg{'?', (long long)c.dims[perm[i]], sd[perm[i]] / g0 * bond});
+        t.legs.push_back(Leg{'?', bond, 1});
+        return t;
+    };
+
+    // ---- workspace: new state at the end opposite to the current one
+    const long long m1cap = std::min<long long>(chi, n1 * n1), m2cap = std::min<long long>(chi, n2 * n2),
+                    m3cap = std::min<long long>(chi, n3 * n3), gcap = std::min<long long>(chi, g0 * nT);
+    const size_t new_cap = (((size_t)(n0 * m1cap * m2cap * m3cap * gcap) * 8 + 255) / 256) * 256;
+    double *phi_new, *psi_new;
+    if (c.state_low) {
+        c.lo = c.state_bytes;
+        c.hi = c.ws_bytes;
+        if (c.hi < c.lo + 2 * new_cap) fail(-12, "workspace too small for the new state");
+        c.hi -= 2 * new_cap;
+        phi_new = (double *)(c.ws + c.hi);
+    } else {
+        c.lo = 0;
+        c.hi = c.ws_bytes - c.state_bytes;
+        if (c.hi < 2 * new_cap) fail(-12, "workspace too small for the new state");
+        phi_new = (double *)(c.ws + c.lo);
+        c.lo += 2 * new_cap;
+    }
+    psi_new = phi_new + new_cap / 8;
+    c.peak = std::max(c.peak, c.lo + (c.ws_bytes - c.hi));
+    std::vector<double> spec[10];
+    double gaps[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
+
+    stage_mark(0);
+    // =================== O2 canonical form ===================
+    Ten Qp = ws_tensor("rg", {R, g0}), Qs = ws_tensor("rg", {R, g0});
+    d2d(Qp.p, c.phi, R * g0);
+    d2d(Qs.p, c.psi, R * g0);
+    Ten Rp = ws_tensor("gr", {g0, g0}), Rs = ws_tensor("hr", {g0, g0});
+    tsqr(Qp.p, R, g0, Rp.p);
+    tsqr(Qs.p, R, g0, Rs.p);
+    // C = R_Phi R_Psi^T, stored transposed ([h][g]) so that the buffer is column-major C
+    Ten Cm = ws_tensor("hg", {g0, g0});
+    contract(Rs, Rp, Cm);
+    Ten Vc = ws_tensor("ah", {g0, g0});    // rows = right singular vectors v_a[h]
+    double *sT = ws_doubles(g0);
+    jacobi_svd(Cm.p, g0, g0, Vc.p, sT, 1, 0, 0, 0);   // C V = U diag(sT); Cm rows -> u_a[g] sT_a
+    spec[0] = d2h(sT, g0);
+    const int a = num_rank(spec[0], -1);
+    if (a < 1) fail(-34, "coarse_grain: tensor is numerically zero");
+    spec[0].resize(a);
+    scale_leg(Cm.p, (long long)a * g0, g0, a, sT, 1);
+    Ten u = Ten::make(Cm.p, "ag", {a, g0});   // u[a][g] = u_a[g]
+    Ten v = Ten::make(Vc.p, "ah", {a, g0});
+    // gauge (reading G12): P = A^T G_ref = u^T (Q_Phi^T G_ref)
+    Ten QpR = rot_view(Qp.p, g0), QsR = rot_view(Qs.p, g0);
+    Ten ref = get_input(5, R, a, cfg, "rb");
+    Ten ref5 = Ten::make(ref.p, "xpqtb", {n0, n1, n2, n3, a});
+    Ten T1 = ws_tensor("gb", {g0, a});
+    contract(QpR.as("xpqtg"), ref5, T1);
+    Ten Pg = ws_tensor("ab", {a, a});
+    contract(u, T1, Pg);
+    Ten Wg = gauge_rotation(Pg, spec[0], a);
+    Ten u2 = ws_tensor("bg", {a, g0}), v2 = ws_tensor("bg", {a, g0});
+    contract(Wg, u, u2);                    // u2[b][g] = sum_a W[a,b] u[a][g]
+    contract(Wg, v.as("ag"), v2);
+    Ten A = ws_tensor("xpqta", {n0, n1, n2, n3, a}), D = ws_tensor("xpqta", {n0, n1, n2, n3, a});
+    contract(QpR.as("xpqtg"), u2.as("ag"), A);
+    contract(QsR.as("xpqtg"), v2.as("ag"), D);
+    stage_mark(1);
+
+    // =================== O3 bond swap (Table 1 row 1) ===================
+    const long long dim = a * nT;
+    const int ell = (int)std::min<long long>((long long)r * chi, dim);
+    Ten omega = get_input(0, dim, ell, cfg, "rz");
+    Ten Z = ws_tensor("cabz", {n0, a, a, ell});
+    auto sw_apply = [&](const double *w, double *out) {   // M w : [(b,J), z] -> [(a,I'), z]
+        contract(D.as("cuvwa"), Ten::make(const_cast<double *>(w), "buvwz", {a, n1, n2, n3, ell}), Z);
+        scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+        scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+        contract(A.as("cpqtb"), Z, Ten::make(out, "apqtz", {a, n1, n2, n3, ell}));
+    };
+    auto sw_apply_t = [&](const double *w, double *out) {  // M^T w : [(a,I'), z] -> [(b,J), z]
+        contract(A.as("cpqtb"), Ten::make(const_cast<double *>(w), "apqtz", {a, n1, n2, n3, ell}), Z.as("cbaz"));
+        scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+        scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+        contract(D.as("cuvwa"), Z.as("cbaz"), Ten::make(out, "buvwz", {a, n1, n2, n3, ell}));
+    };
+    double *Xbuf = ws_doubles(dim * std::min<long long>(chi, ell));
+    double *Ybuf = ws_doubles(dim * std::min<long long>(chi, ell));
+    int gs;
+    double *sig;
+    {
+        size_t mk = ws_mark();
+        RsvdOut ro = rsvd(sw_apply, sw_apply_t, omega, dim, dim, ell, q, chi, Xbuf, Ybuf);
+        gs = ro.k;
+        spec[1].assign(ro.s_full.begin(), ro.s_full.begin() + gs);
+        gaps[0] = rel_gap(ro.s_full, gs);
+        std::vector<double> keep(ro.s_full.begin(), ro.s_full.begin() + gs);
+        ws_release(mk);
+        sig = ws_doubles(gs);
+        h2d(sig, keep.data(), gs);
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    }
+    Ten X = Ten::make(Xbuf, "apqtg", {a, n1, n2, n3, gs});
+    Ten Y = Ten::make(Ybuf, "buvwg", {a, n1, n2, n3, gs});
+    Ten Xs = ws_tensor("apqtg", {a, n1, n2, n3, gs}), Ys = ws_tensor("buvwg", {a, n1, n2, n3, gs});
+    d2d(Xs.p, X.p, X.size());
+    d2d(Ys.p, Y.p, Y.size());
+    scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
+    scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
+    stage_mark(2);
+
+    if (mode != 0) fail(-22, "coarse_grain_atrg: not implemented yet");
+
+    // =================== O4 oversampled isometries (Eqs. 2-3) ===================
+    const int kk = (int)std::min<long long>((long long)r * chi, n12);
+    Ten U[4];   // A, X, Y, D : [p,q,k]
+    if (kk >= n12) {
+        for (int i = 0; i < 4; ++i) {
+            U[i] = ws_tensor("pqk", {n1, n2, n12});
+            fill_identity(U[i].p, (int)n12);
+        }
+    } else {
+        Ten RX = ws_tensor("ab", {a, a}), RY = ws_tensor("ab", {a, a});
+        contract(Xs.as("apqtg"), Xs.as("bpqtg"), RX);
+        contract(Ys.as("apqtg"), Ys.as("bpqtg"), RY);
+        for (int i = 0; i < 4; ++i) {
+            // the symmetric PSD operator S = K K_w^T on the pair space (reading G6b)
+            const Ten &Kt = (i == 0) ? A : (i == 1) ? Xs : (i == 2) ? Ys : D;
+            const bool mid = (i == 0 || i == 3);
+            const Ten &Rm = (i == 0) ? RX : RY;
+            const long long e0 = Kt.legs[0].n, e3 = Kt.legs[3].n, e4 = Kt.legs[4].n;
+            Ten t1 = ws_tensor("xtaz", {e0, e3, e4, kk}), t2 = ws_tensor("xtbz", {e0, e3, e4, kk});
+            auto S_op = [&](const double *w, double *out) {
+                contract(Kt.as("xpqta"), Ten::make(const_cast<double *>(w), "pqz", {n1, n2, kk}), t1);
+                if (mid) {
+                    contract(t1, Rm, t2);
+                    contract(Kt.as("xpqtb"), t2, Ten::make(out, "pqz", {n1, n2, kk}));
+                } else {
+                    contract(Kt.as("xpqta"), t1, Ten::make(out, "pqz", {n1, n2, kk}));
+                }
+            };
+            Ten om = get_input(1 + i, n12, kk, cfg, "rz");
+            Ten Qi = ws_tensor("rz", {n12, kk}), SQ = ws_tensor("ry", {n12, kk});
+            double *Rtmp = ws_doubles((long long)kk * kk);
+            S_op(om.p, Qi.p);
+            tsqr(Qi.p, n12, kk, Rtmp);
+            for (int it = 0; it < q; ++it) {
+                S_op(Qi.p, SQ.p);
+                d2d(Qi.p, SQ.p, n12 * kk);
+                tsqr(Qi.p, n12, kk, Rtmp);
+            }
+            S_op(Qi.p, SQ.p);
+            Ten Hm = ws_tensor("zy", {kk, kk});
+            contract(Qi, SQ, Hm);
+            Ten Vt = ws_tensor("kz", {kk, kk});
+            double *lam = ws_doubles(kk);
+            std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);
+            spec[2 + i].resize(kk);
+            for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
+            U[i] = ws_tensor("pqk", {n1, n2, kk});
+            contract(Ten::make(Qi.p, "pqz", {n1, n2, kk}), Vt, U[i]);
+        }
+    }
+    const long long kd = U[0].legs[2].n;
+    stage_mark(3);
+
+    // =================== O5 triad tensors (Eqs. 4-7) ===================
+    Ten E = ws_tensor("xkta", {n0, kd, n3, a}), F = ws_tensor("aktg", {a, kd, n3, gs});
+    Ten G = ws_tensor("bktg", {a, kd, n3, gs}), H = ws_tensor("xktb", {n0, kd, n3, a});
+    contract(A.as("xpqta"), U[0], E);
+    contract(Xs.as("apqtg"), U[1], F);     // sigma is inside Xs (Eq. 5)
+    contract(Y.as("bpqtg"), U[2], G);
+    contract(D.as("xpqtb"), U[3], H);
+    stage_mark(4);
+
+    // =================== O6 Gram matrices of Gamma^triad (Eq. 12) ===================
+    Ten GL[3], GR[3];
+    const long long nn[3] = {n1, n2, n3};
+    for (int mu = 0; mu < 3; ++mu) {
+        GL[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
+        GR[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
+    }
+    {
+        size_t mk = ws_mark();
+        Ten HH0 = ws_tensor("bc", {a, a}), EE0 = ws_tensor("ab", {a, a});
+        contract(H.as("xktb"), H.as("xktc"), HH0);
+        contract(E.as("xkta"), E.as("xktb"), EE0);
+        Ten Gh = ws_tensor("cktg", {a, kd, n3, gs}), Fh = ws_tensor("bktg", {a, kd, n3, gs});
+        contract(HH0, G.as("bktg"), Gh);
+        contract(EE0, F.as("aktg"), Fh);
+        Ten Sm = ws_tensor("gd", {gs, gs}), Sp = ws_tensor("gd", {gs, gs});
+        contract(Gh, G.as("cktd"), Sm);    // "-" half reduced to the swap bond
+        contract(Fh, F.as("bktd"), Sp);    // "+" half
+        Ten Fs = Fh, Gs = Gh;              // reuse: Fs[b,k,u,g] = sum_d F[b,k,u,d] Sm[g,d]
+        contract(F.as("bkud"), Sm, Fs.as("bkug"));
+        contract(G.as("ckud"), Sp, Gs.as("ckug"));
+        {   // lone leg
+            size_t mk2 = ws_mark();
+            Ten EE3 = ws_tensor("taub", {n3, a, n3, a}), FF3 = ws_tensor("asbv", {a, n3, a, n3});
+            contract(E.as("xkta"), E.as("xkub"), EE3);
+            contract(F.as("aksg"), Fs.as("bkvg"), FF3);
+            contract(EE3, FF3, GL[2].as("tsuv"));
+            Ten GG3 = ws_tensor("btcu", {a, n3, a, n3}), HH3 = ws_tensor("sbvc", {n3, a, n3, a});
+            contract(G.as("bktg"), Gs.as("ckug"), GG3);
+            contract(H.as("xksb"), H.as("xkvc"), HH3);
+            contract(GG3, HH3, GR[2].as("tsuv"));
+            ws_release(mk2);
+        }
+        Ten EEk = ws_tensor("kalb", {kd, a, kd, a}), FFk = ws_tensor("kalb", {kd, a, kd, a});
+        Ten GGk = ws_tensor("kblc", {kd, a, kd, a}), HHk = ws_tensor("kblc", {kd, a, kd, a});
+        contract(E.as("xkta"), E.as("xltb"), EEk);
+        contract(F.as("aktg"), Fs.as("bltg"), FFk);
+        contract(G.as("bktg"), Gs.as("cltg"), GGk);
+        contract(H.as("xktb"), H.as("xltc"), HHk);
+        for (int mu = 0; mu < 2; ++mu) {
+            size_t mk2 = ws_mark();
+            const char *n1s = mu == 0 ? "pqk" : "qpk", *n2s = mu == 0 ? "rql" : "qrl";
+            const long long np = nn[mu];
+            Ten UU = ws_tensor("pkrl", {np, kd, np, kd});
+            Ten Ta = ws_tensor("prab", {np, np, a, a}), Tb = ws_tensor("qsab", {np, np, a, a});
+            contract(U[0].as(n1s), U[0].as(n2s), UU);
+            contract(UU, EEk, Ta);
+            contract(U[1].as(n1s), U[1].as(n2s), UU);
+            contract(UU, FFk, Tb.as("prab"));
+            contract(Ta, Tb, GL[mu].as("pqrs"));
+            contract(U[2].as(n1s), U[2].as(n2s), UU);
+            contract(UU, GGk.as("kalb"), Ta);
+            contract(U[3].as(n1s), U[3].as(n2s), UU);
+            contract(UU, HHk.as("kalb"), Tb.as("prab"));
+            contract(Ta, Tb, GR[mu].as("pqrs"));
+            ws_release(mk2);
+        }
+        ws_release(mk);
+    }
+    stage_mark(5);
+
+    // =================== O6 squeezers (Eq. 12; reading G10) ===================
+    Ten Ms[3], Ns[3];
+    int kq[3];
+    for (int mu = 0; mu < 3; ++mu) {
+        const int N2 = (int)(nn[mu] * nn[mu]);
+        Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
+        Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
+        size_t mk = ws_mark();
+        Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
+        double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
+        std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
+        std::vector<double> lam2 = sym_eig(GR[mu].p, N2, V2.p, l2);
+        const int kl = num_rank(lam1, -1), kr = num_rank(lam2, -1);
+        if (kl < 1 || kr < 1) fail(-34, "squeezer: Gram matrix is numerically zero");
+        // R1 = Lambda^1/2 V^T (rows of V1 scaled), R2^T likewise
+        scale_leg(V1.p, (long long)kl * N2, N2, kl, l1, 2);
+        scale_leg(V2.p, (long long)kr * N2, N2, kr, l2, 2);
+        Ten R1 = V1, R2 = V2;
+        R1.legs[0].n = kl;
+        R2.legs[0].n = kr;
+        Ten Fm = ws_tensor("ji", {kr, kl});        // buffer = column-major F = R1 R2 (kl x kr)
+        contract(R2, R1, Fm);
+        Ten Vf = ws_tensor("kj", {kr, kr});
+        double *sf = ws_doubles(kr);
+        jacobi_svd(Fm.p, kl, kr, Vf.p, sf, 1, 0, 0, 0);   // F V = U diag(s): Fm rows -> U_k[i] s_k
+        std::vector<double> sh = d2h(sf, kr);
+        sh.resize(std::min(kl, kr));
+        const int k = num_rank(sh, chi);
+        if (k < 1) fail(-34, "squeezer: R1 R2 is numerically zero");
+        kq[mu] = k;
+        gaps[1 + mu] = rel_gap(sh, k);
+        spec[6 + mu].assign(sh.begin(), sh.begin() + k);
+        Ten Vk = Vf, Uk = Fm.as("ki");
+        Vk.legs[0].n = k;
+        Uk.legs[0].n = k;
+        Ten Mr = ws_tensor("nk", {N2, k}), Nr = ws_tensor("kn", {k, N2});
+        contract(R2, Vk, Mr);                       // M = R2 V s^-1/2
+        contract(Uk, R1, Nr);                       // N = s^-1/2 U^T R1, U = Fm rows / s
+        scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
+        scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
+        // gauge (reading G12): P = N G_ref
+        Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
+        Ten Pq = ws_tensor("kb", {k, k});
+        contract(Nr, rf, Pq);
+        Ten Wq = gauge_rotation(Pq.as("ab"), sh, k);
+        Ms[mu] = Ten::make(Ms[mu].p, "uok", {nn[mu], nn[mu], k});
+        Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
+        contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
+        contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
+        ws_release(mk);
+    }
+    stage_mark(6);
+
+    // =================== O7 contraction (Eqs. 13-14) ===================
+    const long long m1 = kq[0], m2 = kq[1], m3 = kq[2];
+    const long long nd[4] = {n0, m1, m2, m3};
+    int new_dims[4];
+    for (int i = 0; i < 4; ++i) new_dims[perm[i]] = (int)nd[i];
+    long long nsd[4];
+    nsd[3] = gs;
+    for (int i = 2; i >= 0; --i) nsd[i] = nsd[i + 1] * new_dims[i + 1];
+    auto new_view = [&](double *p) {
+        Ten t;
+        t.p = p;
+        for (int i = 0; i < 4; ++i) t.legs.push_back(Leg{'?', nd[i], nsd[perm[i]]});
+        t.legs.push_back(Leg{'?', (long long)gs, 1});
+        return t;
+    };
+    if ((size_t)(n0 * m1 * m2 * m3 * gs) * 8 > new_cap) fail(-12, "internal: new state exceeds its reservation");
+    for (int side = 0; side < 2; ++side) {
+        size_t mk = ws_mark();
+        Ten W1 = ws_tensor("qkPm", {n2, kd, n1, m1}), V2 = ws_tensor("Plqn", {n1, kd, n2, m2});
+        Ten Qt = ws_tensor("klmn", {kd, kd, m1, m2});
+        if (side == 0) {
+            contract(U[0].as("pqk"), Ms[0].as("pPm"), W1);
+            contract(U[1].as("PQl"), Ms[1].as("qQn"), V2);
+        } else {
+            contract(U[2].as("pqk"), Ns[0].as("mpP"), W1);
+            contract(U[3].as("PQl"), Ns[1].as("nqQ"), V2);
+        }
+        contract(W1, V2, Qt);
+        Ten EM = ws_tensor("xkaTw", {n0, kd, a, n3, m3});
+        Ten Pt = ws_tensor("xkwlg", {n0, kd, m3, kd, gs});
+        Ten out = new_view(side == 0 ? phi_new : psi_new);
+        if (side == 0) {
+            contract(E.as("xkta"), Ms[2].as("tTw"), EM);
+            contract(EM, F.as("alTg"), Pt);
+            contract(Pt, Qt, out.as("xmnwg"));
+        } else {
+            // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
+            contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkatw"));
+            contract(EM.as("xkatw"), G.as("altg"), Pt);   // Pt[x, kD, w, kY, g]
+            contract(Pt.as("xlwkg"), Qt, out.as("xmnwg"));
+        }
+        ws_release(mk);
+    }
+    stage_mark(7);
+
+    // =================== O8 normalise, accumulate ln Z ===================
+    const long long nnew = n0 * m1 * m2 * m3 * gs;
+    double *ss = ws_doubles(2);
+    sumsq(phi_new, nnew, ss);
+    sumsq(psi_new, nnew, ss + 1);
+    scale_by_rsqrt(phi_new, nnew, ss);
+    scale_by_rsqrt(psi_new, nnew, ss + 1);
+    std::vector<double> nv = d2h(ss, 2);
+    stage_mark(8);
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    if (!(nv[0] > 0) || !(nv[1] > 0) || !std::isfinite(nv[0]) || !std::isfinite(nv[1]))
+        fail(-34, "coarse_grain: non-finite or zero norm of the renormalised tensor");
+    // ---- commit
+    const double lnc = 0.5 * (log(nv[0]) + log(nv[1]));
+    c.step += 1;
+    c.log_acc += ldexp(1.0, -c.step) * lnc;
+    for (int i = 0; i < 4; ++i) c.dims[i] = new_dims[i];
+    c.bond = gs;
+    c.phi = phi_new;
+    c.psi = psi_new;
+    c.state_low = !c.state_low;
+    c.state_bytes = 2 * new_cap;
+    spec[9] = {lnc};
+    for (int i = 0; i < 10; ++i) c.spec[i] = spec[i];
+    for (int i = 0; i < 4; ++i) c.gaps[i] = gaps[i];
+    for (int i = 0; i < ST_COUNT; ++i) {
+        float ms = 0;
+        cudaEventElapsedTime(&ms, c.ev[i], c.ev[i + 1]);
+        c.stage_ms[i] = ms;
+    }
+}
+
+}  // namespace tatrg

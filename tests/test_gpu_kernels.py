@@ -1,0 +1,151 @@
+"""GPU kernel checks through the C-ABI: every stand-alone kernel of libtatrg against the plain
+definition of what it computes (numpy FP64 on the host), on sizes that span several tiles and a
+ragged tail, plus the degenerate cases (rank-deficient QR, zero columns, odd sizes)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tt():
+    import torch
+    import paper_2412_14104_b200 as t
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    t.set_workspace(nbytes=1 << 30)
+    t.set_stream()
+    yield t
+    t.destroy()
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+@pytest.mark.parametrize("M,N,K", [(128, 128, 64), (200, 136, 77), (1, 1, 1), (7, 300, 5), (513, 65, 1030),
+                                   (64, 64, 20000)])
+def test_tensor_gemm_plain(tt, M, N, K):
+    rng = np.random.default_rng(M * 7 + N * 3 + K)
+    A, B = rng.standard_normal((M, K)), rng.standard_normal((K, N))
+    import torch
+    dA, dB = _dev(A), _dev(B)
+    dC = torch.zeros(M, N, dtype=torch.float64, device="cuda")
+    maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+    tt.tensor_gemm(dA, dB, dC, M, N, K, maps, alpha=0.5)
+    torch.cuda.synchronize()
+    ref = 0.5 * (A @ B)
+    np.testing.assert_allclose(dC.cpu().numpy(), ref, rtol=0, atol=1e-12 * np.sqrt(K) * 4)
+    # transposed operands (m-contiguous A, k-contiguous B) and accumulate
+    dAt, dBt = _dev(A.T), _dev(B.T)
+    maps = dict(am=[(M, 1)], ak=[(K, M)], bk=[(K, 1)], bn=[(N, K)], cm=[(M, N)], cn=[(N, 1)])
+    tt.tensor_gemm(dAt, dBt, dC, M, N, K, maps, alpha=1.0, accumulate=True)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(dC.cpu().numpy(), 1.5 * (A @ B), rtol=0, atol=1e-12 * np.sqrt(K) * 8)
+
+
+def test_tensor_gemm_permuted_legs_batched(tt):
+    """C[b,x,w,l,g] = sum_{a,u} EM[b,x,a,u,w] F[a,l,u,g] * s : the shape of Eq. 13's inner product
+     with composite row / column / summed indices and a batch leg."""
+    import torch
+    rng = np.random.default_rng(5)
+    nb, nx, na, nu, nw, nl, ng = 3, 5, 6, 4, 7, 9, 6
+    EM = rng.standard_normal((nb, nx, na, nu, nw))
+    F = rng.standard_normal((na, nl, nu, ng))
+    ref = np.ascontiguousarray(np.einsum("bxauw,alug->bxwlg", EM, F))
+    dEM, dF = _dev(EM), _dev(F)
+    dC = torch.empty(ref.shape, dtype=torch.float64, device="cuda")
+    se, sf, sc = [s // 8 for s in EM.strides], [s // 8 for s in F.strides], [s // 8 for s in ref.strides]
+    maps = dict(am=[(nw, se[4]), (nx, se[1])], ak=[(nu, se[3]), (na, se[2])],
+                bk=[(nu, sf[2]), (na, sf[0])], bn=[(ng, sf[3]), (nl, sf[1])],
+                cm=[(nw, sc[2]), (nx, sc[1])], cn=[(ng, sc[4]), (nl, sc[3])],
+                ab=[(nb, se[0])], bb=[(nb, 0)], cb=[(nb, sc[0])])
+    tt.tensor_gemm(dEM, dF, dC, nx * nw, nl * ng, na * nu, maps, batch=nb)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(dC.cpu().numpy(), ref, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("m,n", [(16, 2), (256, 64), (257, 33), (5000, 12), (70000, 64), (1000, 1), (64, 64)])
+def test_qr_pos(tt, m, n):
+    import torch
+    rng = np.random.default_rng(m + n)
+    Y = rng.standard_normal((m, n))
+    dY = _dev(Y)
+    dR = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    tt.qr_pos(dY, dR)
+    torch.cuda.synchronize()
+    Q, R = dY.cpu().numpy(), dR.cpu().numpy()
+    assert np.all(np.diag(R) >= 0) and np.allclose(R, np.triu(R))
+    assert np.abs(Q.T @ Q - np.eye(n)).max() < 1e-13
+    assert np.abs(Q @ R - Y).max() < 1e-12 * np.abs(Y).max() * np.sqrt(m)
+    # uniqueness: LAPACK's QR with the signs moved to R_ii > 0
+    Ql, Rl = np.linalg.qr(Y)
+    d = np.sign(np.diag(Rl))
+    assert np.abs(Q - Ql * d).max() < 1e-10
+
+
+def test_qr_pos_rank_deficient(tt):
+    import torch
+    rng = np.random.default_rng(3)
+    m, n, rk = 3000, 24, 9
+    Y = rng.standard_normal((m, rk)) @ rng.standard_normal((rk, n))
+    Y[:, 5] = 0.0
+    dY = _dev(Y)
+    dR = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    tt.qr_pos(dY, dR)
+    Q, R = dY.cpu().numpy(), dR.cpu().numpy()
+    assert np.abs(Q.T @ Q - np.eye(n)).max() < 1e-12
+    assert np.abs(Q @ R - Y).max() < 1e-11 * np.abs(Y).max()
+
+
+@pytest.mark.parametrize("m,n", [(64, 64), (12, 12), (33, 7), (300, 129), (1, 1), (40, 64)])
+def test_jacobi_svd(tt, m, n):
+    import torch
+    rng = np.random.default_rng(m * 3 + n)
+    G = rng.standard_normal((m, n)) * np.logspace(0, -6, n)
+    dG = _dev(G.T)                       # row j = column j
+    dV = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    ds = torch.empty(n, dtype=torch.float64, device="cuda")
+    tt.jacobi_svd(dG, dV, ds)
+    Us, V, s = dG.cpu().numpy().T, dV.cpu().numpy().T, ds.cpu().numpy()
+    sl = np.linalg.svd(G, compute_uv=False)
+    k = min(m, n)
+    assert np.abs(s[:k] - sl).max() < 1e-13 * sl[0]
+    assert np.all(np.diff(s) <= 0)
+    assert np.abs(V.T @ V - np.eye(n)).max() < 1e-13
+    assert np.abs(G @ V - Us).max() < 1e-13 * sl[0]
+    Un = Us[:, :k] / s[:k]
+    assert np.abs(Un.T @ Un - np.eye(k)).max() < 1e-9   # tiny singular values: columns less orthogonal
+
+
+def test_jacobi_symmetric_psd_eig(tt):
+    import torch
+    rng = np.random.default_rng(11)
+    n, rk = 96, 40
+    B = rng.standard_normal((n, rk)) * np.logspace(0, -5, rk)
+    S = B @ B.T
+    dG = _dev(S)
+    dV = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    ds = torch.empty(n, dtype=torch.float64, device="cuda")
+    tt.jacobi_svd(dG, dV, ds)
+    lam, V = ds.cpu().numpy(), dV.cpu().numpy().T
+    ll = np.linalg.eigvalsh(S)[::-1]
+    assert np.abs(lam - np.maximum(ll, 0)).max() < 1e-13 * ll[0]
+    assert np.abs(S @ V[:, :rk] - V[:, :rk] * lam[:rk]).max() < 1e-12 * ll[0]
+
+
+@pytest.mark.parametrize("n", [1, 31, 4096, 1 << 20, (1 << 22) + 3])
+def test_norm_and_trace_reductions(tt, n):
+    import torch
+    rng = np.random.default_rng(n)
+    x, y = rng.standard_normal(n), rng.standard_normal(n)
+    dx, dy = _dev(x), _dev(y)
+    out = torch.empty(2, dtype=torch.float64, device="cuda")
+    tt.sumsq(dx, out[0:1])
+    tt.dot(dx, dy, out[1:2])
+    o = out.cpu().numpy()
+    assert abs(o[0] - np.sum(x * x)) < 1e-13 * n
+    assert abs(o[1] - np.sum(x * y)) < 1e-13 * n
+    tt.scale_by_rsqrt(dx, out[0:1])
+    np.testing.assert_allclose(dx.cpu().numpy(), x / np.linalg.norm(x), rtol=1e-14, atol=0)

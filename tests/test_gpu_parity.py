@@ -1,0 +1,81 @@
+"""Parity of the CUDA path (through the C-ABI) with the CPU oracle on the same seeded inputs.
+
+Compared: ln Z per site after every step (BASELINE.json north_star: 1e-10 relative) and every
+truncated spectrum of every step (1e-9 of the largest value, reading G13), plus dims.  Gauge
+dependent tensors are not compared (reading G18)."""
+import numpy as np
+import pytest
+
+from oracle import driver
+from oracle import tatrg_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+LNZ_RTOL = 1e-10
+SPEC_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def tt():
+    import torch
+    import paper_2412_14104_b200 as t
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    t.set_workspace(nbytes=6 << 30)
+    t.set_stream()
+    yield t
+    t.destroy()
+
+
+def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None):
+    """Oracle and GPU step by step; returns list of per-step comparison records."""
+    recs = []
+    st = orc.init_ising_tensor(beta, h)
+    tt.init_ising_tensor(beta, h)
+    assert abs(tt.log_Z_per_site() / orc.log_Z_per_site(st) - 1) < 1e-13
+    for m in range(n_steps):
+        d = directions[m % len(directions)] if directions else (m % 4) + 1
+        rec = orc.coarse_grain(st, d, chi, r, q, driver.seeded_inputs_for(seed, m))
+        tt.coarse_grain(d, chi, r, q, seed)
+        out = {"step": m, "lnz_o": orc.log_Z_per_site(st), "lnz_g": tt.log_Z_per_site(),
+               "dims_o": st.dims, "dims_g": tt.get_dims()[:5], "spec": {}}
+        for name in ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3"):
+            so, sg = np.asarray(rec[name]) if name in rec else np.zeros(0), tt.get_spectrum(name)
+            out["spec"][name] = (so, sg)
+        recs.append(out)
+    return recs
+
+
+def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL):
+    for o in recs:
+        assert tuple(o["dims_o"]) == tuple(o["dims_g"]), o
+        for name, (so, sg) in o["spec"].items():
+            assert len(so) == len(sg), (o["step"], name, len(so), len(sg))
+            if len(so):
+                assert np.abs(so - sg).max() <= spec_tol * so[0], (o["step"], name, np.abs(so - sg).max() / so[0])
+        assert abs(o["lnz_g"] / o["lnz_o"] - 1) <= lnz_rtol, (o["step"], o["lnz_g"], o["lnz_o"])
+
+
+def test_config1_chi6_8steps(tt):
+    """BASELINE.json configs[0]: T=6.0, chi=6, r=2, q=2, 8 steps cycling 1..4 (4^4 lattice)."""
+    check(run_both(tt, 1 / 6.0, 0.0, 6, 2, 2, 8, 20241214))
+
+
+def test_untruncated_tiny_lattice_matches_enumeration(tt):
+    """GPU path against exact enumeration directly (2x2x1x1 lattice, chi large enough)."""
+    from exact_refs import brute_force_lnZ
+    tt.init_ising_tensor(1 / 6.0, 0.01)
+    tt.coarse_grain(1, 16, 2, 2, 7)
+    tt.coarse_grain(2, 16, 2, 2, 7)
+    assert abs(tt.log_Z_per_site() / brute_force_lnZ(1 / 6.0, 0.01, (2, 2, 1, 1)) - 1) < 1e-12
+
+
+@pytest.mark.parametrize("dirs", [[2, 3, 1, 4], [4, 4, 1, 2]])
+def test_direction_orders_with_field(tt, dirs):
+    check(run_both(tt, 1 / 6.5, 0.01, 5, 2, 1, 4, 99, directions=dirs))
+
+
+def test_config2_chi16_first_steps(tt):
+    """BASELINE.json configs[1] (T=6.65, chi=16, r=2, q=2): the first 10 of its 40 steps (the oracle
+    needs ~seconds per step at chi=16)."""
+    check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 10, 20241215))
