@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- Triad-ATRG coarse-grain steps/s (FP64) on B200, the metric of BASELINE.json.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl reference]
+
+One "step" = one pass of the whole hot path (canonical form, RSVD bond
+swap, RSVD isometries, triad tensors, squeezers, O(r^2 chi^7) contraction, normalisation) on the
+steady-state tensor (all legs and the bond = chi) of the named config.  Inputs are synthetic by
+construction: the 4D Ising tensor generated from (beta, h) and host-generated seeded Gaussian
+sketches.
+
+Printed JSON line (rank 0): value = whole-job steps/s with the step's sketches already resident in
+HBM; e2e = the same through the C-ABI with HOST sketch buffers (pinned; H2D inside coarse_grain)
+plus the ln Z/V read-back (device reduction + scalar D2H) every step; roofline = the tensor-GEMM
+kernel (FP64 DMMA) timed per launch with CUDA events on the library's stream inside the timed
+region; cpu_baseline = the CPU oracle on this box's host cores on a bounded sample.
+
+N > 1: the path does not shard (BASELINE.json north_star: one GPU, no collectives) -> N
+independent replicas, value = N*K / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Triad-ATRG coarse-grain steps/s (FP64)"
+UNIT = "steps/s"
+
+# BASELINE.json configs; seed = 20241214 + config index
+CONFIGS = {
+    "c1": dict(T=6.0, h=0.0, chi=6, r=2, q=2, seed=20241214, ramp=4),
+    "c2": dict(T=6.65, h=0.0, chi=16, r=2, q=2, seed=20241215, ramp=8),
+    "c3": dict(T=6.65, h=0.0, chi=32, r=2, q=2, seed=20241216, ramp=8),
+    "c5": dict(T=6.5, h=0.01, chi=64, r=2, q=3, seed=20241218, ramp=8),
+}
+# nominal dense peaks of /opt/skills/guides (B200): FP64 tensor 45 TFLOP/s, bf16 2250 TFLOP/s
+FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
+
+
+def workload_name(name, c):
+    return ("%s: 4D Ising T=%.2f h=%g, Triad-ATRG chi=%d r=%d q=%d, steady-state coarse-grain steps "
+            "(all legs = chi), directions cycling 1..4" % (name, c["T"], c["h"], c["chi"], c["r"], c["q"]))
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}, "fallback"
+
+
+# ------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return None
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw = [], [], []
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            with open(self.path) as f:
+                for line in f:
+                    p = [x.strip() for x in line.split(",")]
+                    if len(p) < 8:
+                        continue
+                    try:
+                        sm.append(float(p[1]))
+                        mx.append(float(p[2]))
+                        pw.append(float(p[3]))
+                    except ValueError:
+                        continue
+                    for n, v in zip(names, p[4:8]):
+                        if v.lower().startswith("active"):
+                            reasons.add(n)
+            os.unlink(self.path)
+        except Exception:
+            return None
+        if not sm:
+            return None
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------ inputs
+def pinned_sketches(tt, cfg, step_index, direction):
+    """Host (pinned) seeded Gaussian sketches of one step: {which: torch tensor}; shapes asked from
+    the library for the current state (rows, cols per DESIGN.md 'Input recipe')."""
+    import torch
+    import seeded_inputs as si
+    out = {}
+    for which in range(0, 5):
+        rows, cols = tt.sketch_shape(which, direction, cfg["chi"], cfg["r"])
+        if rows * cols == 0:
+            continue
+        t = torch.empty(rows * cols, dtype=torch.float64, pin_memory=True)
+        si.gauss(si.subseed(cfg["seed"], step_index, which), rows * cols, out=t.numpy())
+        out[which] = t
+    return out
+
+
+def gauge_refs(tt, cfg, direction):
+    """Step-independent gauge reference matrices (reading G12), device resident."""
+    import torch
+    import seeded_inputs as si
+    out = {}
+    for which in range(5, 9):
+        rows, cols = tt.sketch_shape(which, direction, cfg["chi"], cfg["r"])
+        if rows * cols == 0:
+            continue
+        t = torch.from_numpy(si.gauss(si.subseed(cfg["seed"], 0, which), rows * cols))
+        out[which] = t.cuda()
+    return out
+
+
+# ------------------------------------------------------------------------------ reference arm
+def oracle_sample(cfg):
+    """State of the CPU oracle just before the sample step, and the sample step's arguments.
+    Sample = step 4 of the config's schedule (direction 4): legs (chi/2.., chi) -> the first tensor
+    with all legs = chi.  A true steady-state oracle step at chi=32 takes ~2 min on 8 cores."""
+    from oracle import driver
+    from oracle import tatrg_oracle as orc
+    st = orc.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
+    for m in range(3):
+        orc.coarse_grain(st, m + 1, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], m))
+    return st
+
+
+def oracle_time_one(cfg, st0):
+    import copy
+    from oracle import driver
+    from oracle import tatrg_oracle as orc
+    st = copy.deepcopy(st0)
+    t0 = time.perf_counter()
+    orc.coarse_grain(st, 4, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], 3))
+    dt = time.perf_counter() - t0
+    return dt, st
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 0) for p in threadpool_info() if p.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count()
+
+
+SAMPLE_TEXT = ("1 oracle coarse_grain call = step 4 of the schedule (direction 4, input legs "
+               "(chi/2, chi/2, chi/2, chi) -> first tensor with all legs = chi) after 3 untimed ramp-up steps; "
+               "cheaper than a steady-state step (116 s on 8 cores at chi=32), so an upper bound on the "
+               "oracle's steady-state steps/s")
+
+
+def run_reference(args, cfg, name):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy  # noqa: F401  (BLAS threads = all cores)
+    st0 = oracle_sample(cfg)
+    budget_s = 240.0
+    times = []
+    t, _ = oracle_time_one(cfg, st0)          # first warm-up doubles as the cost estimate
+    warm = 1
+    steps = args.steps
+    while warm < args.warmup and (warm + 1 + steps) * t < budget_s:
+        oracle_time_one(cfg, st0)
+        warm += 1
+    steps = max(1, min(steps, int(budget_s / t) - warm))
+    for _ in range(steps):
+        dt, _ = oracle_time_one(cfg, st0)
+        times.append(dt)
+    total = sum(times)
+    val = steps / total
+    cores = blas_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "steps_requested": args.steps, "warmup": warm, "ms_per_step": 1e3 * total / steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": workload_name(name, cfg), "sample": SAMPLE_TEXT},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": SAMPLE_TEXT},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args, cfg, name):
+    import torch
+    import paper_2412_14104_b200 as tt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libtatrg has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
+    K, W = args.steps, max(args.warmup, 0)
+    tt.set_workspace(chi=chi, r=r, device="cuda:%d" % local)
+    stream = torch.cuda.Stream()
+    tt.set_stream(stream)
+    tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
+    m = 0
+    for _ in range(cfg["ramp"]):                       # untimed ramp-up to the steady state
+        tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
+        m += 1
+    dims = tt.get_dims()
+    steady = all(d == chi for d in dims[:5])
+
+    refs = {d: gauge_refs(tt, cfg, d) for d in (1, 2, 3, 4)}
+
+    def set_inputs(sk, d):
+        for which, t in sk.items():          # CUDA tensor -> device pointer; pinned CPU tensor -> host pointer
+            tt.set_sketch(which, t)
+        for which, t in refs[d].items():
+            tt.set_sketch(which, t)
+
+    # ---- pass 1: sketches resident in HBM before the timed region
+    host = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(W + K)]
+    dev = [{w: t.cuda() for w, t in sk.items()} for sk in host]
+    torch.cuda.synchronize()
+    for i in range(W):
+        set_inputs(dev[i], (m + i) % 4 + 1)
+        tt.coarse_grain((m + i) % 4 + 1, chi, r, q, seed)
+    tt.set_profile(True)
+    tt.launch_count(reset=True)
+    tt.gemm_flops(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")
+    sampler = ClockSampler(vis[local] if local < len(vis) and vis[local].strip().isdigit() else local)
+    stages = {}
+    gprof = {}
+    barrier()
+    sampler.start()
+    e0.record(stream)
+    for i in range(W, W + K):
+        d = (m + i) % 4 + 1
+        set_inputs(dev[i], d)
+        tt.coarse_grain(d, chi, r, q, seed)
+        for k, v in tt.stage_ms().items():
+            stages[k] = stages.get(k, 0.0) + v / K
+        for k, v in tt.gemm_profile().items():
+            g = gprof.setdefault(k, {"ms": [0.0, 0.0], "flops": [0.0, 0.0], "launches": [0, 0]})
+            for j in range(2):
+                g["ms"][j] += v["ms"][j]
+                g["flops"][j] += v["flops"][j]
+                g["launches"][j] += v["launches"][j]
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    launches = tt.launch_count(reset=True)
+    flops = tt.gemm_flops(reset=True)
+    tt.set_profile(False)
+    m += W + K
+    lnz = tt.log_Z_per_site()
+    del dev
+    torch.cuda.empty_cache()
+
+    # ---- pass 2: end to end through the C-ABI with host sketch buffers + ln Z read-back
+    Ke = K
+    h2d = 0
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    host2 = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(Ke)]
+    barrier()
+    e2.record(stream)
+    for i in range(Ke):
+        d = (m + i) % 4 + 1
+        set_inputs(host2[i], d)                      # host pointers: copied inside coarse_grain
+        tt.coarse_grain(d, chi, r, q, seed)
+        lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
+        h2d += sum(t.numel() * 8 for t in host2[i].values())
+    e3.record(stream)
+    barrier()
+    ms_e2e = e2.elapsed_time(e3)
+    m += Ke
+
+    # ---- max over ranks
+    if dist is not None:
+        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_e2e = float(t[0]), float(t[1])
+        ln = torch.tensor([float(launches)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(ln)
+        launches = int(ln[0])
+
+    # ---- roofline of the dominant kernel (tensor-GEMM, 128x128 DMMA tile)
+    peaks, how = measured_peaks()
+    g_ms = sum(v["ms"][1] for v in gprof.values())
+    g_fl = sum(v["flops"][1] for v in gprof.values())
+    g_n = sum(v["launches"][1] for v in gprof.values())
+    s_ms = sum(v["ms"][0] for v in gprof.values())
+    s_fl = sum(v["flops"][0] for v in gprof.values())
+    peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * FP64_OVER_BF16_NOMINAL
+    achieved = g_fl / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
+    probe = tt.probe_fp64_peak(0, 1 << 14)
+    probe_dfma = tt.probe_fp64_peak(1, 1 << 14)
+    per_stage = {k: {"gemm_ms_per_step": (v["ms"][0] + v["ms"][1]) / K,
+                     "gemm_tflops": ((v["flops"][0] + v["flops"][1]) / ((v["ms"][0] + v["ms"][1]) * 1e-3) / 1e12
+                                     if v["ms"][0] + v["ms"][1] > 0 else 0.0),
+                     "gemm_launches_per_step": (v["launches"][0] + v["launches"][1]) / K}
+                 for k, v in gprof.items()}
+    roofline = {"bound": "tensor", "kernel": "tgemm_kernel<128,128,32,32,4> (FP64 DMMA.8x8x4)",
+                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
+                "traffic": None,
+                "peak_source": "%s bf16_tflops_sustained x nominal FP64/bf16 ratio 45/2250" % how,
+                "peak_probe_dmma_tflops": probe, "peak_probe_dfma_tflops": probe_dfma,
+                "frac_of_probe": achieved / probe if probe > 0 else None,
+                "flops_per_launch": g_fl / g_n if g_n else 0.0, "avg_launch_ms": g_ms / g_n if g_n else 0.0,
+                "launches": g_n, "share_of_step_time": g_ms / ms if ms > 0 else None,
+                "small_tile_kernel": {"tflops": s_fl / (s_ms * 1e-3) / 1e12 if s_ms > 0 else 0.0,
+                                      "share_of_step_time": s_ms / ms if ms > 0 else None},
+                "whole_step_gemm_tflops": flops / (ms * 1e-3) / 1e12}
+
+    line = None
+    if rank == 0:
+        line = {"metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+                "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": workload_name(name, cfg), "chi": chi, "r": r, "q": q,
+                           "steady_state": steady, "dims": list(dims[:5]),
+                           "l2": "inputs larger than L2 (Phi, Psi, A, D, X, Y are 268 MB each at chi=32)",
+                           "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                "e2e": {"value": world * Ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke,
+                        "d2h_bytes_per_step": 8, "steps": Ke},
+                "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
+                "stages_ms_per_step": stages, "stages_gemm": per_stage, "ln_Z_per_site": lnz}
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="c3", choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg, args.config)
+        return
+    line = run_ours(args, cfg, args.config)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            st0 = oracle_sample(cfg)
+            dt, _ = oracle_time_one(cfg, st0)
+            line["cpu_baseline"] = {"value": 1.0 / dt, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                                    "sample": SAMPLE_TEXT, "seconds": dt}
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

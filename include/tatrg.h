@@ -102,6 +102,13 @@ double tatrg_order_parameter(int leg);
  * named by tatrg_stage_name(i).  Returns the number of stages. */
 int tatrg_get_stage_ms(double *host_out, int cap);
 const char *tatrg_stage_name(int i);
+/* Per-launch device timing of the tensor-GEMM kernel (CUDA event pairs on the library's stream
+ * around every launch inside coarse_grain; a few microseconds of overhead per launch).  After a
+ * step, tatrg_get_gemm_profile copies, for every stage i and tile configuration j (0: 64x64 CTA
+ * tile, 1: 128x128), the triple {milliseconds, FP64 flops, launches} to host_out[(2 i + j) 3 ..];
+ * returns the number of doubles written. */
+int tatrg_set_profile(int on);
+int tatrg_get_gemm_profile(double *host_out, int cap);
 /* Number of kernel launches this library has enqueued since the last call (and reset). */
 long long tatrg_launch_count(int reset);
 /* FP64 flops of the tensor-GEMM launches since the last reset (2*M*N*K*batch each). */

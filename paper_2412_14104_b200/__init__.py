@@ -21,6 +21,7 @@ EXPORTS = [
     "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_peak",
     "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
+    "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
     "tatrg_qr_pos", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
     "tatrg_last_error", "tatrg_destroy",
@@ -65,6 +66,8 @@ def lib():
             "tatrg_order_parameter": (c_d, [c_i]),
             "tatrg_get_stage_ms": (c_i, [c_vp, c_i]),
             "tatrg_stage_name": (ctypes.c_char_p, [c_i]),
+            "tatrg_set_profile": (c_i, [c_i]),
+            "tatrg_get_gemm_profile": (c_i, [c_vp, c_i]),
             "tatrg_launch_count": (ctypes.c_longlong, [c_i]),
             "tatrg_gemm_flops": (c_d, [c_i]),
             "tatrg_probe_fp64_peak": (c_d, [c_i, c_i]),
@@ -209,6 +212,23 @@ def stage_ms() -> dict:
     out = np.zeros(16)
     n = lib().tatrg_get_stage_ms(out.ctypes.data, out.size)
     return {lib().tatrg_stage_name(i).decode(): float(out[i]) for i in range(n)}
+
+
+def set_profile(on: bool):
+    _check(lib().tatrg_set_profile(int(bool(on))))
+
+
+def gemm_profile() -> dict:
+    """{stage: {"ms": [small, big], "flops": [..], "launches": [..]}} of the last profiled step."""
+    out = np.zeros(96)
+    n = lib().tatrg_get_gemm_profile(out.ctypes.data, out.size)
+    res = {}
+    for i in range(n // 6):
+        name = lib().tatrg_stage_name(i).decode()
+        a = out[6 * i:6 * i + 6]
+        res[name] = {"ms": [float(a[0]), float(a[3])], "flops": [float(a[1]), float(a[4])],
+                     "launches": [int(a[2]), int(a[5])]}
+    return res
 
 
 def launch_count(reset=False) -> int:

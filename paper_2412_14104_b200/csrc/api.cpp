@@ -41,6 +41,49 @@ void fail(int code, const char *fmt, ...)
     throw Err{code};
 }
 
+int prof_begin(double flops, int big)
+{
+    Ctx &c = ctx();
+    if (!c.prof) return -1;
+    const size_t slot = c.prof_rec.size();
+    if (2 * slot + 2 > c.prof_ev.size()) {
+        const size_t old = c.prof_ev.size();
+        c.prof_ev.resize(old + 1024);
+        for (size_t i = old; i < c.prof_ev.size(); ++i)
+            if (cudaEventCreate(&c.prof_ev[i]) != cudaSuccess) {
+                c.prof_ev.resize(i & ~(size_t)1);
+                return -1;
+            }
+    }
+    c.prof_rec.push_back(Ctx::ProfRec{c.cur_stage, big, flops});
+    cudaEventRecord(c.prof_ev[2 * slot], c.stream);
+    return (int)slot;
+}
+
+void prof_end(int slot)
+{
+    if (slot < 0) return;
+    Ctx &c = ctx();
+    cudaEventRecord(c.prof_ev[2 * slot + 1], c.stream);
+}
+
+void prof_collect()
+{
+    Ctx &c = ctx();
+    for (int i = 0; i < ST_COUNT; ++i)
+        for (int j = 0; j < 2; ++j) c.gemm_ms[i][j] = c.gemm_fl[i][j] = 0.0, c.gemm_n[i][j] = 0;
+    for (size_t i = 0; i < c.prof_rec.size(); ++i) {
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, c.prof_ev[2 * i], c.prof_ev[2 * i + 1]) != cudaSuccess) continue;
+        const Ctx::ProfRec &r = c.prof_rec[i];
+        if (r.stage < 0 || r.stage >= ST_COUNT) continue;
+        c.gemm_ms[r.stage][r.big] += ms;
+        c.gemm_fl[r.stage][r.big] += r.flops;
+        c.gemm_n[r.stage][r.big] += 1;
+    }
+    c.prof_rec.clear();
+}
+
 void *ws_alloc(size_t bytes)
 {
     Ctx &c = ctx();
@@ -265,6 +308,27 @@ int tatrg_get_stage_ms(double *host_out, int cap)
     return ST_COUNT;
 }
 
+int tatrg_set_profile(int on)
+{
+    ctx().prof = on != 0;
+    ctx().prof_rec.clear();
+    return TATRG_OK;
+}
+
+int tatrg_get_gemm_profile(double *host_out, int cap)
+{
+    Ctx &c = ctx();
+    int k = 0;
+    for (int i = 0; i < ST_COUNT; ++i)
+        for (int j = 0; j < 2; ++j) {
+            if (k + 3 > cap) return k;
+            host_out[k++] = c.gemm_ms[i][j];
+            host_out[k++] = c.gemm_fl[i][j];
+            host_out[k++] = (double)c.gemm_n[i][j];
+        }
+    return k;
+}
+
 const char *tatrg_stage_name(int i) { return (i >= 0 && i < ST_COUNT) ? kStageNames[i] : ""; }
 
 long long tatrg_launch_count(int reset)
@@ -370,6 +434,7 @@ void tatrg_destroy(void)
     Ctx &c = ctx();
     if (c.ev_ok)
         for (auto &e : c.ev) cudaEventDestroy(e);
+    for (auto &e : c.prof_ev) cudaEventDestroy(e);
     c = Ctx();
 }
 

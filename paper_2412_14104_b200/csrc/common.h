@@ -55,6 +55,8 @@ struct GemmParams {
 cudaStream_t stream();
 void count_launch(int n = 1);
 void count_flops(double f);
+int prof_begin(double flops, int big);
+void prof_end(int slot);
 int set_error(int code, const char *fmt, ...);
 void *ws_alloc(size_t bytes);          // bump allocation from the caller's workspace (throws Err)
 double *ws_doubles(long long n);

@@ -42,6 +42,21 @@ struct Ctx {
     long long launches = 0;
     double flops = 0;
     std::string err;
+
+    // optional per-launch timing of the tensor-GEMM kernel (tatrg_set_profile): CUDA event pairs
+    // around every tgemm launch of a step, summed per stage when the step ends
+    bool prof = false;
+    int cur_stage = 0;
+    std::vector<cudaEvent_t> prof_ev;   // pool, two per launch
+    struct ProfRec {
+        int stage;
+        int big;
+        double flops;
+    };
+    std::vector<ProfRec> prof_rec;
+    double gemm_ms[ST_COUNT][2] = {};      // [stage][0: 64x64 tile, 1: 128x128 tile]
+    double gemm_fl[ST_COUNT][2] = {};
+    long long gemm_n[ST_COUNT][2] = {};
 };
 
 Ctx &ctx();
@@ -51,5 +66,9 @@ void do_init(double beta, double h);
 void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mode);
 double do_log_z();
 double do_order_parameter(int leg);
+// api.cpp : per-launch GEMM timing
+int prof_begin(double flops, int big);   // returns slot or -1
+void prof_end(int slot);
+void prof_collect();                     // after a stream sync: fold the event pairs into gemm_ms
 
 }  // namespace tatrg

@@ -259,7 +259,9 @@ void launch_cfg(const GemmParams &p)
         attr_done = true;
     }
     dim3 grid((p.M + BM - 1) / BM, (p.N + BN - 1) / BN, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
+    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, BM == 128);
     kern<<<grid, NT, smem, stream()>>>(p);
+    prof_end(slot);
     TATRG_LAUNCH_CHECK();
     count_launch();
 }

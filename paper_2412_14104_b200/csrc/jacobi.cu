@@ -10,6 +10,8 @@
 #include "common.h"
 
 #include <math.h>
+#include <stdlib.h>
+#include <string.h>
 
 namespace tatrg {
 
@@ -45,6 +47,7 @@ __device__ __forceinline__ void block_sum3(double &a, double &b, double &c)
 __global__ void __launch_bounds__(JT) jacobi_round_kernel(double *__restrict__ G, int m, int n,
                                                          double *__restrict__ V, int round, int npad,
                                                          long long strideG, long long strideV, double tol,
+                                                         const double *__restrict__ fro2,
                                                          unsigned long long *__restrict__ maxcos)
 {
     const int pi = blockIdx.x;
@@ -77,10 +80,16 @@ __global__ void __launch_bounds__(JT) jacobi_round_kernel(double *__restrict__ G
     const bool swap = aa < bb;      // keep the larger column at the lower index
     double c = 1.0, s = 0.0;
     bool rot = false;
-    if (aa > 0.0 && bb > 0.0) {
+    // A column that has collapsed to (numerically) nothing -- the surplus columns of a matrix with
+    // fewer rows than columns, exact null vectors -- carries no direction (and its products
+    // underflow): it is left alone.  1e-20 |G|_F is far below anything the path keeps (RANK_TOL).
+    const double dead = 1e-40 * fro2[blockIdx.y];
+    if (aa > dead && bb > dead) {
         double cosv = fabs(ab) / sqrt(aa * bb);
-        if (threadIdx.x == 0 && cosv > tol) atomicMax(maxcos, (unsigned long long)__double_as_longlong(cosv));
-        if (cosv > 0.25 * tol) {
+        // one threshold for "rotate" and "not converged" (as LAPACK's dgesvj): a converged pair is
+        // never touched again, so rounding in the rotations cannot keep the sweep count alive
+        if (cosv > tol) {
+            if (threadIdx.x == 0) atomicMax(maxcos, (unsigned long long)__double_as_longlong(cosv));
             double zeta = (bb - aa) / (2.0 * ab);
             double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
             c = 1.0 / sqrt(1.0 + tt * tt);
@@ -152,8 +161,11 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
     size_t mark = ws_mark();
     for (int b = 0; b < batch; ++b) fill_identity(V + b * strideV, n);
     const int npad = n + (n & 1);
-    const double tol = sqrt((double)(m > 16 ? m : 16)) * 1.1102230246251565e-16;
+    const int mn = m > n ? m : n;
+    const double tol = 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
     unsigned long long *flag = (unsigned long long *)ws_alloc(sizeof(unsigned long long));
+    double *fro2 = ws_doubles(batch);
+    for (int b = 0; b < batch; ++b) sumsq(G + b * strideG, (long long)m * n, fro2 + b);
     const int max_sweeps = 60;
     int sweep = 0;
     if (n > 1) {
@@ -161,12 +173,17 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
             TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(unsigned long long), stream()));
             dim3 grid(npad / 2, batch);
             for (int r = 0; r < npad - 1; ++r)
-                jacobi_round_kernel<<<grid, JT, 0, stream()>>>(G, m, n, V, r, npad, strideG, strideV, tol, flag);
+                jacobi_round_kernel<<<grid, JT, 0, stream()>>>(G, m, n, V, r, npad, strideG, strideV, tol, fro2, flag);
             TATRG_LAUNCH_CHECK();
             count_launch(npad - 1);
             unsigned long long h = 0;
             TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream()));
             TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+            if (getenv("TATRG_DEBUG")) {
+                double hv;
+                memcpy(&hv, &h, 8);
+                fprintf(stderr, "jacobi m=%d n=%d sweep %d maxcos %.3e (tol %.3e)\n", m, n, sweep, hv, tol);
+            }
             if (h == 0) break;
         }
         if (sweep == max_sweeps) fail(-34, "jacobi_svd: no convergence after %d sweeps (m=%d n=%d)", max_sweeps, m, n);

@@ -125,6 +125,7 @@ void stage_mark(int i)
         c.ev_ok = true;
     }
     TATRG_CUDA_CHECK(cudaEventRecord(c.ev[i], c.stream));
+    c.cur_stage = i < ST_COUNT ? i : ST_COUNT - 1;
 }
 
 // Symmetric PSD eigenproblem of the n x n matrix S (overwritten): on exit the rows of Vt
@@ -283,6 +284,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     if (direction < 1 || direction > 4 || chi < 1 || r < 1 || q < 0) fail(-22, "coarse_grain: bad arguments");
     if ((long long)r * chi > 64) fail(-22, "coarse_grain: r*chi = %d > 64 not supported yet", r * chi);
     StepCfg cfg{seed, c.step};
+    c.prof_rec.clear();
 
     // ---- frames (reading G8)
     int perm[4];
@@ -659,6 +661,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         cudaEventElapsedTime(&ms, c.ev[i], c.ev[i + 1]);
         c.stage_ms[i] = ms;
     }
+    if (c.prof) prof_collect();
 }
 
 }  // namespace tatrg
