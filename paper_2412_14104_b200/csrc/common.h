@@ -107,6 +107,9 @@ void symmetrize(double *x, int n);                                            //
 void fill_identity(double *x, int n);
 void fill_zero(double *x, long long n);
 void transpose_small(const double *in, double *out, int rows, int cols);      // out[c,r] = in[r,c]
+// chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
+// diagonal); false if a pivot was not positive
+bool cholesky_lower(double *A, int n, double shift_rel);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);
 

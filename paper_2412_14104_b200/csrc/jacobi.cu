@@ -166,7 +166,7 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
     unsigned long long *flag = (unsigned long long *)ws_alloc(sizeof(unsigned long long));
     double *fro2 = ws_doubles(batch);
     for (int b = 0; b < batch; ++b) sumsq(G + b * strideG, (long long)m * n, fro2 + b);
-    const int max_sweeps = 60;
+    const int max_sweeps = 300;
     int sweep = 0;
     if (n > 1) {
         for (; sweep < max_sweeps; ++sweep) {

@@ -184,6 +184,83 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
     return out;
 }
 
+// Seeded Gaussian start block of an iterative solver (not a method input: the iteration is run to
+// convergence, so the result does not depend on it beyond rounding).
+Ten solver_start_block(long long rows, long long cols, int tag, const char *names2)
+{
+    std::vector<double> host((size_t)(rows * cols));
+    si_fill_gauss(host.data(), (uint64_t)(rows * cols), si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
+    Ten t = ws_tensor(names2, {rows, cols});
+    h2d(t.p, host.data(), rows * cols);
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    return t;
+}
+
+// Squeezer of one direction without a dense eigensolver: any factors
+// G^L = R1^T R1, G^R = R2 R2^T give the same M = R2 V s^-1/2, N = s^-1/2 U^T R1 (reading O6), so
+// R1 = L_L^T, R2 = L_R from two Cholesky factorisations (tensor-pipe GEMMs), and only the top
+// chi singular triplets of F = R1 R2 are needed: subspace iteration with a block of width b >
+// chi, iteration count from the measured decay s_b / s_chi so that the neglected part is below
+// 1e-13.  Returns false (nothing written) when a Gram matrix is not numerically positive definite
+// or fewer than chi significant triplets exist -- the caller then uses the dense path.
+struct SqueezeOut {
+    int k;
+    std::vector<double> s;   // Ritz values, descending (>= k of them)
+    double *s_dev;
+    double gap;
+};
+
+bool squeezer_subspace(const Ten &GLm, const Ten &GRm, int N2, int chi, int mu, Ten &Mr, Ten &Nr, SqueezeOut &o)
+{
+    const int b = 64;
+    if (N2 < 256 || chi >= b) return false;
+    Ten LL = ws_tensor("ki", {N2, N2}), LR = ws_tensor("kj", {N2, N2});
+    d2d(LL.p, GLm.p, (long long)N2 * N2);
+    d2d(LR.p, GRm.p, (long long)N2 * N2);
+    const double shift = 3e-14;
+    if (!cholesky_lower(LL.p, N2, shift) || !cholesky_lower(LR.p, N2, shift)) return false;
+    Ten F = ws_tensor("ij", {N2, N2});
+    contract(LL, LR, F);                                   // F = L_L^T L_R
+    auto apply = [&](const double *w, double *out) {       // F w
+        contract(F, Ten::make(const_cast<double *>(w), "jz", {N2, b}), Ten::make(out, "iz", {N2, b}));
+    };
+    auto apply_t = [&](const double *w, double *out) {     // F^T w
+        contract(F, Ten::make(const_cast<double *>(w), "iz", {N2, b}), Ten::make(out, "jz", {N2, b}));
+    };
+    Ten om = solver_start_block(N2, b, mu, "jz");
+    double *left = ws_doubles((long long)N2 * b), *right = ws_doubles((long long)N2 * b);
+    int iters = 2;
+    for (int pass = 0; pass < 2; ++pass) {
+        size_t mk = ws_mark();
+        RsvdOut ro = rsvd(apply, apply_t, om, N2, N2, b, iters, chi, left, right);
+        if (pass == 0) {
+            const double rho = ro.s_full[b - 1] / ro.s_full[chi - 1];
+            if (!(ro.s_full[chi - 1] > 1e-6 * ro.s_full[0])) return false;
+            int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
+            iters = std::max(3, std::min(need + 1, 80));
+            ws_release(mk);
+            continue;
+        }
+        o.k = ro.k;
+        o.s = ro.s_full;
+        o.gap = rel_gap(ro.s_full, ro.k);
+        std::vector<double> keep(ro.s_full.begin(), ro.s_full.begin() + ro.k);
+        ws_release(mk);
+        o.s_dev = ws_doubles(ro.k);
+        h2d(o.s_dev, keep.data(), ro.k);
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    }
+    if (o.k < chi) return false;
+    const int k = o.k;
+    Mr = ws_tensor("nk", {N2, k});
+    Nr = ws_tensor("kn", {k, N2});
+    contract(Ten::make(left, "ik", {N2, k}), LL.as("ni"), Nr);    // N = s^-1/2 U^T L_L^T
+    contract(LR.as("nj"), Ten::make(right, "jk", {N2, k}), Mr);   // M = L_R V s^-1/2
+    scale_leg(Nr.p, Nr.size(), N2, k, o.s_dev, 3);
+    scale_leg(Mr.p, Mr.size(), 1, k, o.s_dev, 3);
+    return true;
+}
+
 }  // namespace
 
 // =======================================================================================
@@ -541,38 +618,52 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
         Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
         size_t mk = ws_mark();
-        Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
-        double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
-        std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
-        std::vector<double> lam2 = sym_eig(GR[mu].p, N2, V2.p, l2);
-        const int kl = num_rank(lam1, -1), kr = num_rank(lam2, -1);
-        if (kl < 1 || kr < 1) fail(-34, "squeezer: Gram matrix is numerically zero");
-        // R1 = Lambda^1/2 V^T (rows of V1 scaled), R2^T likewise
-        scale_leg(V1.p, (long long)kl * N2, N2, kl, l1, 2);
-        scale_leg(V2.p, (long long)kr * N2, N2, kr, l2, 2);
-        Ten R1 = V1, R2 = V2;
-        R1.legs[0].n = kl;
-        R2.legs[0].n = kr;
-        Ten Fm = ws_tensor("ji", {kr, kl});        // buffer = column-major F = R1 R2 (kl x kr)
-        contract(R2, R1, Fm);
-        Ten Vf = ws_tensor("kj", {kr, kr});
-        double *sf = ws_doubles(kr);
-        jacobi_svd(Fm.p, kl, kr, Vf.p, sf, 1, 0, 0, 0);   // F V = U diag(s): Fm rows -> U_k[i] s_k
-        std::vector<double> sh = d2h(sf, kr);
-        sh.resize(std::min(kl, kr));
-        const int k = num_rank(sh, chi);
-        if (k < 1) fail(-34, "squeezer: R1 R2 is numerically zero");
+        Ten Mr, Nr;
+        std::vector<double> sh;
+        double *sf;
+        int k;
+        SqueezeOut so;
+        if (squeezer_subspace(GL[mu], GR[mu], N2, chi, mu, Mr, Nr, so)) {
+            k = so.k;
+            sh = so.s;
+            sf = so.s_dev;
+            gaps[1 + mu] = so.gap;
+        } else {
+            ws_release(mk);
+            Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
+            double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
+            std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
+            std::vector<double> lam2 = sym_eig(GR[mu].p, N2, V2.p, l2);
+            const int kl = num_rank(lam1, -1), kr = num_rank(lam2, -1);
+            if (kl < 1 || kr < 1) fail(-34, "squeezer: Gram matrix is numerically zero");
+            // R1 = Lambda^1/2 V^T (rows of V1 scaled), R2^T likewise
+            scale_leg(V1.p, (long long)kl * N2, N2, kl, l1, 2);
+            scale_leg(V2.p, (long long)kr * N2, N2, kr, l2, 2);
+            Ten R1 = V1, R2 = V2;
+            R1.legs[0].n = kl;
+            R2.legs[0].n = kr;
+            Ten Fm = ws_tensor("ji", {kr, kl});        // buffer = column-major F = R1 R2 (kl x kr)
+            contract(R2, R1, Fm);
+            Ten Vf = ws_tensor("kj", {kr, kr});
+            sf = ws_doubles(kr);
+            jacobi_svd(Fm.p, kl, kr, Vf.p, sf, 1, 0, 0, 0);   // F V = U diag(s): Fm rows -> U_k[i] s_k
+            sh = d2h(sf, kr);
+            sh.resize(std::min(kl, kr));
+            k = num_rank(sh, chi);
+            if (k < 1) fail(-34, "squeezer: R1 R2 is numerically zero");
+            gaps[1 + mu] = rel_gap(sh, k);
+            Ten Vk = Vf, Uk = Fm.as("ki");
+            Vk.legs[0].n = k;
+            Uk.legs[0].n = k;
+            Mr = ws_tensor("nk", {N2, k});
+            Nr = ws_tensor("kn", {k, N2});
+            contract(R2, Vk, Mr);                       // M = R2 V s^-1/2
+            contract(Uk, R1, Nr);                       // N = s^-1/2 U^T R1, U = Fm rows / s
+            scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
+            scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
+        }
         kq[mu] = k;
-        gaps[1 + mu] = rel_gap(sh, k);
         spec[6 + mu].assign(sh.begin(), sh.begin() + k);
-        Ten Vk = Vf, Uk = Fm.as("ki");
-        Vk.legs[0].n = k;
-        Uk.legs[0].n = k;
-        Ten Mr = ws_tensor("nk", {N2, k}), Nr = ws_tensor("kn", {k, N2});
-        contract(R2, Vk, Mr);                       // M = R2 V s^-1/2
-        contract(Uk, R1, Nr);                       // N = s^-1/2 U^T R1, U = Fm rows / s
-        scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
-        scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
         // gauge (reading G12): P = N G_ref
         Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
         Ten Pq = ws_tensor("kb", {k, k});
