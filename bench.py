@@ -375,6 +375,49 @@ def run_ours(args, cfg, name):
     return line
 
 
+# ------------------------------------------------------------------------------ kernel micro-benchmark
+GEMM_SHAPES = {   # the c3 (chi=32, r=2) contraction shapes of SURVEY.md 8(a), plain row-major operands
+    "a6_ii_P=EM.F": (65536, 2048, 1024),
+    "a6_iv_Phi=P.Q": (32768, 1024, 4096),
+    "a2_G1_Z=D.w": (1024, 2048, 32768),
+    "a2_G2_Y=A.Z": (32768, 2048, 1024),
+}
+
+
+def run_gemm_micro(args):
+    """Stand-alone timing of the tensor-GEMM kernel on the named shapes (CUDA events on the library's
+    stream, operands larger than L2 in total, 3 warm-up + 10 timed launches each)."""
+    import torch
+    import paper_2412_14104_b200 as tt
+    torch.cuda.set_device(0)
+    tt.set_workspace(nbytes=1 << 30)
+    stream = torch.cuda.Stream()
+    tt.set_stream(stream)
+    out = {}
+    for name, (M, N, K) in GEMM_SHAPES.items():
+        if args.gemm != "all" and args.gemm != name:
+            continue
+        with torch.cuda.stream(stream):
+            A = torch.randn(M, K, dtype=torch.float64, device="cuda")
+            B = torch.randn(K, N, dtype=torch.float64, device="cuda")
+            C = torch.empty(M, N, dtype=torch.float64, device="cuda")
+        maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+        for _ in range(3):
+            tt.tensor_gemm(A, B, C, M, N, K, maps)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 10
+        e0.record(stream)
+        for _ in range(reps):
+            tt.tensor_gemm(A, B, C, M, N, K, maps)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        out[name] = {"M": M, "N": N, "K": K, "ms": ms, "tflops": 2.0 * M * N * K / (ms * 1e-3) / 1e12}
+        del A, B, C
+    out["probe_dmma_tflops"] = tt.probe_fp64_peak(0, 1 << 14)
+    print(json.dumps({"gemm_micro": out}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -383,7 +426,11 @@ def main():
     ap.add_argument("--config", default="c3", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gemm", default=None, help="kernel micro-benchmark: 'all' or one of " + ", ".join(GEMM_SHAPES))
     args = ap.parse_args()
+    if args.gemm:
+        run_gemm_micro(args)
+        return
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg, args.config)

@@ -17,7 +17,8 @@ constexpr int CH_NT = 256;
 // (lower; strict upper part of the block zeroed), Linv (nb x nb row-major, ld NB, lower) = L^-1.
 // A pivot <= 0 (or NaN) raises *flag.
 __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ A, long long lda, int nb,
-                                                          double *__restrict__ Linv, int *__restrict__ flag)
+                                                          double *__restrict__ Linv, int *__restrict__ flag,
+                                                          double *__restrict__ dminmax)
 {
     extern __shared__ double chol_sm[];
     double (*S)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(chol_sm);
@@ -67,6 +68,15 @@ __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ 
         Linv[r * NB + c] = W[r][c];
     }
     if (t == 0 && bad) *flag = 1;
+    if (t == 0 && dminmax) {
+        double lo = S[0][0], hi = S[0][0];
+        for (int j = 1; j < nb; ++j) {
+            lo = fmin(lo, S[j][j]);
+            hi = fmax(hi, S[j][j]);
+        }
+        dminmax[0] = lo;
+        dminmax[1] = hi;
+    }
 }
 
 // x[i][i] += shift_rel * max_diag ; one CTA
@@ -102,7 +112,30 @@ Ten view2(double *p, char a, long long na, long long sa, char b, long long nb_, 
     return t;
 }
 
+constexpr size_t CHOL_SMEM = 2 * NB * (NB + 1) * sizeof(double);
+
+void chol_attr()
+{
+    static bool attr_done = false;
+    if (!attr_done) {
+        TATRG_CUDA_CHECK(cudaFuncSetAttribute(chol_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CHOL_SMEM));
+        attr_done = true;
+    }
+}
+
 }  // namespace
+
+// Asynchronous: the n x n (n <= 64) block A (row-major, leading dimension lda) -> its lower Cholesky
+// factor in place, Linv (row-major, leading dimension 64) = L^-1, *flag raised on a non-positive
+// pivot, dminmax[0..1] = smallest / largest diagonal entry of L (a cheap condition estimate).
+void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax)
+{
+    if (n > NB) fail(-22, "chol_block: n = %d > %d", n, NB);
+    chol_attr();
+    chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(A, lda, n, Linv, flag, dminmax);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
 
 // In place: the n x n symmetric matrix A (row-major, lower triangle read) becomes its lower
 // Cholesky factor (upper triangle zeroed) after adding shift_rel * max_i A_ii to the diagonal.
@@ -118,16 +151,11 @@ bool cholesky_lower(double *A, int n, double shift_rel)
         count_launch();
     }
     double *tmp = ws_doubles((long long)n * NB);
-    constexpr size_t smem = 2 * NB * (NB + 1) * sizeof(double);
-    static bool attr_done = false;
-    if (!attr_done) {
-        TATRG_CUDA_CHECK(cudaFuncSetAttribute(chol_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    chol_attr();
     for (int j0 = 0; j0 < n; j0 += NB) {
         const int nb = n - j0 < NB ? n - j0 : NB;
         double *Ajj = A + (long long)j0 * n + j0;
-        chol_block_kernel<<<1, CH_NT, smem, stream()>>>(Ajj, n, nb, Linv, flag);
+        chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(Ajj, n, nb, Linv, flag, nullptr);
         TATRG_LAUNCH_CHECK();
         count_launch();
         const int rest = n - j0 - nb;

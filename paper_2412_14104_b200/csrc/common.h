@@ -49,6 +49,7 @@ struct GemmParams {
     int ksplit;            // >1: partial sums go to `partial`, reduced by a second kernel
     int ktiles_per_split;  // in units of BK
     double *partial;       // [ksplit][batch][M][N]
+    int tiles_n;           // set by the launcher: column tiles of the chosen CTA tile
 };
 
 // ---- context -------------------------------------------------------------------------
@@ -110,6 +111,7 @@ void transpose_small(const double *in, double *out, int rows, int cols);      //
 // chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
 // diagonal); false if a pivot was not positive
 bool cholesky_lower(double *A, int n, double shift_rel);
+void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);
 

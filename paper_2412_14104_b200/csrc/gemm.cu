@@ -16,6 +16,7 @@ namespace tatrg {
 namespace {
 
 constexpr int BK = 16;
+constexpr int RASTER_W = 12;
 
 __device__ __forceinline__ void cp_async8(double *smem_dst, const double *gsrc, bool valid)
 {
@@ -51,7 +52,18 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
     double *Bs = smem + STAGES * BK * LDA;
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+    // tile order: bands of RASTER_W row tiles, row tile fastest inside a band, so that the CTAs
+    // resident at one time cover a compact block of C and their operand tiles are shared in L2
+    int tile_m, tile_n;
+    {
+        const int tiles_m = (p.M + BM - 1) / BM;
+        const int band = blockIdx.x / (RASTER_W * p.tiles_n);
+        const int in_band = blockIdx.x - band * (RASTER_W * p.tiles_n);
+        const int w = min(RASTER_W, tiles_m - band * RASTER_W);
+        tile_n = in_band / w;
+        tile_m = band * RASTER_W + (in_band - tile_n * w);
+    }
+    const int m0 = tile_m * BM, n0 = tile_n * BN;
     int bz = blockIdx.z;
     const int split = bz / p.batch;
     bz -= split * p.batch;
@@ -248,7 +260,7 @@ __global__ void splitk_reduce_kernel(const __grid_constant__ GemmParams p)
 }
 
 template <int BM, int BN, int WM, int WN, int STAGES>
-void launch_cfg(const GemmParams &p)
+void launch_cfg(const GemmParams &p_in)
 {
     constexpr int NT = (BM / WM) * (BN / WN) * 32;
     constexpr size_t smem = (size_t)STAGES * BK * ((BM + 4) + (BN + 4)) * sizeof(double);
@@ -258,7 +270,11 @@ void launch_cfg(const GemmParams &p)
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    dim3 grid((p.M + BM - 1) / BM, (p.N + BN - 1) / BN, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
+    GemmParams p = p_in;
+    p.tiles_n = (p.N + BN - 1) / BN;
+    const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n;
+    if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
+    dim3 grid((unsigned)tiles, 1, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
     const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, BM == 128);
     kern<<<grid, NT, smem, stream()>>>(p);
     prof_end(slot);
@@ -279,11 +295,10 @@ void tensor_gemm(GemmParams p)
         TATRG_CUDA_CHECK(cudaGetDevice(&dev));
         TATRG_CUDA_CHECK(cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev));
     }
-    if ((long long)p.N / 64 + 1 > 65535) fail(-22, "tensor_gemm: N too large for grid.y");
     count_flops(2.0 * p.M * p.N * (double)p.K * p.batch);
     // tile choice: big tile when it still fills the machine, else the small one
     long long big_tiles = (long long)((p.M + 127) / 128) * ((p.N + 127) / 128) * p.batch;
-    bool big = big_tiles >= g_num_sms && p.M >= 96 && p.N >= 96;
+    bool big = big_tiles * 5 >= 4LL * g_num_sms && p.M >= 96 && p.N >= 96;
     long long tiles = big ? big_tiles : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
     int ktiles = (p.K + BK - 1) / BK;
     p.ksplit = 1;

@@ -8,7 +8,7 @@
 // reads v_j coalesced) and emits its n x n R.  The stacked R's are the next level's matrix.
 // Q is formed top-down: block b of level l applies its reflectors to [C_b; 0], C_b being rows
 // [b n, (b+1) n) of the level above; the top starts from diag(sign(R_jj)) so that R_ii >= 0.
-#include "common.h"
+#include "ctx.h"
 
 namespace tatrg {
 
@@ -247,9 +247,55 @@ void tsqr_impl(double *Y, long long m, int n, double *Rout)
 
 }  // namespace
 
+// Cholesky-QR2 for a tall, well-conditioned block: C = Y^T Y (tensor-GEMM, split-K), C = L L^T in one
+// CTA, Q = Y L^-T (tensor-GEMM), twice; R = L2^T L1^T has a positive diagonal, so this is the same
+// unique qr+ factorisation as the Householder route whenever it applies.  It applies when the
+// first Cholesky factor exists and its diagonal ratio (a lower bound of cond(Y)) is below 1e5, so
+// that cond^2 eps << 1; otherwise nothing has been written and the caller falls back to TSQR.
+bool cholqr2(double *Y, long long m, int n, double *Rout)
+{
+    size_t mark = ws_mark();
+    int *flag = (int *)ws_alloc(sizeof(int));
+    double *mm = ws_doubles(2);
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    Ten Ym = Ten::make(Y, "rc", {m, n});
+    Ten C1 = ws_tensor("cd", {n, n}), C2 = ws_tensor("cd", {n, n});
+    double *Li1 = ws_doubles(64 * 64), *Li2 = ws_doubles(64 * 64);
+    contract(Ym, Ym.as("rd"), C1);
+    chol_block(C1.p, n, n, Li1, flag, mm);
+    struct {
+        int f;
+        double lo, hi;
+    } h;
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.lo, mm, 2 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    if (h.f != 0 || !(h.lo > 1e-5 * h.hi)) {
+        ws_release(mark);
+        return false;
+    }
+    Ten T = ws_tensor("rd", {m, n});
+    Ten L1i = Ten::make(Li1, "dc", {n, 64});   // row d of L^-1; Q[r,d] = sum_c Y[r,c] Linv[d,c]
+    L1i.legs[1].n = n;
+    contract(Ym, L1i, T);
+    contract(T.as("rc"), T, C2);
+    chol_block(C2.p, n, n, Li2, flag, nullptr);
+    Ten L2i = Ten::make(Li2, "dc", {n, 64});
+    L2i.legs[1].n = n;
+    contract(T.as("rc"), L2i, Ym.as("rd"));
+    // R = L2^T L1^T : R[i][j] = sum_k L2[k][i] L1[j][k]   (C1, C2 now hold L1, L2; upper parts zeroed)
+    contract(C2.as("ki"), C1.as("jk"), Ten::make(Rout, "ij", {n, n}));
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    ws_release(mark);
+    if (h.f != 0) fail(-34, "cholqr2: second Cholesky factorisation failed");
+    return true;
+}
+
 void tsqr(double *Y, long long m, int n, double *Rout)
 {
     if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");
+    if (n <= 64 && m >= 16LL * n && m >= 4096 && cholqr2(Y, m, n, Rout)) return;
     if (n > 64) fail(-22, "tsqr: n = %d > 64 not supported yet", n);
     if (n > 32)
         tsqr_impl<64>(Y, m, n, Rout);
