@@ -84,6 +84,7 @@ struct Err {
 // ---- kernels (host launchers) ----------------------------------------------------------
 // gemm.cu
 void tensor_gemm(GemmParams p);
+void tensor_gemm_big(const GemmParams &p);   // gemm_big.cu: the 128x128 CTA tile
 double probe_fp64_peak(int mode, int iters);
 // qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
 // Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).

@@ -317,7 +317,7 @@ void tensor_gemm(GemmParams p)
     }
     if ((long long)p.batch * p.ksplit > 65535) fail(-22, "tensor_gemm: batch too large for grid.z");
     if (big)
-        launch_cfg<128, 128, 32, 32, 4>(p);
+        tensor_gemm_big(p);
     else
         launch_cfg<64, 64, 32, 32, 4>(p);
     if (p.ksplit > 1) {

@@ -1,0 +1,300 @@
+// gemm_big.cu -- the 128x128 CTA tile of the tensor-GEMM (see gemm.cu for the operation):
+//   C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)]
+// on the FP64 tensor pipe (mma.sync m8n8k4 -> DMMA.8x8x4).  This is the kernel the O(q r chi^7) bond
+// swap (Table 1) and the O(r^2 chi^7) triad contraction (Eqs. 13-14)
+// run on.
+//
+// 8 warps, warp tile 32 x 64 (64 FP64 accumulators per thread), BK = 16, 4-stage cp.async pipeline.
+// The shared-memory layout of an operand tile follows the operand's contiguous index in global
+// memory, so that 16-byte cp.async copies land on 16 consecutive bytes of shared memory:
+//   contiguous index = the free index (m or n):  tile stored [k][m], leading dimension 128 + 4
+//   contiguous index = the summed index k:       tile stored [m][k], leading dimension  16 + 4
+// Both leading dimensions are = 4 (mod 8) doubles, which makes the 8-byte DMMA fragment loads
+// (lane -> (row = lane/4, k = lane%4)) conflict free.  Leg permutations stay folded into the gather
+// addresses (Map4); the 16-byte path is taken when every pair of consecutive elements along the
+// contiguous index is 16-byte aligned in global memory (checked on the host), else 8-byte copies.
+#include "common.h"
+
+namespace tatrg {
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, NT = 256;
+constexpr int LD_F = BM + 4;   // [k][m] layout
+constexpr int LD_K = BK + 4;   // [m][k] layout
+constexpr int RASTER_W = 12;
+
+__device__ __forceinline__ void cp_async(double *smem_dst, const double *gsrc, int bytes, int vec)
+{
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    if (vec)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(d), "l"(gsrc), "r"(bytes));
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(d), "l"(gsrc), "r"(bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+__device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1)
+                 : "d"(a), "d"(b));
+}
+
+// Loader of one 128 x 16 operand tile.  KF: k is the contiguous index in global memory.
+// VEC: 16-byte copies (pairs along the contiguous index), else 8-byte copies.
+template <bool KF, bool VEC>
+struct TileLoader {
+    static constexpr int PER = VEC ? 4 : 8;          // copies per thread per tile
+    long long fix[PER];                               // offsets of the free index (fixed over k tiles)
+    int free_left[PER];                               // valid elements from this copy's free index on
+    const double *base;
+    int kl;                                           // this thread's k inside the tile
+    int soff[PER];                                    // shared-memory offsets
+
+    __device__ __forceinline__ void init(const double *b, const Map4 &mfree, int f0, int F, int t)
+    {
+        base = b;
+        if (KF) {
+            // k pairs (VEC) or singles along the 16-wide k; free index strided over threads
+            constexpr int KT = VEC ? 8 : 16;          // threads along k
+            kl = (t % KT) * (VEC ? 2 : 1);
+#pragma unroll
+            for (int j = 0; j < PER; ++j) {
+                int fl = t / KT + (NT / KT) * j;
+                free_left[j] = F - (f0 + fl);
+                fix[j] = free_left[j] > 0 ? map_off(mfree, f0 + fl) : 0;
+                soff[j] = fl * LD_K + kl;
+            }
+        } else {
+            // free-index pairs (VEC) or singles; 16 threads along the free index, k = t / 16
+            kl = t / 16;
+#pragma unroll
+            for (int j = 0; j < PER; ++j) {
+                int fl = ((t % 16) + 16 * j) * (VEC ? 2 : 1);
+                free_left[j] = F - (f0 + fl);
+                fix[j] = free_left[j] > 0 ? map_off(mfree, f0 + fl) : 0;
+                soff[j] = kl * LD_F + fl;
+            }
+        }
+    }
+
+    __device__ __forceinline__ void load(double *stage, const Map4 &mk, int k0, int K) const
+    {
+        const int k_left = K - (k0 + kl);
+        const long long ko = k_left > 0 ? map_off(mk, k0 + kl) : 0;
+#pragma unroll
+        for (int j = 0; j < PER; ++j) {
+            int n;   // valid elements of this copy
+            if (KF)
+                n = free_left[j] > 0 ? min(k_left, VEC ? 2 : 1) : 0;
+            else
+                n = k_left > 0 ? min(free_left[j], VEC ? 2 : 1) : 0;
+            n = max(n, 0);
+            cp_async(stage + soff[j], n > 0 ? base + fix[j] + ko : base, n * 8, VEC);
+        }
+    }
+};
+
+template <bool A_KF, bool B_KF, bool VEC>
+__global__ void __launch_bounds__(NT, 1) tgemm_big_kernel(const __grid_constant__ GemmParams p)
+{
+    constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
+    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_F;
+    constexpr int WM = 32, WN = 64, FM = WM / 8, FN = WN / 8;
+    extern __shared__ __align__(16) double smem[];
+    double *As = smem;
+    double *Bs = smem + STAGES * A_STAGE;
+
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    int tile_m, tile_n;
+    {
+        const int tiles_m = (p.M + BM - 1) / BM;
+        const int band = blockIdx.x / (RASTER_W * p.tiles_n);
+        const int in_band = blockIdx.x - band * (RASTER_W * p.tiles_n);
+        const int w = min(RASTER_W, tiles_m - band * RASTER_W);
+        tile_n = in_band / w;
+        tile_m = band * RASTER_W + (in_band - tile_n * w);
+    }
+    const int m0 = tile_m * BM, n0 = tile_n * BN;
+    int bz = blockIdx.z;
+    const int split = bz / p.batch;
+    bz -= split * p.batch;
+
+    int kt0 = 0, kt1 = (p.K + BK - 1) / BK;
+    if (p.ksplit > 1) {
+        kt0 = split * p.ktiles_per_split;
+        kt1 = min(kt1, kt0 + p.ktiles_per_split);
+    }
+    const int nkt = max(kt1 - kt0, 0);
+
+    TileLoader<A_KF, VEC> la;
+    TileLoader<B_KF, VEC> lb;
+    la.init(p.A + map_off(p.ab, bz), p.am, m0, p.M, t);
+    lb.init(p.B + map_off(p.bb, bz), p.bn, n0, p.N, t);
+
+    double acc[FM][FN][2];
+#pragma unroll
+    for (int i = 0; i < FM; ++i)
+#pragma unroll
+        for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    const int wm0 = (warp & 3) * WM, wn0 = (warp >> 2) * WN;
+    const int lr = lane >> 2, lk = lane & 3;
+    // fragment base offsets inside a stage
+    const int a_off = A_KF ? (wm0 + lr) * LD_K + lk : lk * LD_F + wm0 + lr;
+    const int b_off = B_KF ? (wn0 + lr) * LD_K + lk : lk * LD_F + wn0 + lr;
+    constexpr int A_I = A_KF ? 8 * LD_K : 8;        // step between 8-row fragments
+    constexpr int B_J = B_KF ? 8 * LD_K : 8;
+    constexpr int A_KK = A_KF ? 4 : 4 * LD_F;       // step between k groups of 4
+    constexpr int B_KK = B_KF ? 4 : 4 * LD_F;
+
+#pragma unroll
+    for (int s = 0; s < STAGES - 1; ++s) {
+        if (s < nkt) {
+            la.load(As + s * A_STAGE, p.ak, (kt0 + s) * BK, p.K);
+            lb.load(Bs + s * B_STAGE, p.bk, (kt0 + s) * BK, p.K);
+        }
+        cp_async_commit();
+    }
+    for (int it = 0; it < nkt; ++it) {
+        cp_async_wait<STAGES - 2>();
+        __syncthreads();
+        {
+            const int nx = it + STAGES - 1;
+            if (nx < nkt) {
+                la.load(As + (nx % STAGES) * A_STAGE, p.ak, (kt0 + nx) * BK, p.K);
+                lb.load(Bs + (nx % STAGES) * B_STAGE, p.bk, (kt0 + nx) * BK, p.K);
+            }
+            cp_async_commit();
+        }
+        const double *as = As + (it % STAGES) * A_STAGE + a_off;
+        const double *bs = Bs + (it % STAGES) * B_STAGE + b_off;
+#pragma unroll
+        for (int kk = 0; kk < BK / 4; ++kk) {
+            double a[FM], b[FN];
+#pragma unroll
+            for (int i = 0; i < FM; ++i) a[i] = as[kk * A_KK + i * A_I];
+#pragma unroll
+            for (int j = 0; j < FN; ++j) b[j] = bs[kk * B_KK + j * B_J];
+#pragma unroll
+            for (int i = 0; i < FM; ++i)
+#pragma unroll
+                for (int j = 0; j < FN; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    cp_async_wait<0>();
+
+    // ---- epilogue
+    if (p.ksplit > 1) {
+        double *P = p.partial + ((long long)split * p.batch + bz) * (long long)p.M * p.N;
+#pragma unroll
+        for (int i = 0; i < FM; ++i) {
+            int m = m0 + wm0 + i * 8 + lr;
+            if (m >= p.M) continue;
+#pragma unroll
+            for (int j = 0; j < FN; ++j) {
+                int n = n0 + wn0 + j * 8 + lk * 2;
+                if (n < p.N) P[(long long)m * p.N + n] = acc[i][j][0];
+                if (n + 1 < p.N) P[(long long)m * p.N + n + 1] = acc[i][j][1];
+            }
+        }
+        return;
+    }
+    double *Cb = p.C + map_off(p.cb, bz);
+    long long cmo[FM];
+    bool cmv[FM];
+#pragma unroll
+    for (int i = 0; i < FM; ++i) {
+        int m = m0 + wm0 + i * 8 + lr;
+        cmv[i] = m < p.M;
+        cmo[i] = cmv[i] ? map_off(p.cm, m) : 0;
+    }
+#pragma unroll
+    for (int j = 0; j < FN; ++j) {
+        const int n = n0 + wn0 + j * 8 + lk * 2;
+        const bool v0 = n < p.N, v1 = n + 1 < p.N;
+        const long long c0 = v0 ? map_off(p.cn, n) : 0;
+        const long long c1 = v1 ? map_off(p.cn, n + 1) : 0;
+#pragma unroll
+        for (int i = 0; i < FM; ++i) {
+            if (!cmv[i]) continue;
+            double *Cr = Cb + cmo[i];
+            if (v0) {
+                double v = p.alpha * acc[i][j][0];
+                if (p.accumulate) v += Cr[c0];
+                Cr[c0] = v;
+            }
+            if (v1) {
+                double v = p.alpha * acc[i][j][1];
+                if (p.accumulate) v += Cr[c1];
+                Cr[c1] = v;
+            }
+        }
+    }
+}
+
+template <bool A_KF, bool B_KF, bool VEC>
+void launch_big(const GemmParams &p_in)
+{
+    constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
+    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_F;
+    constexpr size_t smem = (size_t)STAGES * (A_STAGE + B_STAGE) * sizeof(double);
+    static bool attr_done = false;
+    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC>;
+    if (!attr_done) {
+        TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    GemmParams p = p_in;
+    p.tiles_n = (p.N + BN - 1) / BN;
+    const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n;
+    if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
+    dim3 grid((unsigned)tiles, 1, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
+    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, 1);
+    kern<<<grid, NT, smem, stream()>>>(p);
+    prof_end(slot);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
+
+bool even_or_inf(unsigned n) { return n == TATRG_RADIX_INF || (n & 1u) == 0; }
+bool even(long long s) { return (s & 1LL) == 0; }
+
+// every level above the first has an even stride
+bool upper_even(const Map4 &m) { return even(m.s1) && even(m.s2) && even(m.s3); }
+bool all_even(const Map4 &m) { return even(m.s0) && upper_even(m); }
+
+// 16-byte copies along the contiguous index `fast` of an operand (the other index is `slow`)
+bool vec_ok(const double *base, const Map4 &fast, const Map4 &slow, const Map4 &batch)
+{
+    return ((uintptr_t)base & 15) == 0 && fast.s0 == 1 && even_or_inf(fast.n0) && upper_even(fast) && all_even(slow) &&
+           all_even(batch);
+}
+
+}  // namespace
+
+void tensor_gemm_big(const GemmParams &p)
+{
+    const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;
+    const bool va = akf ? vec_ok(p.A, p.ak, p.am, p.ab) : vec_ok(p.A, p.am, p.ak, p.ab);
+    const bool vb = bkf ? vec_ok(p.B, p.bk, p.bn, p.bb) : vec_ok(p.B, p.bn, p.bk, p.bb);
+    const bool vec = va && vb;
+    if (akf) {
+        if (bkf)
+            vec ? launch_big<true, true, true>(p) : launch_big<true, true, false>(p);
+        else
+            vec ? launch_big<true, false, true>(p) : launch_big<true, false, false>(p);
+    } else {
+        if (bkf)
+            vec ? launch_big<false, true, true>(p) : launch_big<false, true, false>(p);
+        else
+            vec ? launch_big<false, false, true>(p) : launch_big<false, false, false>(p);
+    }
+}
+
+}  // namespace tatrg
