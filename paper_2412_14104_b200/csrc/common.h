@@ -94,6 +94,9 @@ void tsqr(double *Y, long long m, int n, double *Rout);
 // major) accumulates the rotations (G_in * V = G_out), s[n] = column norms (descending).
 void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long long strideG,
                 long long strideV, long long strideS);
+// jacobi_small.cu : one-CTA versions for m, n <= 64 (same output conventions)
+void svd_small(double *G, int m, int n, double *V, double *s);
+void eig_small(const double *S, int n, double *V, double *lam);   // symmetric S; V column j = eigenvector j
 // reduce.cu
 void sumsq(const double *x, long long n, double *out);                       // out[0] = sum x^2
 void dot(const double *x, const double *y, long long n, double *out);        // out[0] = sum x y

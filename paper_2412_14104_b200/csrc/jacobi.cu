@@ -158,6 +158,10 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
                 long long strideV, long long strideS)
 {
     if (n < 1 || m < 1 || batch < 1) return;
+    if (batch == 1 && m <= 64 && n <= 64) {
+        svd_small(G, m, n, V, s);
+        return;
+    }
     size_t mark = ws_mark();
     for (int b = 0; b < batch; ++b) fill_identity(V + b * strideV, n);
     const int npad = n + (n & 1);

@@ -1,0 +1,314 @@
+// jacobi_small.cu -- the small dense SVD / symmetric eigenproblems of the path solved by ONE CTA in
+// shared memory (no launch per rotation round): the l x l core of the RSVD (
+// reading O9), the canonical-form SVD, the Ritz step of the isometries (Eq. 3) and
+// the b x b cores of the squeezer's subspace iteration (Eq. 12).  n <= 64.
+//
+//   svd mode: one-sided (Hestenes) Jacobi on the columns of [G; V] stacked (V starts as identity),
+//             G_in V = U diag(s); round-robin ordering, warps own pairs, lanes own rows.
+//   sym mode: two-sided Jacobi on the symmetric S: S <- J^T S J, V <- V J; converges in a handful of
+//             sweeps whatever the grading of the spectrum and returns a complete orthonormal basis
+//             also when S is rank deficient (the one-sided iteration on a graded PSD matrix needs
+//             30+ sweeps: its columns start almost parallel).
+// Results are sorted by decreasing singular value / eigenvalue.
+#include "common.h"
+
+namespace tatrg {
+
+namespace {
+
+constexpr int SJ_NT = 256;
+constexpr int SJ_MAX = 64;
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void rr_pair(int round, int pi, int npad, int &p, int &q)
+{
+    const int nm1 = npad - 1;
+    if (pi == 0) {
+        p = nm1;
+        q = round;
+    } else {
+        p = (round + pi) % nm1;
+        q = (round - pi + nm1) % nm1;
+    }
+    if (p > q) {
+        int t = p;
+        p = q;
+        q = t;
+    }
+}
+
+// G: m x n column-major (ld = m) in global; on exit G = U diag(s) sorted, V (n x n column-major), s[n].
+__global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ Gg, int m, int n,
+                                                         double *__restrict__ Vg, double *__restrict__ sg,
+                                                         double tol, int max_sweeps, int *__restrict__ fail_flag)
+{
+    extern __shared__ double sm[];
+    const int ld = m + n;              // column j = sm[j*ld .. j*ld+m) (G part) then n entries of V
+    double *W = sm;
+    __shared__ int nrot;
+    __shared__ double fro2_s;
+    __shared__ double nrm[SJ_MAX];
+    __shared__ int perm[SJ_MAX];
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    constexpr int NW = SJ_NT / 32;
+
+    for (int i = t; i < n * ld; i += SJ_NT) {
+        int j = i / ld, r = i - j * ld;
+        W[i] = (r < m) ? Gg[(long long)j * m + r] : ((r - m == j) ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    {   // Frobenius norm (for the dead-column rule)
+        double a = 0.0;
+        for (int i = t; i < n * ld; i += SJ_NT) {
+            int r = i % ld;
+            if (r < m) a = fma(W[i], W[i], a);
+        }
+        a = warp_sum(a);
+        if (t == 0) fro2_s = 0.0;
+        __syncthreads();
+        if (lane == 0) atomicAdd(&fro2_s, a);
+        __syncthreads();
+    }
+    const double dead = 1e-40 * fro2_s;
+    const int npad = n + (n & 1);
+    int sweep = 0;
+    for (; n > 1 && sweep < max_sweeps; ++sweep) {
+        if (t == 0) nrot = 0;
+        __syncthreads();
+        for (int round = 0; round < npad - 1; ++round) {
+            for (int pi = warp; pi < npad / 2; pi += NW) {
+                int p, q;
+                rr_pair(round, pi, npad, p, q);
+                if (q >= n) continue;
+                double *cp = W + p * ld, *cq = W + q * ld;
+                double aa = 0.0, bb = 0.0, ab = 0.0;
+                for (int i = lane; i < m; i += 32) {
+                    double a = cp[i], b = cq[i];
+                    aa = fma(a, a, aa);
+                    bb = fma(b, b, bb);
+                    ab = fma(a, b, ab);
+                }
+                aa = warp_sum(aa);
+                bb = warp_sum(bb);
+                ab = warp_sum(ab);
+                if (aa == 0.0 && bb == 0.0) continue;
+                const bool swap = aa < bb;
+                double c = 1.0, s = 0.0;
+                bool rot = false;
+                if (aa > dead && bb > dead) {
+                    double cosv = fabs(ab) / sqrt(aa * bb);
+                    if (cosv > tol) {
+                        double zeta = (bb - aa) / (2.0 * ab);
+                        double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+                        c = 1.0 / sqrt(1.0 + tt * tt);
+                        s = c * tt;
+                        rot = true;
+                        if (lane == 0) atomicAdd(&nrot, 1);
+                    }
+                }
+                if (!rot && !swap) continue;
+                for (int i = lane; i < ld; i += 32) {
+                    double a = cp[i], b = cq[i];
+                    double na = c * a - s * b, nb = s * a + c * b;
+                    cp[i] = swap ? nb : na;
+                    cq[i] = swap ? na : nb;
+                }
+            }
+            __syncthreads();
+        }
+        if (nrot == 0) break;
+        __syncthreads();
+    }
+    if (t == 0 && sweep >= max_sweeps && n > 1) *fail_flag = 1;
+    // norms, ranks, permuted write-back
+    for (int j = warp; j < n; j += NW) {
+        double a = 0.0;
+        for (int i = lane; i < m; i += 32) a = fma(W[j * ld + i], W[j * ld + i], a);
+        a = warp_sum(a);
+        if (lane == 0) nrm[j] = sqrt(a);
+    }
+    __syncthreads();
+    if (t < n) {
+        double v = nrm[t];
+        int r = 0;
+        for (int i = 0; i < n; ++i) r += (nrm[i] > v) || (nrm[i] == v && i < t);
+        perm[r] = t;
+    }
+    __syncthreads();
+    for (int i = t; i < n * ld; i += SJ_NT) {
+        int j = i / ld, r = i - j * ld;
+        double v = W[perm[j] * ld + r];
+        if (r < m)
+            Gg[(long long)j * m + r] = v;
+        else
+            Vg[(long long)j * n + (r - m)] = v;
+    }
+    if (t < n) sg[t] = nrm[perm[t]];
+}
+
+// S: n x n symmetric (row- or column-major alike); on exit V (n x n, column j = eigenvector j,
+// stored column-major) and lam[n] descending.
+__global__ void __launch_bounds__(SJ_NT) eig_small_kernel(const double *__restrict__ Sg, int n,
+                                                         double *__restrict__ Vg, double *__restrict__ lg,
+                                                         int max_sweeps, int *__restrict__ fail_flag)
+{
+    extern __shared__ double sm[];
+    const int ld = n + 1;
+    double *S = sm;                 // S[r*ld + c]
+    double *V = sm + n * ld;        // V[c*ld + r] : column c contiguous
+    __shared__ double cs[SJ_MAX / 2][2];
+    __shared__ int pq[SJ_MAX / 2][2];
+    __shared__ double dmax;
+    __shared__ int nrot;
+    __shared__ double dg[SJ_MAX];
+    __shared__ int perm[SJ_MAX];
+    const int t = threadIdx.x;
+
+    for (int i = t; i < n * n; i += SJ_NT) {
+        int r = i / n, c = i - r * n;
+        S[r * ld + c] = 0.5 * (Sg[i] + Sg[(long long)c * n + r]);
+        V[c * ld + r] = (r == c) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    const int npad = n + (n & 1), half = npad / 2;
+    // entries below 1e-20 of the largest diagonal entry are dead (far below anything the path keeps)
+    if (t == 0) {
+        double d = 0.0;
+        for (int i = 0; i < n; ++i) d = fmax(d, fabs(S[i * ld + i]));
+        dmax = d;
+    }
+    __syncthreads();
+    const double floor_abs = 1e-20 * dmax;
+    int sweep = 0;
+    for (; n > 1 && sweep < max_sweeps; ++sweep) {
+        if (t == 0) nrot = 0;
+        __syncthreads();
+        for (int round = 0; round < npad - 1; ++round) {
+            if (t < half) {
+                int p, q;
+                rr_pair(round, t, npad, p, q);
+                double c = 1.0, s = 0.0;
+                if (q < n) {
+                    double apq = S[p * ld + q], app = S[p * ld + p], aqq = S[q * ld + q];
+                    // the classical relative criterion: a pair is converged when |a_pq| <= eps sqrt(|a_pp a_qq|)
+                    if (fabs(apq) > floor_abs && fabs(apq) > 2.2e-16 * sqrt(fabs(app * aqq))) {
+                        atomicAdd(&nrot, 1);
+                        double zeta = (aqq - app) / (2.0 * apq);
+                        double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
+                        c = 1.0 / sqrt(1.0 + tt * tt);
+                        s = c * tt;
+                    }
+                } else {
+                    q = -1;
+                }
+                pq[t][0] = p;
+                pq[t][1] = q;
+                cs[t][0] = c;
+                cs[t][1] = s;
+            }
+            __syncthreads();
+            // columns: S <- S J, V <- V J   (pair index = i / n, row = i % n)
+            for (int i = t; i < half * n; i += SJ_NT) {
+                int k = i / n, r = i - k * n;
+                int p = pq[k][0], q = pq[k][1];
+                if (q < 0) continue;
+                double c = cs[k][0], s = cs[k][1];
+                double a = S[r * ld + p], b = S[r * ld + q];
+                S[r * ld + p] = c * a - s * b;
+                S[r * ld + q] = s * a + c * b;
+                double va = V[p * ld + r], vb = V[q * ld + r];
+                V[p * ld + r] = c * va - s * vb;
+                V[q * ld + r] = s * va + c * vb;
+            }
+            __syncthreads();
+            // rows: S <- J^T S
+            for (int i = t; i < half * n; i += SJ_NT) {
+                int k = i / n, cc = i - k * n;
+                int p = pq[k][0], q = pq[k][1];
+                if (q < 0) continue;
+                double c = cs[k][0], s = cs[k][1];
+                double a = S[p * ld + cc], b = S[q * ld + cc];
+                S[p * ld + cc] = c * a - s * b;
+                S[q * ld + cc] = s * a + c * b;
+            }
+            __syncthreads();
+        }
+        if (nrot == 0) break;
+        __syncthreads();
+    }
+    if (t == 0 && sweep >= max_sweeps && n > 1) *fail_flag = 1;
+    if (t < n) dg[t] = S[t * ld + t];
+    __syncthreads();
+    if (t < n) {
+        double v = dg[t];
+        int r = 0;
+        for (int i = 0; i < n; ++i) r += (dg[i] > v) || (dg[i] == v && i < t);
+        perm[r] = t;
+    }
+    __syncthreads();
+    for (int i = t; i < n * n; i += SJ_NT) {
+        int j = i / n, r = i - j * n;
+        Vg[i] = V[perm[j] * ld + r];
+    }
+    if (t < n) lg[t] = dg[perm[t]];
+}
+
+bool attr_done = false;
+void set_attr()
+{
+    if (attr_done) return;
+    TATRG_CUDA_CHECK(cudaFuncSetAttribute(svd_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(SJ_MAX * 2 * SJ_MAX * sizeof(double))));
+    TATRG_CUDA_CHECK(cudaFuncSetAttribute(eig_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(2 * SJ_MAX * (SJ_MAX + 1) * sizeof(double))));
+    attr_done = true;
+}
+
+}  // namespace
+
+// One-CTA SVD; requires m, n <= 64.  Same contract as jacobi_svd (batch 1).
+void svd_small(double *G, int m, int n, double *V, double *s)
+{
+    if (m > SJ_MAX || n > SJ_MAX || m < 1 || n < 1) fail(-22, "svd_small: size %d x %d not supported", m, n);
+    set_attr();
+    size_t mark = ws_mark();
+    int *flag = (int *)ws_alloc(sizeof(int));
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    const int mn = m > n ? m : n;
+    const double tol = 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
+    const size_t smem = (size_t)n * (m + n) * sizeof(double);
+    svd_small_kernel<<<1, SJ_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+    int h = 0;
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    ws_release(mark);
+    if (h) fail(-34, "svd_small: no convergence (m=%d n=%d)", m, n);
+}
+
+// One-CTA symmetric eigensolver; n <= 64.  V column-major (column j = eigenvector j), lam descending.
+void eig_small(const double *S, int n, double *V, double *lam)
+{
+    if (n > SJ_MAX || n < 1) fail(-22, "eig_small: n = %d not supported", n);
+    set_attr();
+    size_t mark = ws_mark();
+    int *flag = (int *)ws_alloc(sizeof(int));
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    const size_t smem = (size_t)2 * n * (n + 1) * sizeof(double);
+    eig_small_kernel<<<1, SJ_NT, smem, stream()>>>(S, n, V, lam, 60, flag);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+    int h = 0;
+    TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    ws_release(mark);
+    if (h) fail(-34, "eig_small: no convergence (n=%d)", n);
+}
+
+}  // namespace tatrg

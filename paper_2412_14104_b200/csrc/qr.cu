@@ -295,7 +295,7 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
 void tsqr(double *Y, long long m, int n, double *Rout)
 {
     if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");
-    if (n <= 64 && m >= 16LL * n && m >= 4096 && cholqr2(Y, m, n, Rout)) return;
+    if (n <= 64 && m >= 16LL * n && m >= 512 && cholqr2(Y, m, n, Rout)) return;
     if (n > 64) fail(-22, "tsqr: n = %d > 64 not supported yet", n);
     if (n > 32)
         tsqr_impl<64>(Y, m, n, Rout);

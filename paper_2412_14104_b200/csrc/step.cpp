@@ -132,6 +132,10 @@ void stage_mark(int i)
 // (row-major n x n) are the eigenvectors, lam (device, n) descending; returns lam on the host.
 std::vector<double> sym_eig(double *S, int n, double *Vt, double *lam)
 {
+    if (n <= 64) {
+        eig_small(S, n, Vt, lam);
+        return d2h(lam, n);
+    }
     symmetrize(S, n);
     jacobi_svd(S, n, n, Vt, lam, 1, 0, 0, 0);
     return d2h(lam, n);
