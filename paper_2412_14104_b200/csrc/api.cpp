@@ -206,7 +206,8 @@ size_t tatrg_workspace_bytes(int chi, int r)
     // (state x2 generations, Q_Phi, Q_Psi, A, D, X, Y, Xs, Ys, G_ref, sketch + 3 RSVD blocks of
     // r chi^5, TSQR stacks, P of r^2 chi^5, EM of r chi^5) plus the chi^4-sized Gram intermediates.
     double c5 = pow((double)chi, 5), c4 = pow((double)chi, 4);
-    double doubles = c5 * (4 + 9 + 5.0 * r + 2.0 * r * r) + c4 * (16.0 * r * r + 64) + (1 << 22);
+    double doubles = c5 * (4 + 9 + 5.0 * r + 2.0 * r * r) + c4 * (16.0 * r * r + 64) + (1 << 22) +
+                     2.2 * c4 * chi * chi;   // the chi^6 slices of the plain ATRG contraction
     return (size_t)(doubles * 8.0 * 1.1) + ((size_t)64 << 20);
 }
 

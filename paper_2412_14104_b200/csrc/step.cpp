@@ -489,11 +489,18 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
     stage_mark(2);
 
-    if (mode != 0) fail(-22, "coarse_grain_atrg: not implemented yet");
-
+    Ten U[4];   // A, X, Y, D : [p,q,k]
+    Ten E, F, G, H;
+    long long kd = 0;
+    Ten GL[3], GR[3];
+    const long long nn[3] = {n1, n2, n3};
+    for (int mu = 0; mu < 3; ++mu) {
+        GL[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
+        GR[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
+    }
+    if (mode == 0) {
     // =================== O4 oversampled isometries (Eqs. 2-3) ===================
     const int kk = (int)std::min<long long>((long long)r * chi, n12);
-    Ten U[4];   // A, X, Y, D : [p,q,k]
     if (kk >= n12) {
         for (int i = 0; i < 4; ++i) {
             U[i] = ws_tensor("pqk", {n1, n2, n12});
@@ -541,12 +548,14 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(Ten::make(Qi.p, "pqz", {n1, n2, kk}), Vt, U[i]);
         }
     }
-    const long long kd = U[0].legs[2].n;
+    kd = U[0].legs[2].n;
     stage_mark(3);
 
     // =================== O5 triad tensors (Eqs. 4-7) ===================
-    Ten E = ws_tensor("xkta", {n0, kd, n3, a}), F = ws_tensor("aktg", {a, kd, n3, gs});
-    Ten G = ws_tensor("bktg", {a, kd, n3, gs}), H = ws_tensor("xktb", {n0, kd, n3, a});
+    E = ws_tensor("xkta", {n0, kd, n3, a});
+    F = ws_tensor("aktg", {a, kd, n3, gs});
+    G = ws_tensor("bktg", {a, kd, n3, gs});
+    H = ws_tensor("xktb", {n0, kd, n3, a});
     contract(A.as("xpqta"), U[0], E);
     contract(Xs.as("apqtg"), U[1], F);     // sigma is inside Xs (Eq. 5)
     contract(Y.as("bpqtg"), U[2], G);
@@ -554,12 +563,6 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     stage_mark(4);
 
     // =================== O6 Gram matrices of Gamma^triad (Eq. 12) ===================
-    Ten GL[3], GR[3];
-    const long long nn[3] = {n1, n2, n3};
-    for (int mu = 0; mu < 3; ++mu) {
-        GL[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
-        GR[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
-    }
     {
         size_t mk = ws_mark();
         Ten HH0 = ws_tensor("bc", {a, a}), EE0 = ws_tensor("ab", {a, a});
@@ -611,6 +614,38 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             ws_release(mk2);
         }
         ws_release(mk);
+    }
+    } else {
+        // =================== plain ATRG (Table 1): squeezer Grams of A X sigma and of
+        // sigma Y D only (the canonical form drops the other half; Table 1 "Squeezer step O(chi^7)")
+        stage_mark(3);
+        stage_mark(4);
+        // leg letters of the three transverse legs: upper (p,q,t) / bar (P,Q,T); lower (r,s,u) / bar (R,S,U)
+        const char up[3] = {'p', 'q', 't'}, ub[3] = {'P', 'Q', 'T'};
+        for (int mu = 0; mu < 3; ++mu) {
+            size_t mk = ws_mark();
+            const long long nm = nn[mu];
+            char n1s[6] = "xpqta", n2s[6] = "xpqtb";
+            n2s[1 + mu] = ub[mu];
+            char o[5] = {up[mu], 'a', ub[mu], 'b', 0};
+            Ten AA = ws_tensor("taub", {nm, a, nm, a});
+            contract(A.as(n1s), A.as(n2s), AA.as(o));                    // AA[i, al, ibar, albar]
+            char x1[6] = "apqtg", x2[6] = "bpqtg";
+            x2[1 + mu] = ub[mu];
+            char ox[5] = {'a', up[mu], 'b', ub[mu], 0};
+            Ten XX = ws_tensor("asbv", {a, nm, a, nm});
+            contract(Xs.as(x1), Xs.as(x2), XX.as(ox));                   // XX[al, i', albar, ibar']
+            contract(AA.as("taub"), XX.as("asbv"), GL[mu].as("tsuv"));   // G^L[(up,lo),(upbar,lobar)]
+            Ten YY = AA, DD = XX;                                        // reuse the buffers
+            YY = Ten::make(AA.p, "btcu", {a, nm, a, nm});
+            DD = Ten::make(XX.p, "sbvc", {nm, a, nm, a});
+            char oy[5] = {'a', up[mu], 'b', ub[mu], 0};
+            contract(Ys.as(x1), Ys.as(x2), YY.as(oy));                   // YY[be, j, bebar, jbar]
+            char od[5] = {up[mu], 'a', ub[mu], 'b', 0};
+            contract(D.as(n1s), D.as(n2s), DD.as(od));                   // DD[j', be, jbar', bebar]
+            contract(YY.as("btcu"), DD.as("sbvc"), GR[mu].as("tsuv"));
+            ws_release(mk);
+        }
     }
     stage_mark(5);
 
@@ -697,7 +732,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         return t;
     };
     if ((size_t)(n0 * m1 * m2 * m3 * gs) * 8 > new_cap) fail(-12, "internal: new state exceeds its reservation");
-    for (int side = 0; side < 2; ++side) {
+    for (int side = 0; side < 2 && mode == 0; ++side) {
         size_t mk = ws_mark();
         Ten W1 = ws_tensor("qkPm", {n2, kd, n1, m1}), V2 = ws_tensor("Plqn", {n1, kd, n2, m2});
         Ten Qt = ws_tensor("klmn", {kd, kd, m1, m2});
@@ -721,6 +756,41 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkatw"));
             contract(EM.as("xkatw"), G.as("altg"), Pt);   // Pt[x, kD, w, kY, g]
             contract(Pt.as("xlwkg"), Qt, out.as("xmnwg"));
+        }
+        ws_release(mk);
+    }
+    if (mode != 0) {
+        // plain ATRG contraction, O(chi^9) (Table 1): Phi = sum A (X sigma) M1 M2 M3,
+        // Psi = sum Y D N1 N2 N3, one slice of the direction-0 leg at a time (the chi^7-sized
+        // intermediate of the whole tensor would not fit)
+        size_t mk = ws_mark();
+        Ten T1 = ws_tensor("qtarm", {n2, n3, a, n1, m1});          // per x: A[x] M1
+        Ten T2 = ws_tensor("qtmsug", {n2, n3, m1, n2, n3, gs});    // . (X sigma) over (a, r)
+        Ten T3 = ws_tensor("tmnug", {n3, m1, m2, n3, gs});         // . M2 over (q, s)
+        Ten outP = new_view(phi_new), outS = new_view(psi_new);
+        for (long long x = 0; x < n0; ++x) {
+            Ten Ax = Ten::make(A.p + x * (n1 * n2 * n3 * a), "pqta", {n1, n2, n3, a});
+            contract(Ax, Ms[0].as("prm"), T1);
+            contract(T1, Xs.as("arsug"), T2);
+            contract(T2, Ms[1].as("qsn"), T3);
+            Ten ox = outP;
+            ox.p += x * ox.legs[0].stride;
+            ox.legs.erase(ox.legs.begin());
+            contract(T3, Ms[2].as("tuw"), ox.as("mnwg"));
+        }
+        // Psi[x,m,n,w,g] = sum Y[b,p,q,t,g] D[x,r,s,u,b] N1[m,p,r] N2[n,q,s] N3[w,t,u]
+        Ten S1 = ws_tensor("subpm", {n2, n3, a, n1, m1});          // per x: D[x] N1 over r
+        Ten S2 = ws_tensor("sumqtg", {n2, n3, m1, n2, n3, gs});    // . Y over (b, p)
+        Ten S3 = ws_tensor("umntg", {n3, m1, m2, n3, gs});         // . N2 over (q, s)
+        for (long long x = 0; x < n0; ++x) {
+            Ten Dx = Ten::make(D.p + x * (n1 * n2 * n3 * a), "rsub", {n1, n2, n3, a});
+            contract(Dx, Ns[0].as("mpr"), S1);
+            contract(S1, Y.as("bpqtg"), S2);
+            contract(S2, Ns[1].as("nqs"), S3);
+            Ten ox = outS;
+            ox.p += x * ox.legs[0].stride;
+            ox.legs.erase(ox.legs.begin());
+            contract(S3, Ns[2].as("wtu"), ox.as("mnwg"));
         }
         ws_release(mk);
     }

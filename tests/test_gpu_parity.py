@@ -27,7 +27,7 @@ def tt():
     t.destroy()
 
 
-def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None):
+def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None, mode="triad"):
     """Oracle and GPU step by step; returns list of per-step comparison records."""
     recs = []
     st = orc.init_ising_tensor(beta, h)
@@ -35,8 +35,8 @@ def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None):
     assert abs(tt.log_Z_per_site() / orc.log_Z_per_site(st) - 1) < 1e-13
     for m in range(n_steps):
         d = directions[m % len(directions)] if directions else (m % 4) + 1
-        rec = orc.coarse_grain(st, d, chi, r, q, driver.seeded_inputs_for(seed, m))
-        tt.coarse_grain(d, chi, r, q, seed)
+        rec = orc.coarse_grain(st, d, chi, r, q, driver.seeded_inputs_for(seed, m), mode=mode)
+        (tt.coarse_grain if mode == "triad" else tt.coarse_grain_atrg)(d, chi, r, q, seed)
         out = {"step": m, "lnz_o": orc.log_Z_per_site(st), "lnz_g": tt.log_Z_per_site(),
                "dims_o": st.dims, "dims_g": tt.get_dims()[:5], "spec": {}}
         for name in ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3"):
@@ -79,3 +79,33 @@ def test_config2_chi16_first_steps(tt):
     """BASELINE.json configs[1] (T=6.65, chi=16, r=2, q=2): the first 10 of its 40 steps (the oracle
     needs ~seconds per step at chi=16)."""
     check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 10, 20241215))
+
+
+def test_plain_atrg_parity(tt):
+    """coarse_grain_atrg (Table 1: no triads, O(chi^9) contraction) against the oracle's
+    mode='atrg' on the same seeded bond-swap sketches."""
+    check(run_both(tt, 1 / 6.65, 0.0, 6, 2, 2, 6, 20241217, mode="atrg"))
+
+
+def test_triad_equals_atrg_when_r_chi_covers_pair_gpu(tt):
+    """r*chi >= d2*d3 => the isometries are identities and Triad-ATRG is ATRG (GPU vs GPU)."""
+    out = []
+    for fn in (tt.coarse_grain, tt.coarse_grain_atrg):
+        tt.init_ising_tensor(1 / 6.0, 0.02)
+        for m in range(4):
+            fn(m % 4 + 1, 4, 4, 2, 31)
+        out.append(tt.log_Z_per_site())
+    assert abs(out[0] / out[1] - 1) < 1e-12, out
+
+
+def test_config4_atrg_chi24_vs_triad(tt):
+    """BASELINE.json configs[3] shape check at reduced length: plain ATRG chi=24 (O(chi^9) GEMM
+    13824 x 13824 x 576 per slice), 5 steps, against a Triad-ATRG run at the same chi: the free
+    energies agree to truncation level (PAPER.md:139 quotes 0.0013 % at chi=54; not a pin)."""
+    out = []
+    for fn in (tt.coarse_grain_atrg, tt.coarse_grain):
+        tt.init_ising_tensor(1 / 6.65, 0.0)
+        for m in range(5):
+            fn(m % 4 + 1, 24, 2, 2, 20241217)
+        out.append(tt.log_Z_per_site())
+    assert abs(out[0] / out[1] - 1) < 1e-4, out
