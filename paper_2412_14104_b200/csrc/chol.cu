@@ -16,63 +16,116 @@ constexpr int CH_NT = 256;
 // One CTA: A (nb x nb, row-major, leading dimension lda, lower triangle used) -> L in place
 // (lower; strict upper part of the block zeroed), Linv (nb x nb row-major, ld NB, lower) = L^-1.
 // A pivot <= 0 (or NaN) raises *flag.
+//
+// Right-looking, register tiled: thread (ty, tx) of the 16 x 16 grid owns the cyclic 4 x 4 sub-blocks
+// S[ty+16a][tx+16b] of the (symmetrised) block and of W = L^-1 (forward substitution L W = I fused
+// into the same loop).  Per step j the pivot column of S and the pivot row of W go through a
+// double-buffered shared-memory line: one barrier per step.  A block smaller than 64 is padded
+// with the identity.
 __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ A, long long lda, int nb,
                                                           double *__restrict__ Linv, int *__restrict__ flag,
-                                                          double *__restrict__ dminmax)
+                                                          double *__restrict__ dminmax, double shift_rel)
 {
-    extern __shared__ double chol_sm[];
-    double (*S)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(chol_sm);
-    double (*W)[NB + 1] = reinterpret_cast<double (*)[NB + 1]>(chol_sm + NB * (NB + 1));
+    __shared__ double col[2][NB];
+    __shared__ double wrow[2][NB];
+    __shared__ double diag[NB];
     __shared__ int bad;
-    const int t = threadIdx.x;
+    const int t = threadIdx.x, ty = t >> 4, tx = t & 15;
     if (t == 0) bad = 0;
-    for (int i = t; i < nb * nb; i += CH_NT) {
-        int r = i / nb, c = i - r * nb;
-        S[r][c] = (c <= r) ? A[r * lda + c] : 0.0;
-    }
+    double s[4][4], w[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int i = ty + 16 * a, c = tx + 16 * b;
+            const int r = i > c ? i : c, cc = i > c ? c : i;   // lower-triangle source
+            s[a][b] = (r < nb) ? A[r * lda + cc] : (i == c ? 1.0 : 0.0);
+            w[a][b] = (i == c) ? 1.0 : 0.0;
+            if (i == c) diag[i] = (i < nb) ? s[a][b] : 0.0;
+        }
     __syncthreads();
-    for (int j = 0; j < nb; ++j) {
-        // column j: S[j][j] = sqrt(pivot), S[i][j] /= S[j][j]
-        double piv = S[j][j];
+    if (shift_rel > 0.0) {   // A + shift_rel * max_i A_ii on the diagonal
+        double mx = 0.0;
+        for (int i = 0; i < NB; ++i) mx = fmax(mx, diag[i]);
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b)
+                if (ty + 16 * a == tx + 16 * b && ty + 16 * a < nb) s[a][b] += shift_rel * mx;
         __syncthreads();
+    }
+#pragma unroll 1
+    for (int j = 0; j < NB; ++j) {
+        const int buf = j & 1, bj = j >> 4;
+        if (tx == (j & 15)) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                double v = s[a][0];
+                if (bj == 1) v = s[a][1];
+                if (bj == 2) v = s[a][2];
+                if (bj == 3) v = s[a][3];
+                col[buf][ty + 16 * a] = v;
+            }
+        }
+        if (ty == (j & 15)) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                double v = w[0][b];
+                if (bj == 1) v = w[1][b];
+                if (bj == 2) v = w[2][b];
+                if (bj == 3) v = w[3][b];
+                wrow[buf][tx + 16 * b] = v;
+            }
+        }
+        __syncthreads();
+        double piv = col[buf][j];
         if (!(piv > 0.0)) {
             if (t == 0) bad = 1;
             piv = 1.0;
         }
-        const double d = sqrt(piv);
-        if (t == 0) S[j][j] = d;
-        for (int i = j + 1 + t; i < nb; i += CH_NT) S[i][j] /= d;
-        __syncthreads();
-        // trailing update of the lower triangle: S[i][c] -= S[i][j] S[c][j], j < c <= i
-        const int rem = nb - j - 1;
-        for (int e = t; e < rem * rem; e += CH_NT) {
-            int i = j + 1 + e / rem, c = j + 1 + e % rem;
-            if (c <= i) S[i][c] = fma(-S[i][j], S[c][j], S[i][c]);
+        const double d = sqrt(piv), rd = 1.0 / d;
+        if (t == 0) diag[j] = d;
+        double li[4], lc[4], wj[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const int i = ty + 16 * a;
+            li[a] = (i > j) ? col[buf][i] * rd : 0.0;
         }
-        __syncthreads();
-    }
-    // inverse of the lower-triangular L: column c of W solved by forward substitution, one
-    // thread per column (nb <= 64 columns; tiny)
-    if (t < nb) {
-        const int c = t;
-        for (int i = 0; i < nb; ++i) {
-            double s = (i == c) ? 1.0 : 0.0;
-            for (int k = c; k < i; ++k) s = fma(-S[i][k], W[k][c], s);
-            W[i][c] = (i >= c) ? s / S[i][i] : 0.0;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int c = tx + 16 * b;
+            lc[b] = (c > j) ? col[buf][c] * rd : 0.0;
+            wj[b] = wrow[buf][c] * rd;
+        }
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const int i = ty + 16 * a;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int c = tx + 16 * b;
+                s[a][b] = fma(-li[a], lc[b], s[a][b]);
+                if (c == j) s[a][b] = (i > j) ? li[a] : (i == j ? d : 0.0);   // finished column of L
+                w[a][b] = (i == j) ? wj[b] : fma(-li[a], wj[b], w[a][b]);
+            }
         }
     }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int i = ty + 16 * a, c = tx + 16 * b;
+            if (i < nb && c < nb) {
+                A[i * lda + c] = (c <= i) ? s[a][b] : 0.0;
+                Linv[i * NB + c] = (c <= i) ? w[a][b] : 0.0;
+            }
+        }
     __syncthreads();
-    for (int i = t; i < nb * nb; i += CH_NT) {
-        int r = i / nb, c = i - r * nb;
-        A[r * lda + c] = S[r][c];
-        Linv[r * NB + c] = W[r][c];
-    }
     if (t == 0 && bad) *flag = 1;
     if (t == 0 && dminmax) {
-        double lo = S[0][0], hi = S[0][0];
+        double lo = diag[0], hi = diag[0];
         for (int j = 1; j < nb; ++j) {
-            lo = fmin(lo, S[j][j]);
-            hi = fmax(hi, S[j][j]);
+            lo = fmin(lo, diag[j]);
+            hi = fmax(hi, diag[j]);
         }
         dminmax[0] = lo;
         dminmax[1] = hi;
@@ -112,7 +165,7 @@ Ten view2(double *p, char a, long long na, long long sa, char b, long long nb_, 
     return t;
 }
 
-constexpr size_t CHOL_SMEM = 2 * NB * (NB + 1) * sizeof(double);
+constexpr size_t CHOL_SMEM = 0;
 
 void chol_attr()
 {
@@ -127,12 +180,13 @@ void chol_attr()
 
 // Asynchronous: the n x n (n <= 64) block A (row-major, leading dimension lda) -> its lower Cholesky
 // factor in place, Linv (row-major, leading dimension 64) = L^-1, *flag raised on a non-positive
-// pivot, dminmax[0..1] = smallest / largest diagonal entry of L (a cheap condition estimate).
-void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax)
+// pivot, dminmax[0..1] = smallest / largest diagonal entry of L (a cheap condition estimate);
+// shift_rel > 0 adds shift_rel * max_i A_ii to the diagonal first.
+void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel)
 {
     if (n > NB) fail(-22, "chol_block: n = %d > %d", n, NB);
     chol_attr();
-    chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(A, lda, n, Linv, flag, dminmax);
+    chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(A, lda, n, Linv, flag, dminmax, shift_rel);
     TATRG_LAUNCH_CHECK();
     count_launch();
 }
@@ -155,7 +209,7 @@ bool cholesky_lower(double *A, int n, double shift_rel)
     for (int j0 = 0; j0 < n; j0 += NB) {
         const int nb = n - j0 < NB ? n - j0 : NB;
         double *Ajj = A + (long long)j0 * n + j0;
-        chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(Ajj, n, nb, Linv, flag, nullptr);
+        chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(Ajj, n, nb, Linv, flag, nullptr, 0.0);
         TATRG_LAUNCH_CHECK();
         count_launch();
         const int rest = n - j0 - nb;

@@ -89,6 +89,12 @@ double probe_fp64_peak(int mode, int iters);
 // qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
 // Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).
 void tsqr(double *Y, long long m, int n, double *Rout);
+// Asynchronous Cholesky-QR of a tall block (n <= 64): `passes` rounds of {C = Y^T Y (+ shift_rel * max diag),
+// C = L L^T, Y <- Y L^-T}; no host synchronisation.  A failed factorisation raises *flag_dev (sticky);
+// ratio_dev (optional) receives min / max of the first pass's diag(L); Rout (optional, n x n row-major)
+// receives the accumulated triangular factor.  The caller checks the flag when it next synchronises.
+void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
+                  double *Rout);
 // jacobi.cu : one-sided Jacobi SVD of `batch` column-major m x n matrices (ld = m), m >= n.
 // On exit G = U*diag(s) (columns orthogonal, sorted by decreasing norm), V (n x n, column
 // major) accumulates the rotations (G_in * V = G_out), s[n] = column norms (descending).
@@ -115,7 +121,7 @@ void transpose_small(const double *in, double *out, int rows, int cols);      //
 // chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
 // diagonal); false if a pivot was not positive
 bool cholesky_lower(double *A, int n, double shift_rel);
-void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax);
+void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel = 0.0);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);
 

@@ -16,7 +16,7 @@ namespace tatrg {
 
 namespace {
 
-constexpr int SJ_NT = 256;
+constexpr int SJ_NT = 1024;
 constexpr int SJ_MAX = 64;
 
 __device__ __forceinline__ double warp_sum(double v)

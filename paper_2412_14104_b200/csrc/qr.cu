@@ -292,6 +292,42 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
     return true;
 }
 
+void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
+                  double *Rout)
+{
+    if (n < 1 || n > 64 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
+    size_t mark = ws_mark();
+    Ten Ym = Ten::make(Y, "rc", {m, n});
+    Ten T = ws_tensor("rd", {m, n});
+    Ten C[3];
+    double *Li = ws_doubles(64 * 64);
+    Ten cur = Ym, nxt = T;
+    for (int p = 0; p < passes; ++p) {
+        C[p] = ws_tensor("cd", {n, n});
+        contract(cur.as("rc"), cur.as("rd"), C[p]);
+        chol_block(C[p].p, n, n, Li, flag_dev, p == 0 ? ratio_dev : nullptr, p == 0 ? shift_rel : 0.0);
+        Ten Linv = Ten::make(Li, "dc", {n, 64});   // Q[r,d] = sum_c Y[r,c] Linv[d,c]
+        Linv.legs[1].n = n;
+        contract(cur.as("rc"), Linv, nxt.as("rd"));
+        std::swap(cur, nxt);
+    }
+    if (cur.p != Y) TATRG_CUDA_CHECK(cudaMemcpyAsync(Y, cur.p, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, stream()));
+    if (Rout) {
+        // R = L_p^T ... L_1^T (the C[p] now hold the lower factors, upper parts zeroed)
+        Ten Rm = Ten::make(Rout, "ij", {n, n});
+        if (passes == 1) {
+            transpose_small(C[0].p, Rout, n, n);
+        } else if (passes == 2) {
+            contract(C[1].as("ki"), C[0].as("jk"), Rm);          // R[i][j] = sum_k L2[k][i] L1[j][k]
+        } else {
+            Ten R12 = ws_tensor("kj", {n, n});
+            contract(C[1].as("lk"), C[0].as("jl"), R12);         // (L2^T L1^T)[k][j]
+            contract(C[2].as("ki"), R12, Rm);
+        }
+    }
+    ws_release(mark);
+}
+
 void tsqr(double *Y, long long m, int n, double *Rout)
 {
     if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");

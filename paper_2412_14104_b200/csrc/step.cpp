@@ -192,8 +192,15 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
 // convergence, so the result does not depend on it beyond rounding).
 Ten solver_start_block(long long rows, long long cols, int tag, const char *names2)
 {
-    std::vector<double> host((size_t)(rows * cols));
-    si_fill_gauss(host.data(), (uint64_t)(rows * cols), si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
+    static std::vector<double> cache[4];
+    static long long cache_n[4] = {0, 0, 0, 0};
+    std::vector<double> local;
+    std::vector<double> &host = (tag >= 0 && tag < 4) ? cache[tag] : local;
+    if ((tag < 0 || tag >= 4) || cache_n[tag] != rows * cols) {
+        host.resize((size_t)(rows * cols));
+        si_fill_gauss(host.data(), (uint64_t)(rows * cols), si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
+        if (tag >= 0 && tag < 4) cache_n[tag] = rows * cols;
+    }
     Ten t = ws_tensor(names2, {rows, cols});
     h2d(t.p, host.data(), rows * cols);
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
@@ -225,41 +232,76 @@ bool squeezer_subspace(const Ten &GLm, const Ten &GRm, int N2, int chi, int mu, 
     if (!cholesky_lower(LL.p, N2, shift) || !cholesky_lower(LR.p, N2, shift)) return false;
     Ten F = ws_tensor("ij", {N2, N2});
     contract(LL, LR, F);                                   // F = L_L^T L_R
-    auto apply = [&](const double *w, double *out) {       // F w
+    auto mulF = [&](const double *w, double *out) {        // F w
         contract(F, Ten::make(const_cast<double *>(w), "jz", {N2, b}), Ten::make(out, "iz", {N2, b}));
     };
-    auto apply_t = [&](const double *w, double *out) {     // F^T w
+    auto mulFt = [&](const double *w, double *out) {       // F^T w
         contract(F, Ten::make(const_cast<double *>(w), "iz", {N2, b}), Ten::make(out, "jz", {N2, b}));
     };
+    // Subspace iteration Q <- orth(F orth(F^T Q)).  Between iterations one (shifted) Cholesky-QR pass
+    // is enough: only the span is carried on; the two blocks that enter the Ritz step get two passes.
+    int *flag = (int *)ws_alloc(sizeof(int));
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    double *ratio = ws_doubles(4);
     Ten om = solver_start_block(N2, b, mu, "jz");
-    double *left = ws_doubles((long long)N2 * b), *right = ws_doubles((long long)N2 * b);
-    int iters = 2;
-    for (int pass = 0; pass < 2; ++pass) {
-        size_t mk = ws_mark();
-        RsvdOut ro = rsvd(apply, apply_t, om, N2, N2, b, iters, chi, left, right);
-        if (pass == 0) {
-            const double rho = ro.s_full[b - 1] / ro.s_full[chi - 1];
-            if (!(ro.s_full[chi - 1] > 1e-6 * ro.s_full[0])) return false;
-            int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
-            iters = std::max(3, std::min(need + 1, 80));
-            ws_release(mk);
-            continue;
-        }
-        o.k = ro.k;
-        o.s = ro.s_full;
-        o.gap = rel_gap(ro.s_full, ro.k);
-        std::vector<double> keep(ro.s_full.begin(), ro.s_full.begin() + ro.k);
-        ws_release(mk);
-        o.s_dev = ws_doubles(ro.k);
-        h2d(o.s_dev, keep.data(), ro.k);
-        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    double *Q = ws_doubles((long long)N2 * b), *Qt = ws_doubles((long long)N2 * b);
+    double *Rb = ws_doubles((long long)b * b), *V = ws_doubles((long long)b * b), *sv = ws_doubles(b);
+    const double it_shift = 1e-13;
+    mulF(om.p, Q);
+    cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
+    auto ritz_blocks = [&](std::vector<double> &sh) {      // Q <- orth2(F Qt) is done by the caller
+        mulFt(Q, Qt);                                      // B^T = F^T Q = Q_B R_B
+        cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
+        jacobi_svd(Rb, b, b, V, sv, 1, 0, 0, 0);           // R_B^T V = U diag(s)
+        struct {
+            int f;
+            double r[4];
+        } h;
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(h.r, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+        sh = d2h(sv, b);
+        // a failed factorisation, or a block too ill conditioned for two Cholesky-QR passes
+        return h.f == 0 && h.r[0] > 1e-5 * h.r[1] && h.r[2] > 1e-5 * h.r[3];
+    };
+    for (int it = 0; it < 2; ++it) {
+        mulFt(Q, Qt);
+        cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
+        mulF(Qt, Q);
+        cholqr_async(Q, N2, b, it == 1 ? 2 : 1, it == 1 ? 0.0 : it_shift, flag, it == 1 ? ratio : nullptr, nullptr);
     }
+    std::vector<double> sh;
+    if (!ritz_blocks(sh)) return false;
+    if (!(sh[chi - 1] > 1e-6 * sh[0])) return false;
+    const double rho = sh[b - 1] / sh[chi - 1];
+    const int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
+    const int more = std::max(1, std::min(need + 1, 80) - 2);   // two iterations are done
+    for (int it = 0; it < more; ++it) {
+        const bool last = it == more - 1;
+        mulF(Qt, Q);                                       // Qt = orth(F^T Q) from the Ritz step / the loop
+        cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
+        if (!last) {
+            mulFt(Q, Qt);
+            cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
+        }
+    }
+    if (!ritz_blocks(sh)) return false;
+    o.k = num_rank(sh, chi);
     if (o.k < chi) return false;
     const int k = o.k;
+    o.s = sh;
+    o.gap = rel_gap(sh, k);
+    o.s_dev = sv;
+    scale_leg(Rb, (long long)k * b, b, k, sv, 1);          // columns of U
+    Ten Uk = Ten::make(Rb, "kz", {b, b}), Vk = Ten::make(V, "kz", {b, b});
+    Uk.legs[0].n = k;
+    Vk.legs[0].n = k;
+    Ten left = ws_tensor("ik", {N2, k}), right = ws_tensor("jk", {N2, k});
+    contract(Ten::make(Q, "iz", {N2, b}), Uk, left);
+    contract(Ten::make(Qt, "jz", {N2, b}), Vk, right);
     Mr = ws_tensor("nk", {N2, k});
     Nr = ws_tensor("kn", {k, N2});
-    contract(Ten::make(left, "ik", {N2, k}), LL.as("ni"), Nr);    // N = s^-1/2 U^T L_L^T
-    contract(LR.as("nj"), Ten::make(right, "jk", {N2, k}), Mr);   // M = L_R V s^-1/2
+    contract(left, LL.as("ni"), Nr);                       // N = s^-1/2 U^T L_L^T
+    contract(LR.as("nj"), right, Mr);                      // M = L_R V s^-1/2
     scale_leg(Nr.p, Nr.size(), N2, k, o.s_dev, 3);
     scale_leg(Mr.p, Mr.size(), 1, k, o.s_dev, 3);
     return true;
