@@ -103,10 +103,12 @@ double tatrg_order_parameter(int leg);
 int tatrg_get_stage_ms(double *host_out, int cap);
 const char *tatrg_stage_name(int i);
 /* Per-launch device timing of the tensor-GEMM kernel (CUDA event pairs on the library's stream
- * around every launch inside coarse_grain; a few microseconds of overhead per launch).  After a
- * step, tatrg_get_gemm_profile copies, for every stage i and tile configuration j (0: 64x64 CTA
- * tile, 1: 128x128), the triple {milliseconds, FP64 flops, launches} to host_out[(2 i + j) 3 ..];
- * returns the number of doubles written. */
+ * around the launches inside coarse_grain; a few microseconds of overhead per timed launch).
+ * on = 1: only the 128x128-tile launches (the dominant kernel) are timed; on = 2: every tensor-GEMM
+ * launch; 0: off.  After a step, tatrg_get_gemm_profile copies, for every stage i and tile class j
+ * (0: the 64x64 and 128x64 CTA tiles, 1: 128x128), the triple {milliseconds, FP64 flops, launches}
+ * to host_out[(2 i + j) 3 ..]; returns the number of doubles written.  With the environment variable
+ * TATRG_TRACE set, every timed launch is also logged on stderr (shape, split, ms, TFLOP/s). */
 int tatrg_set_profile(int on);
 int tatrg_get_gemm_profile(double *host_out, int cap);
 /* Number of kernel launches this library has enqueued since the last call (and reset). */
@@ -134,6 +136,20 @@ int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N,
  * Y, R (n x n row-major upper triangular) goes to R (device).  The "QR decomposition in the RSVD"
  * of PAPER.md:106 / the canonical form of PAPER.md:37 (Householder TSQR, robust to rank deficiency). */
 int tatrg_qr_pos(double *Y, int64_t m, int n, double *R);
+
+/* Blocked Cholesky factorisation of the symmetric positive definite n x n matrix A (device, row-major,
+ * lower triangle read) + shift_rel * max_i A_ii on the diagonal: A <- L (lower, upper part zeroed);
+ * Linv (device, n x n row-major, may be NULL) <- L^-1.  The factorisations behind the squeezers
+ * (Eq. 12) and the reduced bond swap.  Returns 0,
+ * 1 if a pivot was not positive (A then holds garbage), < 0 on error. */
+int tatrg_cholesky(double *A, int n, double shift_rel, double *Linv);
+
+/* Cholesky-QR of the tall row-major m x n block Y (device, n <= 64): `passes` (1..3) rounds of
+ * {C = Y^T Y (+ shift_rel * max diag in the first round), C = L L^T, Y <- Y L^-T}; Q overwrites Y and
+ * R (device, n x n row-major, may be NULL) receives the accumulated upper-triangular factor.  The
+ * orthonormalisation inside the subspace iterations ("iterations of the QR decomposition").
+ * Returns 0, 1 if a factorisation broke down, < 0 on error. */
+int tatrg_cholqr(double *Y, int64_t m, int n, int passes, double shift_rel, double *R);
 
 /* One-sided Jacobi SVD of the column-major m x n matrix G (device, ld = m): on exit G = U diag(s)
  * with orthogonal columns sorted by decreasing norm, V (n x n column-major, device) such that

@@ -23,7 +23,7 @@ EXPORTS = [
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
-    "tatrg_qr_pos", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
+    "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
     "tatrg_last_error", "tatrg_destroy",
 ]
 
@@ -73,6 +73,8 @@ def lib():
             "tatrg_probe_fp64_peak": (c_d, [c_i, c_i]),
             "tatrg_tensor_gemm": (c_i, [c_vp, c_vp, c_vp, c_i, c_i, c_i, c_i, c_vp, c_d, c_i]),
             "tatrg_qr_pos": (c_i, [c_vp, c_i64, c_i, c_vp]),
+            "tatrg_cholesky": (c_i, [c_vp, c_i, c_d, c_vp]),
+            "tatrg_cholqr": (c_i, [c_vp, c_i64, c_i, c_i, c_d, c_vp]),
             "tatrg_jacobi_svd": (c_i, [c_vp, c_i, c_i, c_vp, c_vp]),
             "tatrg_sumsq": (c_i, [c_vp, c_i64, c_vp]),
             "tatrg_dot": (c_i, [c_vp, c_vp, c_i64, c_vp]),
@@ -214,8 +216,9 @@ def stage_ms() -> dict:
     return {lib().tatrg_stage_name(i).decode(): float(out[i]) for i in range(n)}
 
 
-def set_profile(on: bool):
-    _check(lib().tatrg_set_profile(int(bool(on))))
+def set_profile(on):
+    """0 / False: off; 1 / True: time the 128x128-tile launches; 2: every tensor-GEMM launch."""
+    _check(lib().tatrg_set_profile(int(on)))
 
 
 def gemm_profile() -> dict:
@@ -277,6 +280,28 @@ def qr_pos(Y, R):
     _require_cuda()
     m, n = Y.shape
     _check(lib().tatrg_qr_pos(Y.data_ptr(), int(m), int(n), R.data_ptr()))
+
+
+def cholesky(A, Linv=None, shift_rel=0.0) -> bool:
+    """In place: A (n x n row-major CUDA tensor, lower triangle read) <- lower Cholesky factor;
+    Linv (optional, n x n) <- L^-1.  False if A was not numerically positive definite."""
+    _require_cuda()
+    n = A.shape[0]
+    rc = lib().tatrg_cholesky(A.data_ptr(), int(n), float(shift_rel), Linv.data_ptr() if Linv is not None else None)
+    if rc < 0:
+        _check(rc)
+    return rc == 0
+
+
+def cholqr(Y, R=None, passes=2, shift_rel=0.0) -> bool:
+    """In place Cholesky-QR of the tall m x n block Y (n <= 64): Y <- Q, R (optional) <- R."""
+    _require_cuda()
+    m, n = Y.shape
+    rc = lib().tatrg_cholqr(Y.data_ptr(), int(m), int(n), int(passes), float(shift_rel),
+                            R.data_ptr() if R is not None else None)
+    if rc < 0:
+        _check(rc)
+    return rc == 0
 
 
 def jacobi_svd(G, V, s):

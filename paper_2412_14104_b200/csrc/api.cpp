@@ -5,6 +5,8 @@
 #include <string.h>
 
 #include "../../include/tatrg.h"
+#include <stdlib.h>
+
 #include "ctx.h"
 
 namespace tatrg {
@@ -44,7 +46,7 @@ void fail(int code, const char *fmt, ...)
 int prof_begin(double flops, int big)
 {
     Ctx &c = ctx();
-    if (!c.prof) return -1;
+    if (!c.prof || (c.prof == 1 && big != 1)) return -1;
     const size_t slot = c.prof_rec.size();
     if (2 * slot + 2 > c.prof_ev.size()) {
         const size_t old = c.prof_ev.size();
@@ -55,9 +57,21 @@ int prof_begin(double flops, int big)
                 return -1;
             }
     }
-    c.prof_rec.push_back(Ctx::ProfRec{c.cur_stage, big, flops});
+    Ctx::ProfRec rec{c.cur_stage, big, flops, {0, 0, 0, 0, 0}};
+    for (int i = 0; i < 5; ++i) rec.shape[i] = c.prof_shape[i];
+    c.prof_rec.push_back(rec);
     cudaEventRecord(c.prof_ev[2 * slot], c.stream);
     return (int)slot;
+}
+
+void prof_shape(int M, int N, int K, int batch, int ksplit)
+{
+    Ctx &c = ctx();
+    c.prof_shape[0] = M;
+    c.prof_shape[1] = N;
+    c.prof_shape[2] = K;
+    c.prof_shape[3] = batch;
+    c.prof_shape[4] = ksplit;
 }
 
 void prof_end(int slot)
@@ -70,6 +84,7 @@ void prof_end(int slot)
 void prof_collect()
 {
     Ctx &c = ctx();
+    static const bool trace = getenv("TATRG_TRACE") != nullptr;   // per-launch GEMM log on stderr
     for (int i = 0; i < ST_COUNT; ++i)
         for (int j = 0; j < 2; ++j) c.gemm_ms[i][j] = c.gemm_fl[i][j] = 0.0, c.gemm_n[i][j] = 0;
     for (size_t i = 0; i < c.prof_rec.size(); ++i) {
@@ -77,6 +92,9 @@ void prof_collect()
         if (cudaEventElapsedTime(&ms, c.prof_ev[2 * i], c.prof_ev[2 * i + 1]) != cudaSuccess) continue;
         const Ctx::ProfRec &r = c.prof_rec[i];
         if (r.stage < 0 || r.stage >= ST_COUNT) continue;
+        if (trace)
+            fprintf(stderr, "tatrg-trace stage %d tile %d M %d N %d K %d batch %d ksplit %d ms %.4f tflops %.2f\n", r.stage,
+                    r.big, r.shape[0], r.shape[1], r.shape[2], r.shape[3], r.shape[4], ms, r.flops / (ms * 1e-3) / 1e12);
         c.gemm_ms[r.stage][r.big] += ms;
         c.gemm_fl[r.stage][r.big] += r.flops;
         c.gemm_n[r.stage][r.big] += 1;
@@ -311,7 +329,7 @@ int tatrg_get_stage_ms(double *host_out, int cap)
 
 int tatrg_set_profile(int on)
 {
-    ctx().prof = on != 0;
+    ctx().prof = on < 0 ? 0 : (on > 2 ? 2 : on);
     ctx().prof_rec.clear();
     return TATRG_OK;
 }
@@ -396,6 +414,32 @@ int tatrg_qr_pos(double *Y, int64_t m, int n, double *R)
         scratch_begin();
         tsqr(Y, m, n, R);
     });
+}
+
+int tatrg_cholesky(double *A, int n, double shift_rel, double *Linv)
+{
+    bool ok = false;
+    int rc = guarded([&] {
+        if (!A || n < 1) fail(TATRG_EINVAL, "tatrg_cholesky: need A and n >= 1");
+        scratch_begin();
+        ok = cholesky_lower(A, n, shift_rel, Linv);
+    });
+    return rc < 0 ? rc : (ok ? 0 : 1);
+}
+
+int tatrg_cholqr(double *Y, int64_t m, int n, int passes, double shift_rel, double *R)
+{
+    int h = 0;
+    int rc = guarded([&] {
+        if (!Y || m < n || n < 1) fail(TATRG_EINVAL, "tatrg_cholqr: need m >= n >= 1");
+        scratch_begin();
+        int *flag = (int *)ws_alloc(sizeof(int));
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+        cholqr_async(Y, m, n, passes, shift_rel, flag, nullptr, R);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    });
+    return rc < 0 ? rc : (h ? 1 : 0);
 }
 
 int tatrg_jacobi_svd(double *G, int m, int n, double *V, double *s)

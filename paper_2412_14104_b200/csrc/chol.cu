@@ -24,7 +24,8 @@ constexpr int CH_NT = 256;
 // with the identity.
 __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ A, long long lda, int nb,
                                                           double *__restrict__ Linv, int *__restrict__ flag,
-                                                          double *__restrict__ dminmax, double shift_rel)
+                                                          double *__restrict__ dminmax, double shift_rel,
+                                                          long long ldinv)
 {
     __shared__ double col[2][NB];
     __shared__ double wrow[2][NB];
@@ -116,7 +117,7 @@ __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ 
             const int i = ty + 16 * a, c = tx + 16 * b;
             if (i < nb && c < nb) {
                 A[i * lda + c] = (c <= i) ? s[a][b] : 0.0;
-                Linv[i * NB + c] = (c <= i) ? w[a][b] : 0.0;
+                Linv[i * ldinv + c] = (c <= i) ? w[a][b] : 0.0;
             }
         }
     __syncthreads();
@@ -157,6 +158,20 @@ __global__ void zero_upper_kernel(double *__restrict__ A, int n)
     }
 }
 
+// G = I + E with |E| tiny: L = I + strict_lower(E) + diag(E)/2 and L^-1 = 2I - L, both to O(|E|^2)
+__global__ void near_identity_chol_kernel(double *__restrict__ G, double *__restrict__ Linv, int n)
+{
+    long long total = (long long)n * n;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total;
+         i += (long long)gridDim.x * blockDim.x) {
+        int r = (int)(i / n), c = (int)(i - (long long)r * n);
+        double e = G[i] - (r == c ? 1.0 : 0.0);
+        double l = (c < r) ? e : (c == r ? 0.5 * e : 0.0);
+        G[i] = (r == c ? 1.0 : 0.0) + l;
+        Linv[i] = (r == c ? 1.0 : 0.0) - l;
+    }
+}
+
 Ten view2(double *p, char a, long long na, long long sa, char b, long long nb_, long long sb)
 {
     Ten t;
@@ -186,15 +201,16 @@ void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double
 {
     if (n > NB) fail(-22, "chol_block: n = %d > %d", n, NB);
     chol_attr();
-    chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(A, lda, n, Linv, flag, dminmax, shift_rel);
+    chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(A, lda, n, Linv, flag, dminmax, shift_rel, NB);
     TATRG_LAUNCH_CHECK();
     count_launch();
 }
 
 // In place: the n x n symmetric matrix A (row-major, lower triangle read) becomes its lower
 // Cholesky factor (upper triangle zeroed) after adding shift_rel * max_i A_ii to the diagonal.
+// Linv_full (optional, n x n row-major) receives L^-1.
 // Returns false when a pivot was not positive (A then holds garbage).
-bool cholesky_lower(double *A, int n, double shift_rel)
+bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
 {
     size_t mark = ws_mark();
     int *flag = (int *)ws_alloc(sizeof(int));
@@ -204,12 +220,15 @@ bool cholesky_lower(double *A, int n, double shift_rel)
         add_shift_kernel<<<1, 256, 0, stream()>>>(A, n, shift_rel);
         count_launch();
     }
+    if (Linv_full) fill_zero(Linv_full, (long long)n * n);
     double *tmp = ws_doubles((long long)n * NB);
     chol_attr();
     for (int j0 = 0; j0 < n; j0 += NB) {
         const int nb = n - j0 < NB ? n - j0 : NB;
         double *Ajj = A + (long long)j0 * n + j0;
-        chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(Ajj, n, nb, Linv, flag, nullptr, 0.0);
+        double *Lij = Linv_full ? Linv_full + (long long)j0 * n + j0 : Linv;   // inverse of the diagonal block
+        const long long ldi = Linv_full ? n : NB;
+        chol_block_kernel<<<1, CH_NT, CHOL_SMEM, stream()>>>(Ajj, n, nb, Lij, flag, nullptr, 0.0, ldi);
         TATRG_LAUNCH_CHECK();
         count_launch();
         const int rest = n - j0 - nb;
@@ -218,7 +237,7 @@ bool cholesky_lower(double *A, int n, double shift_rel)
         double *A22 = A + (long long)(j0 + nb) * n + j0 + nb;
         // L21 = A21 Linv^T
         Ten T = view2(tmp, 'i', rest, nb, 'j', nb, 1);
-        contract(view2(A21, 'i', rest, n, 'k', nb, 1), view2(Linv, 'j', nb, NB, 'k', nb, 1), T);
+        contract(view2(A21, 'i', rest, n, 'k', nb, 1), view2(Lij, 'j', nb, ldi, 'k', nb, 1), T);
         // A22 -= L21 L21^T ; then store L21
         contract(T.as("ik"), T.as("jk"), view2(A22, 'i', rest, n, 'j', rest, 1), -1.0, true);
         TATRG_CUDA_CHECK(cudaMemcpy2DAsync(A21, sizeof(double) * n, tmp, sizeof(double) * nb, sizeof(double) * nb,
@@ -228,11 +247,47 @@ bool cholesky_lower(double *A, int n, double shift_rel)
     zero_upper_kernel<<<blocks, 256, 0, stream()>>>(A, n);
     TATRG_LAUNCH_CHECK();
     count_launch();
+    if (Linv_full) {
+        // L^-1 from the inverted diagonal blocks, doubling the block size:
+        // inv([L11 0; L21 L22]) = [inv11 0; -inv22 L21 inv11, inv22]; equal pairs of one level are one batched GEMM
+        double *tt = ws_doubles((long long)n * n / 2 + NB * NB);
+        for (long long sz = NB; sz < n; sz *= 2) {
+            const long long full = n / (2 * sz);                       // pairs with two complete halves
+            auto pair = [&](long long j0, long long s2, long long nbat) {
+                const long long bs = 2 * sz * ((long long)n + 1);      // batch stride along the diagonal
+                auto v3 = [&](double *p, char a, long long na, long long sa, char b, long long nb_, long long sb) {
+                    Ten t;
+                    t.p = p;
+                    t.legs = {Leg{'B', nbat, bs}, Leg{a, na, sa}, Leg{b, nb_, sb}};
+                    return t;
+                };
+                const double *L21 = A + (j0 + sz) * n + j0;
+                double *I11 = Linv_full + j0 * n + j0, *I22 = Linv_full + (j0 + sz) * n + j0 + sz;
+                double *I21 = Linv_full + (j0 + sz) * n + j0;
+                Ten T;
+                T.p = tt;
+                T.legs = {Leg{'B', nbat, s2 * sz}, Leg{'i', s2, sz}, Leg{'j', sz, 1}};
+                contract(v3(const_cast<double *>(L21), 'i', s2, n, 'k', sz, 1), v3(I11, 'k', sz, n, 'j', sz, 1), T);
+                contract(v3(I22, 'l', s2, n, 'i', s2, 1), T, v3(I21, 'l', s2, n, 'j', sz, 1), -1.0, false);
+            };
+            if (full > 0) pair(0, sz, full);
+            const long long j0 = full * 2 * sz;
+            if (n - j0 > sz) pair(j0, n - j0 - sz, 1);                 // ragged last pair
+        }
+    }
     int h = 0;
     TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
     ws_release(mark);
     return h == 0;
+}
+
+void near_identity_chol(double *G, int n, double *Linv)
+{
+    int blocks = (int)(((long long)n * n + 255) / 256 < 1184 ? ((long long)n * n + 255) / 256 : 1184);
+    near_identity_chol_kernel<<<blocks, 256, 0, stream()>>>(G, Linv, n);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
 }
 
 }  // namespace tatrg

@@ -58,6 +58,7 @@ void count_launch(int n = 1);
 void count_flops(double f);
 int prof_begin(double flops, int big);
 void prof_end(int slot);
+void prof_shape(int M, int N, int K, int batch, int ksplit);   // shape of the next profiled launch (trace)
 int set_error(int code, const char *fmt, ...);
 void *ws_alloc(size_t bytes);          // bump allocation from the caller's workspace (throws Err)
 double *ws_doubles(long long n);
@@ -84,7 +85,7 @@ struct Err {
 // ---- kernels (host launchers) ----------------------------------------------------------
 // gemm.cu
 void tensor_gemm(GemmParams p);
-void tensor_gemm_big(const GemmParams &p);   // gemm_big.cu: the 128x128 CTA tile
+void tensor_gemm_big(const GemmParams &p, int bn);   // gemm_big.cu: the 128 x bn CTA tile, bn = 128 or 64
 double probe_fp64_peak(int mode, int iters);
 // qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
 // Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).
@@ -118,9 +119,12 @@ void symmetrize(double *x, int n);                                            //
 void fill_identity(double *x, int n);
 void fill_zero(double *x, long long n);
 void transpose_small(const double *in, double *out, int rows, int cols);      // out[c,r] = in[r,c]
+void max_dev_identity(const double *G, int n, double *out);                   // out[0] = max |G - I|
 // chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
 // diagonal); false if a pivot was not positive
-bool cholesky_lower(double *A, int n, double shift_rel);
+bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full = nullptr);
+// G = I + E, |E| <~ 1e-8: in place lower Cholesky factor and its inverse by the first-order formulas (error O(|E|^2))
+void near_identity_chol(double *G, int n, double *Linv);
 void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel = 0.0);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);

@@ -45,14 +45,16 @@ struct Ctx {
 
     // optional per-launch timing of the tensor-GEMM kernel (tatrg_set_profile): CUDA event pairs
     // around every tgemm launch of a step, summed per stage when the step ends
-    bool prof = false;
+    int prof = 0;   // 0 off, 1 the 128x128 tile only, 2 every tensor-GEMM launch
     int cur_stage = 0;
     std::vector<cudaEvent_t> prof_ev;   // pool, two per launch
     struct ProfRec {
         int stage;
         int big;
         double flops;
+        int shape[5];   // M, N, K, batch, ksplit
     };
+    int prof_shape[5] = {0, 0, 0, 0, 0};
     std::vector<ProfRec> prof_rec;
     double gemm_ms[ST_COUNT][2] = {};      // [stage][0: 64x64 tile, 1: 128x128 tile]
     double gemm_fl[ST_COUNT][2] = {};

@@ -9,6 +9,8 @@
 // cp.async gather addresses: no transpose kernel runs.  Operand tiles are staged in shared
 // memory as [k][m] / [k][n] with a leading dimension = 4 (mod 16) doubles, which makes the
 // 8-byte DMMA fragment loads bank-conflict free, through a STAGES-deep cp.async pipeline.
+#include <math.h>
+
 #include "common.h"
 
 namespace tatrg {
@@ -296,18 +298,37 @@ void tensor_gemm(GemmParams p)
         TATRG_CUDA_CHECK(cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev));
     }
     count_flops(2.0 * p.M * p.N * (double)p.K * p.batch);
-    // tile choice: big tile when it still fills the machine, else the small one
-    long long big_tiles = (long long)((p.M + 127) / 128) * ((p.N + 127) / 128) * p.batch;
-    bool big = big_tiles * 5 >= 4LL * g_num_sms && p.M >= 96 && p.N >= 96;
-    long long tiles = big ? big_tiles : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
+    // tile choice: 128x128 when it fills the machine (with split-K when the summed index is long),
+    // 128x64 for outputs at most 64 columns wide with enough rows, else the 64x64 tile
     int ktiles = (p.K + BK - 1) / BK;
+    long long big_tiles = (long long)((p.M + 127) / 128) * ((p.N + 127) / 128) * p.batch;
+    const int max_split = ktiles / 8 < 512 ? ktiles / 8 : 512;
+    bool big = p.M >= 96 && p.N >= 96 &&
+               (big_tiles * 5 >= 4LL * g_num_sms || big_tiles * (long long)(max_split > 1 ? max_split : 1) >= 2LL * g_num_sms);
+    const bool mid = !big && p.N <= 64 && p.N >= 33 && p.M >= 96;
+    long long tiles = big ? big_tiles
+                          : mid ? (long long)((p.M + 127) / 128) * p.batch
+                                : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
     p.ksplit = 1;
     p.ktiles_per_split = ktiles;
     p.partial = nullptr;
     size_t mark = ws_mark();
-    if (tiles < g_num_sms && ktiles >= 16) {
-        int want = (int)((2LL * g_num_sms + tiles - 1) / tiles);
-        int ks = want < ktiles / 8 ? want : ktiles / 8;
+    // split-K: the number of splits that fills whole waves of resident CTAs best (fewer on ties)
+    const long long slots = (long long)g_num_sms * (big ? 1 : mid ? 2 : 3);
+    if (tiles < 4 * slots && max_split > 1) {
+        auto eff = [&](int ks) {
+            const double x = (double)tiles * ks / (double)slots;
+            return (x < 1.0 ? x : x / ceil(x)) - 0.0005 * ks;   // machine fill, then whole waves
+        };
+        int ks = 1;
+        double best = eff(1);
+        for (int c = 2; c <= max_split; ++c) {
+            const double e = eff(c);
+            if (e > best * 1.08) {
+                best = e;
+                ks = c;
+            }
+        }
         if (ks > 1) {
             p.ktiles_per_split = (ktiles + ks - 1) / ks;
             p.ksplit = (ktiles + p.ktiles_per_split - 1) / p.ktiles_per_split;
@@ -316,8 +337,11 @@ void tensor_gemm(GemmParams p)
         }
     }
     if ((long long)p.batch * p.ksplit > 65535) fail(-22, "tensor_gemm: batch too large for grid.z");
+    prof_shape(p.M, p.N, p.K, p.batch, p.ksplit);
     if (big)
-        tensor_gemm_big(p);
+        tensor_gemm_big(p, 128);
+    else if (mid)
+        tensor_gemm_big(p, 64);
     else
         launch_cfg<64, 64, 32, 32, 4>(p);
     if (p.ksplit > 1) {

@@ -1,10 +1,11 @@
-// gemm_big.cu -- the 128x128 CTA tile of the tensor-GEMM (see gemm.cu for the operation):
+// gemm_big.cu -- the 128x128 (and 128x64, for outputs at most 64 columns wide) CTA tiles of the
+// tensor-GEMM (see gemm.cu for the operation):
 //   C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)]
 // on the FP64 tensor pipe (mma.sync m8n8k4 -> DMMA.8x8x4).  This is the kernel the O(q r chi^7) bond
 // swap (Table 1) and the O(r^2 chi^7) triad contraction (Eqs. 13-14)
 // run on.
 //
-// 8 warps, warp tile 32 x 64 (64 FP64 accumulators per thread), BK = 16, 4-stage cp.async pipeline.
+// 8 (4) warps, warp tile 32 x 64 (64 FP64 accumulators per thread), BK = 16, 4-stage cp.async pipeline.
 // The shared-memory layout of an operand tile follows the operand's contiguous index in global
 // memory, so that 16-byte cp.async copies land on 16 consecutive bytes of shared memory:
 //   contiguous index = the free index (m or n):  tile stored [k][m], leading dimension 128 + 4
@@ -19,7 +20,7 @@ namespace tatrg {
 
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 16, STAGES = 4, NT = 256;
+constexpr int BM = 128, BK = 16, STAGES = 4;
 constexpr int LD_F = BM + 4;   // [k][m] layout
 constexpr int LD_K = BK + 4;   // [m][k] layout
 constexpr int RASTER_W = 12;
@@ -45,11 +46,15 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
                  : "d"(a), "d"(b));
 }
 
-// Loader of one 128 x 16 operand tile.  KF: k is the contiguous index in global memory.
-// VEC: 16-byte copies (pairs along the contiguous index), else 8-byte copies.
-template <bool KF, bool VEC>
+// Loader of one ROWS x 16 operand tile by NT threads.  KF: k is the contiguous index in global
+// memory.  VEC: 16-byte copies (pairs along the contiguous index), else 8-byte copies.
+template <bool KF, bool VEC, int ROWS, int NT>
 struct TileLoader {
-    static constexpr int PER = VEC ? 4 : 8;          // copies per thread per tile
+    static constexpr int W = VEC ? 2 : 1;             // elements per copy
+    static constexpr int PER = ROWS * BK / (NT * W);  // copies per thread per tile
+    static constexpr int TPR = NT / BK;               // !KF: threads along the free index per k row
+    static constexpr int LDF = ROWS + 4;              // !KF: leading dimension of the [k][free] tile
+    static_assert(PER >= 1 && PER * NT * W == ROWS * BK, "loader layout");
     long long fix[PER];                               // offsets of the free index (fixed over k tiles)
     int free_left[PER];                               // valid elements from this copy's free index on
     const double *base;
@@ -71,14 +76,14 @@ struct TileLoader {
                 soff[j] = fl * LD_K + kl;
             }
         } else {
-            // free-index pairs (VEC) or singles; 16 threads along the free index, k = t / 16
-            kl = t / 16;
+            // free-index pairs (VEC) or singles; TPR threads along the free index, k = t / TPR
+            kl = t / TPR;
 #pragma unroll
             for (int j = 0; j < PER; ++j) {
-                int fl = ((t % 16) + 16 * j) * (VEC ? 2 : 1);
+                int fl = ((t % TPR) + TPR * j) * W;
                 free_left[j] = F - (f0 + fl);
                 fix[j] = free_left[j] > 0 ? map_off(mfree, f0 + fl) : 0;
-                soff[j] = kl * LD_F + fl;
+                soff[j] = kl * LDF + fl;
             }
         }
     }
@@ -100,11 +105,13 @@ struct TileLoader {
     }
 };
 
-template <bool A_KF, bool B_KF, bool VEC>
-__global__ void __launch_bounds__(NT, 1) tgemm_big_kernel(const __grid_constant__ GemmParams p)
+template <bool A_KF, bool B_KF, bool VEC, int BN>
+__global__ void __launch_bounds__(BN * 2, BN == 128 ? 1 : 2) tgemm_big_kernel(const __grid_constant__ GemmParams p)
 {
+    constexpr int NT = BN * 2;                        // (BM / 32) * (BN / 64) warps
+    constexpr int LD_FB = BN + 4;                     // [k][n] layout of the B tile
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
-    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_F;
+    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_FB;
     constexpr int WM = 32, WN = 64, FM = WM / 8, FN = WN / 8;
     extern __shared__ __align__(16) double smem[];
     double *As = smem;
@@ -132,8 +139,8 @@ __global__ void __launch_bounds__(NT, 1) tgemm_big_kernel(const __grid_constant_
     }
     const int nkt = max(kt1 - kt0, 0);
 
-    TileLoader<A_KF, VEC> la;
-    TileLoader<B_KF, VEC> lb;
+    TileLoader<A_KF, VEC, BM, NT> la;
+    TileLoader<B_KF, VEC, BN, NT> lb;
     la.init(p.A + map_off(p.ab, bz), p.am, m0, p.M, t);
     lb.init(p.B + map_off(p.bb, bz), p.bn, n0, p.N, t);
 
@@ -147,11 +154,11 @@ __global__ void __launch_bounds__(NT, 1) tgemm_big_kernel(const __grid_constant_
     const int lr = lane >> 2, lk = lane & 3;
     // fragment base offsets inside a stage
     const int a_off = A_KF ? (wm0 + lr) * LD_K + lk : lk * LD_F + wm0 + lr;
-    const int b_off = B_KF ? (wn0 + lr) * LD_K + lk : lk * LD_F + wn0 + lr;
+    const int b_off = B_KF ? (wn0 + lr) * LD_K + lk : lk * LD_FB + wn0 + lr;
     constexpr int A_I = A_KF ? 8 * LD_K : 8;        // step between 8-row fragments
     constexpr int B_J = B_KF ? 8 * LD_K : 8;
     constexpr int A_KK = A_KF ? 4 : 4 * LD_F;       // step between k groups of 4
-    constexpr int B_KK = B_KF ? 4 : 4 * LD_F;
+    constexpr int B_KK = B_KF ? 4 : 4 * LD_FB;
 
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
@@ -238,14 +245,15 @@ __global__ void __launch_bounds__(NT, 1) tgemm_big_kernel(const __grid_constant_
     }
 }
 
-template <bool A_KF, bool B_KF, bool VEC>
+template <bool A_KF, bool B_KF, bool VEC, int BN>
 void launch_big(const GemmParams &p_in)
 {
+    constexpr int NT = BN * 2;
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
-    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_F;
+    constexpr int B_STAGE = B_KF ? BN * LD_K : BK * (BN + 4);
     constexpr size_t smem = (size_t)STAGES * (A_STAGE + B_STAGE) * sizeof(double);
     static bool attr_done = false;
-    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC>;
+    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN>;
     if (!attr_done) {
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
@@ -255,7 +263,7 @@ void launch_big(const GemmParams &p_in)
     const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n;
     if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
     dim3 grid((unsigned)tiles, 1, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
-    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, 1);
+    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, BN == 128);
     kern<<<grid, NT, smem, stream()>>>(p);
     prof_end(slot);
     TATRG_LAUNCH_CHECK();
@@ -276,9 +284,8 @@ bool vec_ok(const double *base, const Map4 &fast, const Map4 &slow, const Map4 &
            all_even(batch);
 }
 
-}  // namespace
-
-void tensor_gemm_big(const GemmParams &p)
+template <int BN>
+void dispatch_big(const GemmParams &p)
 {
     const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;
     const bool va = akf ? vec_ok(p.A, p.ak, p.am, p.ab) : vec_ok(p.A, p.am, p.ak, p.ab);
@@ -286,15 +293,25 @@ void tensor_gemm_big(const GemmParams &p)
     const bool vec = va && vb;
     if (akf) {
         if (bkf)
-            vec ? launch_big<true, true, true>(p) : launch_big<true, true, false>(p);
+            vec ? launch_big<true, true, true, BN>(p) : launch_big<true, true, false, BN>(p);
         else
-            vec ? launch_big<true, false, true>(p) : launch_big<true, false, false>(p);
+            vec ? launch_big<true, false, true, BN>(p) : launch_big<true, false, false, BN>(p);
     } else {
         if (bkf)
-            vec ? launch_big<false, true, true>(p) : launch_big<false, true, false>(p);
+            vec ? launch_big<false, true, true, BN>(p) : launch_big<false, true, false, BN>(p);
         else
-            vec ? launch_big<false, false, true>(p) : launch_big<false, false, false>(p);
+            vec ? launch_big<false, false, true, BN>(p) : launch_big<false, false, false, BN>(p);
     }
+}
+
+}  // namespace
+
+void tensor_gemm_big(const GemmParams &p, int bn)
+{
+    if (bn == 64)
+        dispatch_big<64>(p);
+    else
+        dispatch_big<128>(p);
 }
 
 }  // namespace tatrg

@@ -252,6 +252,34 @@ void fill_zero(double *x, long long n)
     TATRG_CUDA_CHECK(cudaMemsetAsync(x, 0, n * sizeof(double), stream()));
 }
 
+// out[0] = max_ij |G_ij - delta_ij| (non-negative doubles order like their bit patterns)
+__global__ void max_dev_identity_kernel(const double *__restrict__ G, int n, unsigned long long *__restrict__ out)
+{
+    const long long total = (long long)n * n;
+    double m = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const int r = (int)(i / n), c = (int)(i - (long long)r * n);
+        const double v = fabs(G[i] - (r == c ? 1.0 : 0.0));
+        m = (v > m || v != v) ? v : m;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const double w = __shfl_xor_sync(0xffffffffu, m, o);
+        m = (w > m || w != w) ? w : m;
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (m != m) m = INFINITY;
+        atomicMax(out, (unsigned long long)__double_as_longlong(m));
+    }
+}
+
+void max_dev_identity(const double *G, int n, double *out)
+{
+    TATRG_CUDA_CHECK(cudaMemsetAsync(out, 0, sizeof(double), stream()));
+    max_dev_identity_kernel<<<grid_for((long long)n * n), RED_THREADS, 0, stream()>>>(G, n, (unsigned long long *)out);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
+
 void transpose_small(const double *in, double *out, int rows, int cols)
 {
     transpose_kernel<<<grid_for((long long)rows * cols), RED_THREADS, 0, stream()>>>(in, out, rows, cols);

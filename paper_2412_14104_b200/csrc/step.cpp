@@ -307,6 +307,57 @@ bool squeezer_subspace(const Ten &GLm, const Ten &GRm, int N2, int chi, int mu, 
     return true;
 }
 
+// Orthonormal basis of the column space of the matricisation T2[(pqt); (c,b)] of T[c,p,q,t,b]
+// (nT x nk, nk = n0 * a), by two Cholesky-QR passes with explicit triangular inverses so that all
+// O(nT nk^2) work is three full-size tensor-GEMMs:
+//   G1 = T2^T T2 = L1 L1^T,  Q1 = T2 L1^-T,  G2 = Q1^T Q1 = L2 L2^T,  Q = Q1 L2^-T (kept implicit),
+//   T2 = Q R,  R = L2^T L1^T.
+// Used by the bond swap (reduced operator, below).  Returns false -- nothing the caller keeps has
+// been written -- when T2 is rank deficient or too ill conditioned for two passes (|G2 - I| > 0.05).
+struct RedBasis {
+    Ten Q1;      // [p,q,t,k]
+    Ten R;       // [k,c,b]
+    Ten L2inv;   // [k,l] lower triangular: Q = Q1 L2inv^T
+};
+
+bool ortho_factor(const Ten &T, RedBasis &o)
+{
+    const long long n0 = T.legs[0].n, n1 = T.legs[1].n, n2 = T.legs[2].n, n3 = T.legs[3].n, a = T.legs[4].n;
+    const long long nk = n0 * a;
+    if (nk > 0x7fffffff) return false;
+    o.Q1 = ws_tensor("pqtk", {n1, n2, n3, nk});
+    o.R = ws_tensor("kcb", {nk, n0, a});
+    o.L2inv = ws_tensor("kl", {nk, nk});
+    size_t mk = ws_mark();
+    Ten G1 = ws_tensor("cbde", {n0, a, n0, a});
+    Ten L1inv = ws_tensor("kcb", {nk, n0, a});
+    contract(T.as("cpqtb"), T.as("dpqte"), G1);
+    if (!cholesky_lower(G1.p, (int)nk, 0.0, L1inv.p)) {
+        ws_release(mk);
+        return false;
+    }
+    contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
+    Ten G2 = ws_tensor("kl", {nk, nk});
+    contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2);
+    double *dev = ws_doubles(1);
+    max_dev_identity(G2.p, (int)nk, dev);
+    const double err = d2h(dev, 1)[0];
+    if (!(err < 0.05)) {
+        ws_release(mk);
+        return false;
+    }
+    if (err < 1e-8) {
+        near_identity_chol(G2.p, (int)nk, o.L2inv.p);
+    } else if (!cholesky_lower(G2.p, (int)nk, 0.0, o.L2inv.p)) {
+        ws_release(mk);
+        return false;
+    }
+    // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
+    contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
+    ws_release(mk);
+    return true;
+}
+
 }  // namespace
 
 // =======================================================================================
@@ -492,26 +543,87 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     // =================== O3 bond swap (Table 1 row 1) ===================
     const long long dim = a * nT;
     const int ell = (int)std::min<long long>((long long)r * chi, dim);
-    Ten omega = get_input(0, dim, ell, cfg, "rz");
-    Ten Z = ws_tensor("cabz", {n0, a, a, ell});
-    auto sw_apply = [&](const double *w, double *out) {   // M w : [(b,J), z] -> [(a,I'), z]
-        contract(D.as("cuvwa"), Ten::make(const_cast<double *>(w), "buvwz", {a, n1, n2, n3, ell}), Z);
-        scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
-        scale_leg(Z.p, Z.size(), ell, a, sT, 0);
-        contract(A.as("cpqtb"), Z, Ten::make(out, "apqtz", {a, n1, n2, n3, ell}));
-    };
-    auto sw_apply_t = [&](const double *w, double *out) {  // M^T w : [(a,I'), z] -> [(b,J), z]
-        contract(A.as("cpqtb"), Ten::make(const_cast<double *>(w), "apqtz", {a, n1, n2, n3, ell}), Z.as("cbaz"));
-        scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
-        scale_leg(Z.p, Z.size(), ell, a, sT, 0);
-        contract(D.as("cuvwa"), Z.as("cbaz"), Ten::make(out, "buvwz", {a, n1, n2, n3, ell}));
-    };
     double *Xbuf = ws_doubles(dim * std::min<long long>(chi, ell));
     double *Ybuf = ws_doubles(dim * std::min<long long>(chi, ell));
-    int gs;
-    double *sig;
-    {
+    int gs = 0;
+    double *sig = nullptr;
+    bool swapped = false;
+    // Reduced operator: M = (1 x Q_A) m (1 x Q_D)^T with A[c,I',b] = sum_k Q_A[I',k] R_A[k,c,b] and
+    // D likewise (Q_A, Q_D orthonormal, nT x n0 a), m[(a k),(b l)] = sum_c sT_a R_D[l,c,a] R_A[k,c,b] sT_b.
+    // Every iterate of the subspace iteration lies in the range of 1 x Q_A (resp. 1 x Q_D) and
+    // qr+((1 x Q) y) = (1 x Q) qr+(y), so the RSVD of M with the sketch Omega is the RSVD of m with the
+    // sketch (1 x Q_D)^T Omega, expanded at the end: the same X, sigma, Y at 1/chi of the flops.
+    const long long nk = n0 * a;
+    if (nT >= 2 * nk && nk >= 16) {
         size_t mk = ws_mark();
+        RedBasis bA, bD;
+        if (ortho_factor(A, bA) && ortho_factor(D, bD)) {
+            const long long rdim = a * nk;
+            const int ellr = (int)std::min<long long>(ell, rdim);
+            // Omega_red[b,l,z] = sum_l' L2inv_D[l,l'] sum_uvw Q1_D[uvw,l'] Omega[b,uvw,z]
+            Ten om_red = ws_tensor("blz", {a, nk, ell});
+            {
+                size_t mk2 = ws_mark();
+                Ten omega = get_input(0, dim, ell, cfg, "rz");
+                Ten t1 = ws_tensor("bmz", {a, nk, ell});
+                contract(bD.Q1.as("uvwm"), Ten::make(omega.p, "buvwz", {a, n1, n2, n3, ell}), t1);
+                contract(bD.L2inv.as("lm"), t1, om_red);
+                ws_release(mk2);
+            }
+            Ten Z = ws_tensor("cabz", {n0, a, a, ell});
+            auto apply = [&](const double *w, double *out) {     // m w : [(b,l), z] -> [(a,k), z]
+                contract(bD.R.as("lca"), Ten::make(const_cast<double *>(w), "blz", {a, nk, ell}), Z);
+                scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+                scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+                contract(bA.R.as("kcb"), Z, Ten::make(out, "akz", {a, nk, ell}));
+            };
+            auto apply_t = [&](const double *w, double *out) {   // m^T w : [(a,k), z] -> [(b,l), z]
+                contract(bA.R.as("kcb"), Ten::make(const_cast<double *>(w), "akz", {a, nk, ell}), Z.as("cbaz"));
+                scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+                scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+                contract(bD.R.as("lca"), Z.as("cbaz"), Ten::make(out, "blz", {a, nk, ell}));
+            };
+            double *xr = ws_doubles(rdim * std::min<long long>(chi, ellr)), *yr = ws_doubles(rdim * std::min<long long>(chi, ellr));
+            if (ellr == ell) {
+                size_t mk2 = ws_mark();
+                RsvdOut ro = rsvd(apply, apply_t, om_red, rdim, rdim, ell, q, chi, xr, yr);
+                gs = ro.k;
+                spec[1].assign(ro.s_full.begin(), ro.s_full.begin() + gs);
+                gaps[0] = rel_gap(ro.s_full, gs);
+                ws_release(mk2);
+                // expand: X[a,pqt,g] = sum_m Q1_A[pqt,m] sum_k L2inv_A[k,m] x[a,k,g]
+                Ten t2 = ws_tensor("amg", {a, nk, gs});
+                contract(bA.L2inv.as("km"), Ten::make(xr, "akg", {a, nk, gs}), t2);
+                contract(bA.Q1.as("pqtm"), t2, Ten::make(Xbuf, "apqtg", {a, n1, n2, n3, gs}));
+                contract(bD.L2inv.as("km"), Ten::make(yr, "akg", {a, nk, gs}), t2);
+                contract(bD.Q1.as("pqtm"), t2, Ten::make(Ybuf, "apqtg", {a, n1, n2, n3, gs}));
+                swapped = true;
+            }
+        }
+        std::vector<double> keep(spec[1]);
+        ws_release(mk);
+        if (swapped) {
+            sig = ws_doubles(gs);
+            h2d(sig, keep.data(), gs);
+            TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+        }
+    }
+    if (!swapped) {
+        size_t mk = ws_mark();
+        Ten omega = get_input(0, dim, ell, cfg, "rz");
+        Ten Z = ws_tensor("cabz", {n0, a, a, ell});
+        auto sw_apply = [&](const double *w, double *out) {   // M w : [(b,J), z] -> [(a,I'), z]
+            contract(D.as("cuvwa"), Ten::make(const_cast<double *>(w), "buvwz", {a, n1, n2, n3, ell}), Z);
+            scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+            scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+            contract(A.as("cpqtb"), Z, Ten::make(out, "apqtz", {a, n1, n2, n3, ell}));
+        };
+        auto sw_apply_t = [&](const double *w, double *out) {  // M^T w : [(a,I'), z] -> [(b,J), z]
+            contract(A.as("cpqtb"), Ten::make(const_cast<double *>(w), "apqtz", {a, n1, n2, n3, ell}), Z.as("cbaz"));
+            scale_leg(Z.p, Z.size(), (long long)a * ell, a, sT, 0);
+            scale_leg(Z.p, Z.size(), ell, a, sT, 0);
+            contract(D.as("cuvwa"), Z.as("cbaz"), Ten::make(out, "buvwz", {a, n1, n2, n3, ell}));
+        };
         RsvdOut ro = rsvd(sw_apply, sw_apply_t, omega, dim, dim, ell, q, chi, Xbuf, Ybuf);
         gs = ro.k;
         spec[1].assign(ro.s_full.begin(), ro.s_full.begin() + gs);

@@ -149,6 +149,10 @@ void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accum
     p.B = B.p;
     p.C = C.p;
     long long M = total(gm), N = total(gn), K = total(gk), Bt = total(gb);
+    if (M <= 64 && N > 64) {   // the wide index goes to the 128-row side of the CTA tile
+        contract(B, A, C, alpha, accumulate);
+        return;
+    }
     if (M > 0x7fffffff || N > 0x7fffffff || K > 0x7fffffff || Bt > 65535)
         fail(-22, "contract: index range too large (M=%lld N=%lld K=%lld batch=%lld)", M, N, K, Bt);
     p.M = (int)M;

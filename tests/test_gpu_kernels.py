@@ -149,3 +149,78 @@ def test_norm_and_trace_reductions(tt, n):
     assert abs(o[1] - np.sum(x * y)) < 1e-13 * n
     tt.scale_by_rsqrt(dx, out[0:1])
     np.testing.assert_allclose(dx.cpu().numpy(), x / np.linalg.norm(x), rtol=1e-14, atol=0)
+
+
+@pytest.mark.parametrize("n", [1, 7, 64, 65, 200, 320, 1024])
+def test_cholesky_and_triangular_inverse(tt, n):
+    """Blocked Cholesky (register-tiled 64x64 diagonal kernel + tensor-GEMM panels) and the
+    block-doubling triangular inverse against numpy on a well-conditioned SPD matrix."""
+    import torch
+    rng = np.random.default_rng(n)
+    B = rng.standard_normal((n, n + 5))
+    A = B @ B.T + 0.5 * n * np.eye(n)
+    dA = _dev(A)
+    dLi = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    assert tt.cholesky(dA, dLi)
+    L, Li = dA.cpu().numpy(), dLi.cpu().numpy()
+    Lr = np.linalg.cholesky(A)
+    assert np.abs(np.triu(L, 1)).max() == 0.0 and np.abs(np.triu(Li, 1)).max() == 0.0
+    assert np.abs(L - Lr).max() < 1e-12 * np.abs(Lr).max()
+    assert np.abs(Li @ Lr - np.eye(n)).max() < 1e-12
+
+
+def test_cholesky_flags_indefinite(tt):
+    import torch
+    A = np.eye(100)
+    A[70, 70] = -1.0
+    assert not tt.cholesky(_dev(A))
+    # the relative diagonal shift makes a semidefinite matrix factorisable
+    v = np.ones((100, 1))
+    assert tt.cholesky(_dev(v @ v.T), shift_rel=1e-10)
+
+
+@pytest.mark.parametrize("m,n,passes", [(1024, 64, 2), (4096, 33, 2), (50000, 64, 2), (2048, 16, 3)])
+def test_cholqr(tt, m, n, passes):
+    """Asynchronous Cholesky-QR against LAPACK's QR (unique with R_ii > 0) on a block of
+    condition number ~1e3."""
+    import torch
+    rng = np.random.default_rng(m + n)
+    Y = rng.standard_normal((m, n)) * np.logspace(0, -3, n)
+    dY = _dev(Y)
+    dR = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    assert tt.cholqr(dY, dR, passes=passes)
+    Q, R = dY.cpu().numpy(), dR.cpu().numpy()
+    assert np.abs(Q.T @ Q - np.eye(n)).max() < 1e-13
+    assert np.abs(Q @ R - Y).max() < 1e-12 * np.abs(Y).max() * np.sqrt(m)
+    Ql, Rl = np.linalg.qr(Y)
+    d = np.sign(np.diag(Rl))
+    assert np.abs(Q - Ql * d).max() < 1e-9
+
+
+def test_cholqr_single_shifted_pass_spans_the_block(tt):
+    """One shifted pass (what the subspace iterations use between Ritz steps): not orthonormal to
+    rounding, but the same column space and a well-conditioned basis."""
+    rng = np.random.default_rng(5)
+    Y = rng.standard_normal((1024, 64)) * np.logspace(0, -5, 64)
+    dY = _dev(Y)
+    assert tt.cholqr(dY, None, passes=1, shift_rel=1e-13)
+    Q = dY.cpu().numpy()
+    assert np.abs(Q.T @ Q - np.eye(64)).max() < 1e-2
+    Qr, _ = np.linalg.qr(Y)
+    assert np.abs(Q - Qr @ (Qr.T @ Q)).max() < 1e-9
+
+
+@pytest.mark.parametrize("M,N,K", [(1000, 64, 300), (4096, 40, 1024), (130, 64, 20000), (40, 3000, 256),
+                                   (1024, 1024, 32768), (200, 200, 9000)])
+def test_tensor_gemm_tile_variants(tt, M, N, K):
+    """Shapes that select the 128x64 tile, the operand swap for short-and-wide outputs, and the
+    128x128 tile with split-K."""
+    import torch
+    rng = np.random.default_rng(M + N + K)
+    A, B = rng.standard_normal((M, K)), rng.standard_normal((K, N))
+    dA, dB = _dev(A), _dev(B)
+    dC = torch.empty(M, N, dtype=torch.float64, device="cuda")
+    maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+    tt.tensor_gemm(dA, dB, dC, M, N, K, maps)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(dC.cpu().numpy(), A @ B, rtol=0, atol=1e-11 * np.sqrt(K))
