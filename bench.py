@@ -476,7 +476,10 @@ def run_small_micro(args):
             out["qr_pos_%dx%d_ms" % (m, n)] = timeit(h)
             del Y0, Y, R
         for n in (32, 64):
-            G0 = torch.tril(torch.randn(n, n, dtype=torch.float64, device="cuda")) * torch.logspace(0, -6, n, dtype=torch.float64, device="cuda")
+            # column-major lower-triangular matrix with graded columns (what the RSVD core R_B^T looks like);
+            # the tensor's row j is column j
+            G0 = torch.triu(torch.randn(n, n, dtype=torch.float64, device="cuda")) * \
+                torch.logspace(0, -6, n, dtype=torch.float64, device="cuda")[:, None]
             G = G0.clone()
             V = torch.empty(n, n, dtype=torch.float64, device="cuda")
             sv = torch.empty(n, dtype=torch.float64, device="cuda")

@@ -221,7 +221,6 @@ bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
         count_launch();
     }
     if (Linv_full) fill_zero(Linv_full, (long long)n * n);
-    double *tmp = ws_doubles((long long)n * NB);
     chol_attr();
     for (int j0 = 0; j0 < n; j0 += NB) {
         const int nb = n - j0 < NB ? n - j0 : NB;
@@ -235,13 +234,13 @@ bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
         if (rest <= 0) break;
         double *A21 = A + (long long)(j0 + nb) * n + j0;
         double *A22 = A + (long long)(j0 + nb) * n + j0 + nb;
-        // L21 = A21 Linv^T
-        Ten T = view2(tmp, 'i', rest, nb, 'j', nb, 1);
-        contract(view2(A21, 'i', rest, n, 'k', nb, 1), view2(Lij, 'j', nb, ldi, 'k', nb, 1), T);
-        // A22 -= L21 L21^T ; then store L21
-        contract(T.as("ik"), T.as("jk"), view2(A22, 'i', rest, n, 'j', rest, 1), -1.0, true);
-        TATRG_CUDA_CHECK(cudaMemcpy2DAsync(A21, sizeof(double) * n, tmp, sizeof(double) * nb, sizeof(double) * nb,
-                                           rest, cudaMemcpyDeviceToDevice, stream()));
+        // L21 = A21 Linv^T, in place: the output is one column tile wide and K = nb is never split, so
+        // every CTA reads exactly the rows it later writes
+        contract(view2(A21, 'i', rest, n, 'k', nb, 1), view2(Lij, 'j', nb, ldi, 'k', nb, 1),
+                 view2(A21, 'i', rest, n, 'j', nb, 1));
+        // A22 -= L21 L21^T
+        contract(view2(A21, 'i', rest, n, 'k', nb, 1), view2(A21, 'j', rest, n, 'k', nb, 1),
+                 view2(A22, 'i', rest, n, 'j', rest, 1), -1.0, true, true);
     }
     int blocks = (int)(((long long)n * n + 255) / 256 < 1184 ? ((long long)n * n + 255) / 256 : 1184);
     zero_upper_kernel<<<blocks, 256, 0, stream()>>>(A, n);

@@ -45,12 +45,21 @@ struct GemmParams {
     Map4 ab, bb, cb;       // batch index maps of A, B, C
     double alpha;
     int accumulate;        // C += instead of C =
+    int lower_only;        // symmetric output (A^T A): tiles strictly above the diagonal are skipped, the
+                           // upper triangle of C is then undefined
     int a_kfast, b_kfast;  // loader thread order: 1 = consecutive threads walk k (k is the contiguous index)
     int ksplit;            // >1: partial sums go to `partial`, reduced by a second kernel
     int ktiles_per_split;  // in units of BK
     double *partial;       // [ksplit][batch][M][N]
     int tiles_n;           // set by the launcher: column tiles of the chosen CTA tile
 };
+
+// algorithmic flops of one launch (a symmetric lower-only output counts its lower triangle)
+inline double gemm_flops(const GemmParams &p)
+{
+    const double mn = p.lower_only ? 0.5 * p.M * ((double)p.N + 1.0) : (double)p.M * p.N;
+    return 2.0 * mn * (double)p.K * p.batch;
+}
 
 // ---- context -------------------------------------------------------------------------
 cudaStream_t stream();
@@ -119,7 +128,7 @@ void symmetrize(double *x, int n);                                            //
 void fill_identity(double *x, int n);
 void fill_zero(double *x, long long n);
 void transpose_small(const double *in, double *out, int rows, int cols);      // out[c,r] = in[r,c]
-void max_dev_identity(const double *G, int n, double *out);                   // out[0] = max |G - I|
+void max_dev_identity(const double *G, int n, double *out);                   // out[0] = max |G - I| over the lower triangle
 // chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
 // diagonal); false if a pivot was not positive
 bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full = nullptr);

@@ -11,6 +11,8 @@
 // 8-byte DMMA fragment loads bank-conflict free, through a STAGES-deep cp.async pipeline.
 #include <math.h>
 
+#include <algorithm>
+
 #include "common.h"
 
 namespace tatrg {
@@ -66,6 +68,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
         tile_m = band * RASTER_W + (in_band - tile_n * w);
     }
     const int m0 = tile_m * BM, n0 = tile_n * BN;
+    if (p.lower_only && n0 >= m0 + BM) return;   // tile strictly above the diagonal of a symmetric output
     int bz = blockIdx.z;
     const int split = bz / p.batch;
     bz -= split * p.batch;
@@ -277,7 +280,7 @@ void launch_cfg(const GemmParams &p_in)
     const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n;
     if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
     dim3 grid((unsigned)tiles, 1, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
-    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, BM == 128);
+    const int slot = prof_begin(gemm_flops(p), BM == 128);
     kern<<<grid, NT, smem, stream()>>>(p);
     prof_end(slot);
     TATRG_LAUNCH_CHECK();
@@ -297,7 +300,7 @@ void tensor_gemm(GemmParams p)
         TATRG_CUDA_CHECK(cudaGetDevice(&dev));
         TATRG_CUDA_CHECK(cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev));
     }
-    count_flops(2.0 * p.M * p.N * (double)p.K * p.batch);
+    count_flops(gemm_flops(p));
     // tile choice: 128x128 when it fills the machine (with split-K when the summed index is long),
     // 128x64 for outputs at most 64 columns wide with enough rows, else the 64x64 tile
     int ktiles = (p.K + BK - 1) / BK;
@@ -309,6 +312,13 @@ void tensor_gemm(GemmParams p)
     long long tiles = big ? big_tiles
                           : mid ? (long long)((p.M + 127) / 128) * p.batch
                                 : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
+    if (p.lower_only) {   // only the tiles that touch the lower triangle do work
+        const int bm = (big || mid) ? 128 : 64, bn = big ? 128 : 64;
+        const int tn = (p.N + bn - 1) / bn;
+        long long cnt = 0;
+        for (int m0 = 0; m0 < p.M; m0 += bm) cnt += std::min(tn, (m0 + bm - 1) / bn + 1);
+        tiles = cnt * p.batch;
+    }
     p.ksplit = 1;
     p.ktiles_per_split = ktiles;
     p.partial = nullptr;

@@ -5,7 +5,8 @@
 // swap (Table 1) and the O(r^2 chi^7) triad contraction (Eqs. 13-14)
 // run on.
 //
-// 8 (4) warps, warp tile 32 x 64 (64 FP64 accumulators per thread), BK = 16, 4-stage cp.async pipeline.
+// 128x128: 16 warps, warp tile 32 x 32 (32 FP64 accumulators per thread); 128x64: 4 warps, warp tile
+// 32 x 64.  BK = 16, 4-stage cp.async pipeline.
 // The shared-memory layout of an operand tile follows the operand's contiguous index in global
 // memory, so that 16-byte cp.async copies land on 16 consecutive bytes of shared memory:
 //   contiguous index = the free index (m or n):  tile stored [k][m], leading dimension 128 + 4
@@ -14,6 +15,8 @@
 // (lane -> (row = lane/4, k = lane%4)) conflict free.  Leg permutations stay folded into the gather
 // addresses (Map4); the 16-byte path is taken when every pair of consecutive elements along the
 // contiguous index is 16-byte aligned in global memory (checked on the host), else 8-byte copies.
+#include <stdlib.h>
+
 #include "common.h"
 
 namespace tatrg {
@@ -105,14 +108,14 @@ struct TileLoader {
     }
 };
 
-template <bool A_KF, bool B_KF, bool VEC, int BN>
-__global__ void __launch_bounds__(BN * 2, BN == 128 ? 1 : 2) tgemm_big_kernel(const __grid_constant__ GemmParams p)
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN>
+__global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_kernel(const __grid_constant__ GemmParams p)
 {
-    constexpr int NT = BN * 2;                        // (BM / 32) * (BN / 64) warps
+    constexpr int NT = 128 * BN / WN;                 // (BM / 32) * (BN / WN) warps
     constexpr int LD_FB = BN + 4;                     // [k][n] layout of the B tile
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
     constexpr int B_STAGE = B_KF ? BN * LD_K : BK * LD_FB;
-    constexpr int WM = 32, WN = 64, FM = WM / 8, FN = WN / 8;
+    constexpr int WM = 32, FM = WM / 8, FN = WN / 8;
     extern __shared__ __align__(16) double smem[];
     double *As = smem;
     double *Bs = smem + STAGES * A_STAGE;
@@ -128,6 +131,7 @@ __global__ void __launch_bounds__(BN * 2, BN == 128 ? 1 : 2) tgemm_big_kernel(co
         tile_m = band * RASTER_W + (in_band - tile_n * w);
     }
     const int m0 = tile_m * BM, n0 = tile_n * BN;
+    if (p.lower_only && n0 >= m0 + BM) return;   // tile strictly above the diagonal of a symmetric output
     int bz = blockIdx.z;
     const int split = bz / p.batch;
     bz -= split * p.batch;
@@ -245,15 +249,15 @@ __global__ void __launch_bounds__(BN * 2, BN == 128 ? 1 : 2) tgemm_big_kernel(co
     }
 }
 
-template <bool A_KF, bool B_KF, bool VEC, int BN>
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN>
 void launch_big(const GemmParams &p_in)
 {
-    constexpr int NT = BN * 2;
+    constexpr int NT = 128 * BN / WN;
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
     constexpr int B_STAGE = B_KF ? BN * LD_K : BK * (BN + 4);
     constexpr size_t smem = (size_t)STAGES * (A_STAGE + B_STAGE) * sizeof(double);
     static bool attr_done = false;
-    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN>;
+    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN, WN>;
     if (!attr_done) {
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
@@ -263,7 +267,7 @@ void launch_big(const GemmParams &p_in)
     const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n;
     if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
     dim3 grid((unsigned)tiles, 1, p.batch * (p.ksplit > 1 ? p.ksplit : 1));
-    const int slot = prof_begin(2.0 * p.M * p.N * (double)p.K * p.batch, BN == 128);
+    const int slot = prof_begin(gemm_flops(p), BN == 128);
     kern<<<grid, NT, smem, stream()>>>(p);
     prof_end(slot);
     TATRG_LAUNCH_CHECK();
@@ -284,7 +288,7 @@ bool vec_ok(const double *base, const Map4 &fast, const Map4 &slow, const Map4 &
            all_even(batch);
 }
 
-template <int BN>
+template <int BN, int WN>
 void dispatch_big(const GemmParams &p)
 {
     const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;
@@ -293,14 +297,14 @@ void dispatch_big(const GemmParams &p)
     const bool vec = va && vb;
     if (akf) {
         if (bkf)
-            vec ? launch_big<true, true, true, BN>(p) : launch_big<true, true, false, BN>(p);
+            vec ? launch_big<true, true, true, BN, WN>(p) : launch_big<true, true, false, BN, WN>(p);
         else
-            vec ? launch_big<true, false, true, BN>(p) : launch_big<true, false, false, BN>(p);
+            vec ? launch_big<true, false, true, BN, WN>(p) : launch_big<true, false, false, BN, WN>(p);
     } else {
         if (bkf)
-            vec ? launch_big<false, true, true, BN>(p) : launch_big<false, true, false, BN>(p);
+            vec ? launch_big<false, true, true, BN, WN>(p) : launch_big<false, true, false, BN, WN>(p);
         else
-            vec ? launch_big<false, false, true, BN>(p) : launch_big<false, false, false, BN>(p);
+            vec ? launch_big<false, false, true, BN, WN>(p) : launch_big<false, false, false, BN, WN>(p);
     }
 }
 
@@ -308,10 +312,16 @@ void dispatch_big(const GemmParams &p)
 
 void tensor_gemm_big(const GemmParams &p, int bn)
 {
+    // 128x128: 16 warps x (32 x 32) measured 2.5-3 % faster than 8 warps x (32 x 64) on the c3 shapes
+    // (four warps per scheduler keep the DMMA pipe fed across the per-k-tile barrier);
+    // TATRG_GEMM_WN64 selects the 8-warp variant for comparison
+    static const bool wn64 = getenv("TATRG_GEMM_WN64") != nullptr;
     if (bn == 64)
-        dispatch_big<64>(p);
+        dispatch_big<64, 64>(p);
+    else if (wn64)
+        dispatch_big<128, 64>(p);
     else
-        dispatch_big<128>(p);
+        dispatch_big<128, 32>(p);
 }
 
 }  // namespace tatrg

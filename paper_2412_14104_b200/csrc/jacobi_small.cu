@@ -75,10 +75,19 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
         __syncthreads();
     }
     const double dead = 1e-40 * fro2_s;
+    const double tol2 = tol * tol;
     const int npad = n + (n & 1);
     int sweep = 0;
     for (; n > 1 && sweep < max_sweeps; ++sweep) {
         if (t == 0) nrot = 0;
+        // squared column norms: recomputed once per sweep, then carried through the rotations
+        // (a_pp' = a_pp - t a_pq, a_qq' = a_qq + t a_pq), so that a pair costs one dot product
+        for (int j = warp; j < n; j += NW) {
+            double a = 0.0;
+            for (int i = lane; i < m; i += 32) a = fma(W[j * ld + i], W[j * ld + i], a);
+            a = warp_sum(a);
+            if (lane == 0) nrm[j] = a;
+        }
         __syncthreads();
         for (int round = 0; round < npad - 1; ++round) {
             for (int pi = warp; pi < npad / 2; pi += NW) {
@@ -86,30 +95,24 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
                 rr_pair(round, pi, npad, p, q);
                 if (q >= n) continue;
                 double *cp = W + p * ld, *cq = W + q * ld;
-                double aa = 0.0, bb = 0.0, ab = 0.0;
-                for (int i = lane; i < m; i += 32) {
-                    double a = cp[i], b = cq[i];
-                    aa = fma(a, a, aa);
-                    bb = fma(b, b, bb);
-                    ab = fma(a, b, ab);
-                }
-                aa = warp_sum(aa);
-                bb = warp_sum(bb);
-                ab = warp_sum(ab);
+                const double aa = nrm[p], bb = nrm[q];
                 if (aa == 0.0 && bb == 0.0) continue;
+                double ab = 0.0;
+                for (int i = lane; i < m; i += 32) ab = fma(cp[i], cq[i], ab);
+                ab = warp_sum(ab);
                 const bool swap = aa < bb;
-                double c = 1.0, s = 0.0;
+                double c = 1.0, s = 0.0, na2 = aa, nb2 = bb;
                 bool rot = false;
-                if (aa > dead && bb > dead) {
-                    double cosv = fabs(ab) / sqrt(aa * bb);
-                    if (cosv > tol) {
-                        double zeta = (bb - aa) / (2.0 * ab);
-                        double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                        c = 1.0 / sqrt(1.0 + tt * tt);
-                        s = c * tt;
-                        rot = true;
-                        if (lane == 0) atomicAdd(&nrot, 1);
-                    }
+                if (aa > dead && bb > dead && ab * ab > tol2 * aa * bb) {
+                    // tan of the rotation angle: the smaller root of t^2 + 2 zeta t - 1 = 0, zeta = (bb - aa) / (2 ab)
+                    const double dlt = bb - aa;
+                    const double tt = copysign(2.0 * fabs(ab), dlt * ab) / (fabs(dlt) + sqrt(fma(dlt, dlt, 4.0 * ab * ab)));
+                    c = rsqrt(fma(tt, tt, 1.0));
+                    s = c * tt;
+                    na2 = aa - tt * ab;
+                    nb2 = bb + tt * ab;
+                    rot = true;
+                    if (lane == 0) atomicAdd(&nrot, 1);
                 }
                 if (!rot && !swap) continue;
                 for (int i = lane; i < ld; i += 32) {
@@ -117,6 +120,10 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
                     double na = c * a - s * b, nb = s * a + c * b;
                     cp[i] = swap ? nb : na;
                     cq[i] = swap ? na : nb;
+                }
+                if (lane == 0) {
+                    nrm[p] = swap ? nb2 : na2;
+                    nrm[q] = swap ? na2 : nb2;
                 }
             }
             __syncthreads();
@@ -198,9 +205,9 @@ __global__ void __launch_bounds__(SJ_NT) eig_small_kernel(const double *__restri
                     // the classical relative criterion: a pair is converged when |a_pq| <= eps sqrt(|a_pp a_qq|)
                     if (fabs(apq) > floor_abs && fabs(apq) > 2.2e-16 * sqrt(fabs(app * aqq))) {
                         atomicAdd(&nrot, 1);
-                        double zeta = (aqq - app) / (2.0 * apq);
-                        double tt = copysign(1.0, zeta) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                        c = 1.0 / sqrt(1.0 + tt * tt);
+                        const double dlt = aqq - app;
+                        const double tt = copysign(2.0 * fabs(apq), dlt * apq) / (fabs(dlt) + sqrt(fma(dlt, dlt, 4.0 * apq * apq)));
+                        c = rsqrt(fma(tt, tt, 1.0));
                         s = c * tt;
                     }
                 } else {

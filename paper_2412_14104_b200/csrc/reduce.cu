@@ -252,13 +252,14 @@ void fill_zero(double *x, long long n)
     TATRG_CUDA_CHECK(cudaMemsetAsync(x, 0, n * sizeof(double), stream()));
 }
 
-// out[0] = max_ij |G_ij - delta_ij| (non-negative doubles order like their bit patterns)
+// out[0] = max_{i >= j} |G_ij - delta_ij| (non-negative doubles order like their bit patterns)
 __global__ void max_dev_identity_kernel(const double *__restrict__ G, int n, unsigned long long *__restrict__ out)
 {
     const long long total = (long long)n * n;
     double m = 0.0;
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
         const int r = (int)(i / n), c = (int)(i - (long long)r * n);
+        if (c > r) continue;
         const double v = fabs(G[i] - (r == c ? 1.0 : 0.0));
         m = (v > m || v != v) ? v : m;
     }

@@ -331,14 +331,14 @@ bool ortho_factor(const Ten &T, RedBasis &o)
     size_t mk = ws_mark();
     Ten G1 = ws_tensor("cbde", {n0, a, n0, a});
     Ten L1inv = ws_tensor("kcb", {nk, n0, a});
-    contract(T.as("cpqtb"), T.as("dpqte"), G1);
+    contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true);
     if (!cholesky_lower(G1.p, (int)nk, 0.0, L1inv.p)) {
         ws_release(mk);
         return false;
     }
     contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
     Ten G2 = ws_tensor("kl", {nk, nk});
-    contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2);
+    contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
     double *dev = ws_doubles(1);
     max_dev_identity(G2.p, (int)nk, dev);
     const double err = d2h(dev, 1)[0];

@@ -113,7 +113,7 @@ long long total(const std::vector<GLeg> &g)
 
 }  // namespace
 
-void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accumulate)
+void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accumulate, bool lower_only)
 {
     std::vector<GLeg> gb, gm, gn, gk;  // strides: batch (A,B,C); m (A,C); n (B,C); k (A,B)
     std::string seen;
@@ -149,7 +149,7 @@ void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accum
     p.B = B.p;
     p.C = C.p;
     long long M = total(gm), N = total(gn), K = total(gk), Bt = total(gb);
-    if (M <= 64 && N > 64) {   // the wide index goes to the 128-row side of the CTA tile
+    if (M <= 64 && N > 64 && !lower_only) {   // the wide index goes to the 128-row side of the CTA tile
         contract(B, A, C, alpha, accumulate);
         return;
     }
@@ -170,6 +170,7 @@ void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accum
     p.cb = to_map(gb, 2, "batch");
     p.alpha = alpha;
     p.accumulate = accumulate ? 1 : 0;
+    p.lower_only = (lower_only && M == N) ? 1 : 0;
     // loader order: walk whichever index has the smaller leading stride in that operand
     long long am0 = gm.empty() ? (1LL << 60) : gm[0].s[0];
     long long ak0 = gk.empty() ? (1LL << 60) : gk[0].s[0];

@@ -34,6 +34,9 @@ Ten ws_tensor(const char *names, std::initializer_list<long long> dims);
 
 // C (+)= alpha * sum_{legs shared by A and B only} A * B.
 // Legs in A, B and C: batch; A and C: rows; B and C: columns.  Any other pattern is an error.
-void contract(const Ten &A, const Ten &B, const Ten &C, double alpha = 1.0, bool accumulate = false);
+// lower_only: C is a symmetric matrix (rows and columns enumerate the same index in the same order);
+// only its lower triangle is guaranteed to be written.
+void contract(const Ten &A, const Ten &B, const Ten &C, double alpha = 1.0, bool accumulate = false,
+              bool lower_only = false);
 
 }  // namespace tatrg
