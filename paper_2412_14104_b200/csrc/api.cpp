@@ -100,6 +100,12 @@ void prof_collect()
         c.gemm_n[r.stage][r.big] += 1;
     }
     c.prof_rec.clear();
+    if (trace) {
+        fprintf(stderr, "tatrg-trace host: %lld tensor_gemm calls, %.3f ms on the host (%.2f us each)\n", c.host_contract_n,
+                1e3 * c.host_contract_s, c.host_contract_n ? 1e6 * c.host_contract_s / c.host_contract_n : 0.0);
+        c.host_contract_s = 0;
+        c.host_contract_n = 0;
+    }
 }
 
 void *ws_alloc(size_t bytes)
@@ -144,6 +150,7 @@ int guarded(F f)
         f();
         return TATRG_OK;
     } catch (const Err &e) {
+        cudaDeviceSynchronize();   // nothing of a failed call (side streams included) is left in flight
         cudaGetLastError();
         return e.code;
     } catch (const std::exception &e) {
@@ -480,6 +487,14 @@ void tatrg_destroy(void)
     if (c.ev_ok)
         for (auto &e : c.ev) cudaEventDestroy(e);
     for (auto &e : c.prof_ev) cudaEventDestroy(e);
+    if (c.side_ok) {
+        for (auto &st : c.side) cudaStreamDestroy(st);
+        for (auto &e : c.join_ev) cudaEventDestroy(e);
+        cudaEventDestroy(c.fork_ev);
+    }
+    if (c.pinned) cudaFreeHost(c.pinned);
+    for (auto &b : c.start_blk)
+        if (b) cudaFreeHost(b);
     c = Ctx();
 }
 

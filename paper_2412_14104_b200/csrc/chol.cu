@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ 
             if (t == 0) bad = 1;
             piv = 1.0;
         }
-        const double d = sqrt(piv), rd = 1.0 / d;
+        const double rd = rsqrt(piv), d = piv * rd;   // one special-function chain instead of sqrt + divide
         if (t == 0) diag[j] = d;
         double li[4], lc[4], wj[4];
 #pragma unroll
@@ -210,11 +210,9 @@ void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double
 // Cholesky factor (upper triangle zeroed) after adding shift_rel * max_i A_ii to the diagonal.
 // Linv_full (optional, n x n row-major) receives L^-1.
 // Returns false when a pivot was not positive (A then holds garbage).
-bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
+void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full, int *flag)
 {
     size_t mark = ws_mark();
-    int *flag = (int *)ws_alloc(sizeof(int));
-    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
     double *Linv = ws_doubles(NB * NB);
     if (shift_rel > 0.0) {
         add_shift_kernel<<<1, 256, 0, stream()>>>(A, n, shift_rel);
@@ -274,6 +272,15 @@ bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
             if (n - j0 > sz) pair(j0, n - j0 - sz, 1);                 // ragged last pair
         }
     }
+    ws_release(mark);
+}
+
+bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
+{
+    size_t mark = ws_mark();
+    int *flag = (int *)ws_alloc(sizeof(int));
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    cholesky_lower_async(A, n, shift_rel, Linv_full, flag);
     int h = 0;
     TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));

@@ -112,6 +112,9 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
                 long long strideV, long long strideS);
 // jacobi_small.cu : one-CTA versions for m, n <= 64 (same output conventions)
 void svd_small(double *G, int m, int n, double *V, double *s);
+// without host synchronisation: no convergence within the sweep limit raises *flag_dev (sticky, device)
+void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev);
+void eig_small_async(const double *S, int n, double *V, double *lam, int *flag_dev);
 void eig_small(const double *S, int n, double *V, double *lam);   // symmetric S; V column j = eigenvector j
 // reduce.cu
 void sumsq(const double *x, long long n, double *out);                       // out[0] = sum x^2
@@ -132,6 +135,8 @@ void max_dev_identity(const double *G, int n, double *out);                   //
 // chol.cu : in place lower Cholesky factor of the symmetric n x n matrix A (+ shift_rel * max diag on the
 // diagonal); false if a pivot was not positive
 bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full = nullptr);
+// the same without host synchronisation: a non-positive pivot raises *flag_dev (sticky, device)
+void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full, int *flag_dev);
 // G = I + E, |E| <~ 1e-8: in place lower Cholesky factor and its inverse by the first-order formulas (error O(|E|^2))
 void near_identity_chol(double *G, int n, double *Linv);
 void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel = 0.0);

@@ -31,6 +31,18 @@ struct Ctx {
     bool state_low = true;                  // the state sits at the low end of ws
     size_t state_bytes = 0;
 
+    // independent chains of small kernels (the three squeezers, the four isometries) run on side
+    // streams forked from / joined to `stream` with events; each chain bump-allocates from its own
+    // slice of the free workspace (step.cpp: Fork)
+    static constexpr int MAX_CHAINS = 4;
+    cudaStream_t side[MAX_CHAINS] = {};
+    cudaEvent_t fork_ev = nullptr, join_ev[MAX_CHAINS] = {};
+    bool side_ok = false;
+    char *pinned = nullptr;                 // page-locked host scratch for asynchronous read-backs
+    static constexpr size_t PINNED_BYTES = 1 << 16;
+    double *start_blk[4] = {};              // page-locked start blocks of the iterative solvers
+    long long start_blk_n[4] = {};
+
     Input in[9];
     std::vector<double> spec[10];
     double gaps[4] = {0, 0, 0, 0};
@@ -55,6 +67,8 @@ struct Ctx {
         int shape[5];   // M, N, K, batch, ksplit
     };
     int prof_shape[5] = {0, 0, 0, 0, 0};
+    double host_contract_s = 0;   // host seconds spent inside contract() (trace only)
+    long long host_contract_n = 0;
     std::vector<ProfRec> prof_rec;
     double gemm_ms[ST_COUNT][2] = {};      // [stage][0: 64x64 tile, 1: 128x128 tile]
     double gemm_fl[ST_COUNT][2] = {};

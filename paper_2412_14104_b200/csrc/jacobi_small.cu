@@ -278,20 +278,25 @@ void set_attr()
 
 }  // namespace
 
-// One-CTA SVD; requires m, n <= 64.  Same contract as jacobi_svd (batch 1).
-void svd_small(double *G, int m, int n, double *V, double *s)
+void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev)
 {
     if (m > SJ_MAX || n > SJ_MAX || m < 1 || n < 1) fail(-22, "svd_small: size %d x %d not supported", m, n);
     set_attr();
-    size_t mark = ws_mark();
-    int *flag = (int *)ws_alloc(sizeof(int));
-    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
     const int mn = m > n ? m : n;
     const double tol = 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
     const size_t smem = (size_t)n * (m + n) * sizeof(double);
-    svd_small_kernel<<<1, SJ_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag);
+    svd_small_kernel<<<1, SJ_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag_dev);
     TATRG_LAUNCH_CHECK();
     count_launch();
+}
+
+// One-CTA SVD; requires m, n <= 64.  Same contract as jacobi_svd (batch 1).
+void svd_small(double *G, int m, int n, double *V, double *s)
+{
+    size_t mark = ws_mark();
+    int *flag = (int *)ws_alloc(sizeof(int));
+    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    svd_small_async(G, m, n, V, s, flag);
     int h = 0;
     TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
@@ -299,18 +304,23 @@ void svd_small(double *G, int m, int n, double *V, double *s)
     if (h) fail(-34, "svd_small: no convergence (m=%d n=%d)", m, n);
 }
 
-// One-CTA symmetric eigensolver; n <= 64.  V column-major (column j = eigenvector j), lam descending.
-void eig_small(const double *S, int n, double *V, double *lam)
+void eig_small_async(const double *S, int n, double *V, double *lam, int *flag_dev)
 {
     if (n > SJ_MAX || n < 1) fail(-22, "eig_small: n = %d not supported", n);
     set_attr();
+    const size_t smem = (size_t)2 * n * (n + 1) * sizeof(double);
+    eig_small_kernel<<<1, SJ_NT, smem, stream()>>>(S, n, V, lam, 60, flag_dev);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
+
+// One-CTA symmetric eigensolver; n <= 64.  V column-major (column j = eigenvector j), lam descending.
+void eig_small(const double *S, int n, double *V, double *lam)
+{
     size_t mark = ws_mark();
     int *flag = (int *)ws_alloc(sizeof(int));
     TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
-    const size_t smem = (size_t)2 * n * (n + 1) * sizeof(double);
-    eig_small_kernel<<<1, SJ_NT, smem, stream()>>>(S, n, V, lam, 60, flag);
-    TATRG_LAUNCH_CHECK();
-    count_launch();
+    eig_small_async(S, n, V, lam, flag);
     int h = 0;
     TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));

@@ -86,6 +86,81 @@ Ten gauge_rotation(const Ten &P, const std::vector<double> &s, int k)
     return W;
 }
 
+// Fork / join of independent chains of small kernels (the three squeezers, the four isometries):
+// chain i enqueues on side stream i, which waits for everything enqueued on the main stream so
+// far, and bump-allocates from its own slice of the free workspace; join() makes the main stream
+// wait for all chains and returns the slices.  Between enter(i) and leave() every launcher of the
+// library (they all use stream() and the workspace allocator) works for chain i.  Buffers that must
+// outlive the join are allocated on the main stream before the Fork is constructed.
+class Fork {
+public:
+    explicit Fork(int n) : c_(ctx()), n_(n), main_(c_.stream), lo0_(c_.lo), hi0_(c_.hi)
+    {
+        if (n < 1 || n > Ctx::MAX_CHAINS) fail(-22, "Fork: %d chains", n);
+        if (!c_.side_ok) {
+            for (auto &st : c_.side) TATRG_CUDA_CHECK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+            for (auto &e : c_.join_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&c_.fork_ev, cudaEventDisableTiming));
+            c_.side_ok = true;
+        }
+        if (!c_.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c_.pinned, Ctx::PINNED_BYTES));
+        TATRG_CUDA_CHECK(cudaEventRecord(c_.fork_ev, main_));
+        const size_t slice = ((hi0_ - lo0_) / n) & ~(size_t)255;
+        for (int i = 0; i < n; ++i) {
+            TATRG_CUDA_CHECK(cudaStreamWaitEvent(c_.side[i], c_.fork_ev, 0));
+            lo_[i] = lo0_ + i * slice;
+            hi_[i] = lo_[i] + slice;
+        }
+        c_.lo = c_.hi = hi0_;   // nothing is allocated on the main stream while forked
+    }
+    void enter(int i)
+    {
+        cur_ = i;
+        c_.stream = c_.side[i];
+        c_.lo = lo_[i];
+        c_.hi = hi_[i];
+    }
+    void leave()
+    {
+        if (cur_ < 0) return;
+        lo_[cur_] = c_.lo;
+        c_.peak = std::max(c_.peak, c_.lo + (c_.ws_bytes - hi0_));
+        cur_ = -1;
+        c_.stream = main_;
+        c_.lo = c_.hi = hi0_;
+    }
+    void sync(int i) { TATRG_CUDA_CHECK(cudaStreamSynchronize(c_.side[i])); }
+    // page-locked host scratch of chain i (PINNED_BYTES / MAX_CHAINS bytes)
+    char *pinned(int i) { return c_.pinned + (size_t)i * (Ctx::PINNED_BYTES / Ctx::MAX_CHAINS); }
+    void join()
+    {
+        leave();
+        for (int i = 0; i < n_; ++i) {
+            TATRG_CUDA_CHECK(cudaEventRecord(c_.join_ev[i], c_.side[i]));
+            TATRG_CUDA_CHECK(cudaStreamWaitEvent(main_, c_.join_ev[i], 0));
+        }
+        c_.lo = lo0_;
+        c_.hi = hi0_;
+        joined_ = true;
+    }
+    ~Fork()
+    {
+        if (joined_) return;
+        c_.stream = main_;   // unwinding after an error: the caller (guarded) drains the device
+        c_.lo = lo0_;
+        c_.hi = hi0_;
+    }
+
+private:
+    Ctx &c_;
+    int n_;
+    cudaStream_t main_;
+    size_t lo0_, hi0_;
+    size_t lo_[Ctx::MAX_CHAINS], hi_[Ctx::MAX_CHAINS];
+    int cur_ = -1;
+    bool joined_ = false;
+};
+
 struct StepCfg {
     uint64_t seed;
     int step;
@@ -192,18 +267,19 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
 // convergence, so the result does not depend on it beyond rounding).
 Ten solver_start_block(long long rows, long long cols, int tag, const char *names2)
 {
-    static std::vector<double> cache[4];
-    static long long cache_n[4] = {0, 0, 0, 0};
-    std::vector<double> local;
-    std::vector<double> &host = (tag >= 0 && tag < 4) ? cache[tag] : local;
-    if ((tag < 0 || tag >= 4) || cache_n[tag] != rows * cols) {
-        host.resize((size_t)(rows * cols));
-        si_fill_gauss(host.data(), (uint64_t)(rows * cols), si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
-        if (tag >= 0 && tag < 4) cache_n[tag] = rows * cols;
+    Ctx &c = ctx();
+    if (tag < 0 || tag >= 4) fail(-22, "solver_start_block: tag %d", tag);
+    const long long n = rows * cols;
+    if (c.start_blk_n[tag] != n) {   // page-locked host cache: the upload below is then truly asynchronous
+        if (c.start_blk[tag]) cudaFreeHost(c.start_blk[tag]);
+        c.start_blk[tag] = nullptr;
+        c.start_blk_n[tag] = 0;
+        TATRG_CUDA_CHECK(cudaMallocHost((void **)&c.start_blk[tag], sizeof(double) * n));
+        si_fill_gauss(c.start_blk[tag], (uint64_t)n, si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
+        c.start_blk_n[tag] = n;
     }
     Ten t = ws_tensor(names2, {rows, cols});
-    h2d(t.p, host.data(), rows * cols);
-    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    h2d(t.p, c.start_blk[tag], n);
     return t;
 }
 
@@ -214,98 +290,135 @@ Ten solver_start_block(long long rows, long long cols, int tag, const char *name
 // chi, iteration count from the measured decay s_b / s_chi so that the neglected part is below
 // 1e-13.  Returns false (nothing written) when a Gram matrix is not numerically positive definite
 // or fewer than chi significant triplets exist -- the caller then uses the dense path.
-struct SqueezeOut {
-    int k;
-    std::vector<double> s;   // Ritz values, descending (>= k of them)
-    double *s_dev;
-    double gap;
-};
-
-bool squeezer_subspace(const Ten &GLm, const Ten &GRm, int N2, int chi, int mu, Ten &Mr, Ten &Nr, SqueezeOut &o)
-{
-    const int b = 64;
-    if (N2 < 256 || chi >= b) return false;
-    Ten LL = ws_tensor("ki", {N2, N2}), LR = ws_tensor("kj", {N2, N2});
-    d2d(LL.p, GLm.p, (long long)N2 * N2);
-    d2d(LR.p, GRm.p, (long long)N2 * N2);
-    const double shift = 3e-14;
-    if (!cholesky_lower(LL.p, N2, shift) || !cholesky_lower(LR.p, N2, shift)) return false;
-    Ten F = ws_tensor("ij", {N2, N2});
-    contract(LL, LR, F);                                   // F = L_L^T L_R
-    auto mulF = [&](const double *w, double *out) {        // F w
-        contract(F, Ten::make(const_cast<double *>(w), "jz", {N2, b}), Ten::make(out, "iz", {N2, b}));
+// It is written as a chain in phases (enqueue only; the host reads the page-locked read-back
+// after synchronising the chain's stream), so that the three squeezers of a step run concurrently
+// on three streams (Fork).
+struct SqChain {
+    static constexpr int b = 64;
+    struct Back {          // page-locked read-back
+        int flag;
+        int pad;
+        double ratio[4];
+        double s[b];
     };
-    auto mulFt = [&](const double *w, double *out) {       // F^T w
-        contract(F, Ten::make(const_cast<double *>(w), "iz", {N2, b}), Ten::make(out, "jz", {N2, b}));
-    };
-    // Subspace iteration Q <- orth(F orth(F^T Q)).  Between iterations one (shifted) Cholesky-QR pass
-    // is enough: only the span is carried on; the two blocks that enter the Ritz step get two passes.
-    int *flag = (int *)ws_alloc(sizeof(int));
-    TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
-    double *ratio = ws_doubles(4);
-    Ten om = solver_start_block(N2, b, mu, "jz");
-    double *Q = ws_doubles((long long)N2 * b), *Qt = ws_doubles((long long)N2 * b);
-    double *Rb = ws_doubles((long long)b * b), *V = ws_doubles((long long)b * b), *sv = ws_doubles(b);
-    const double it_shift = 1e-13;
-    mulF(om.p, Q);
-    cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
-    auto ritz_blocks = [&](std::vector<double> &sh) {      // Q <- orth2(F Qt) is done by the caller
-        mulFt(Q, Qt);                                      // B^T = F^T Q = Q_B R_B
-        cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
-        jacobi_svd(Rb, b, b, V, sv, 1, 0, 0, 0);           // R_B^T V = U diag(s)
-        struct {
-            int f;
-            double r[4];
-        } h;
-        TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
-        TATRG_CUDA_CHECK(cudaMemcpyAsync(h.r, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
-        sh = d2h(sv, b);
-        // a failed factorisation, or a block too ill conditioned for two Cholesky-QR passes
-        return h.f == 0 && h.r[0] > 1e-5 * h.r[1] && h.r[2] > 1e-5 * h.r[3];
-    };
-    for (int it = 0; it < 2; ++it) {
-        mulFt(Q, Qt);
-        cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
-        mulF(Qt, Q);
-        cholqr_async(Q, N2, b, it == 1 ? 2 : 1, it == 1 ? 0.0 : it_shift, flag, it == 1 ? ratio : nullptr, nullptr);
-    }
+    Ten GLm, GRm;
+    int N2 = 0, chi = 0, mu = 0;
+    bool active = false, ok = false;
+    Ten LL, LR, F;
+    int *flag = nullptr;
+    double *ratio = nullptr, *Q = nullptr, *Qt = nullptr, *Rb = nullptr, *V = nullptr, *sv = nullptr;
+    Back *back = nullptr;
     std::vector<double> sh;
-    if (!ritz_blocks(sh)) return false;
-    if (!(sh[chi - 1] > 1e-6 * sh[0])) return false;
-    const double rho = sh[b - 1] / sh[chi - 1];
-    const int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
-    const int more = std::max(1, std::min(need + 1, 80) - 2);   // two iterations are done
-    for (int it = 0; it < more; ++it) {
-        const bool last = it == more - 1;
-        mulF(Qt, Q);                                       // Qt = orth(F^T Q) from the Ritz step / the loop
-        cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
-        if (!last) {
+    int more = 0, k = 0;
+    double gap = INFINITY;
+    Ten Mr, Nr;
+    static constexpr double it_shift = 1e-13;
+
+    void mulF(const double *w, double *out)    // F w
+    {
+        contract(F, Ten::make(const_cast<double *>(w), "jz", {N2, b}), Ten::make(out, "iz", {N2, b}));
+    }
+    void mulFt(const double *w, double *out)   // F^T w
+    {
+        contract(F, Ten::make(const_cast<double *>(w), "iz", {N2, b}), Ten::make(out, "jz", {N2, b}));
+    }
+    // Ritz step on the current Q (two Cholesky-QR passes have just been applied to it):
+    // B^T = F^T Q = Q_B R_B, R_B^T V = U diag(s); read-back of flag, condition estimates, s
+    void enqueue_ritz()
+    {
+        mulFt(Q, Qt);
+        cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
+        svd_small_async(Rb, b, b, V, sv, flag);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(back->s, sv, b * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+    }
+    // after the chain's stream has been synchronised
+    bool read_back()
+    {
+        sh.assign(back->s, back->s + b);
+        // a failed factorisation / Jacobi, or a block too ill conditioned for two Cholesky-QR passes
+        return back->flag == 0 && back->ratio[0] > 1e-5 * back->ratio[1] && back->ratio[2] > 1e-5 * back->ratio[3];
+    }
+    void phaseA(char *pinned)
+    {
+        back = reinterpret_cast<Back *>(pinned);
+        LL = ws_tensor("ki", {N2, N2});
+        LR = ws_tensor("kj", {N2, N2});
+        d2d(LL.p, GLm.p, (long long)N2 * N2);
+        d2d(LR.p, GRm.p, (long long)N2 * N2);
+        flag = (int *)ws_alloc(sizeof(int));
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+        const double shift = 3e-14;
+        cholesky_lower_async(LL.p, N2, shift, nullptr, flag);
+        cholesky_lower_async(LR.p, N2, shift, nullptr, flag);
+        F = ws_tensor("ij", {N2, N2});
+        contract(LL, LR, F);                               // F = L_L^T L_R
+        ratio = ws_doubles(4);
+        Ten om = solver_start_block(N2, b, mu, "jz");
+        Q = ws_doubles((long long)N2 * b);
+        Qt = ws_doubles((long long)N2 * b);
+        Rb = ws_doubles((long long)b * b);
+        V = ws_doubles((long long)b * b);
+        sv = ws_doubles(b);
+        // Subspace iteration Q <- orth(F orth(F^T Q)).  Between iterations one (shifted) Cholesky-QR
+        // pass is enough: only the span is carried on; the blocks that enter a Ritz step get two.
+        mulF(om.p, Q);
+        cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
+        for (int it = 0; it < 2; ++it) {
             mulFt(Q, Qt);
             cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
+            mulF(Qt, Q);
+            cholqr_async(Q, N2, b, it == 1 ? 2 : 1, it == 1 ? 0.0 : it_shift, flag, it == 1 ? ratio : nullptr, nullptr);
         }
+        enqueue_ritz();
     }
-    if (!ritz_blocks(sh)) return false;
-    o.k = num_rank(sh, chi);
-    if (o.k < chi) return false;
-    const int k = o.k;
-    o.s = sh;
-    o.gap = rel_gap(sh, k);
-    o.s_dev = sv;
-    scale_leg(Rb, (long long)k * b, b, k, sv, 1);          // columns of U
-    Ten Uk = Ten::make(Rb, "kz", {b, b}), Vk = Ten::make(V, "kz", {b, b});
-    Uk.legs[0].n = k;
-    Vk.legs[0].n = k;
-    Ten left = ws_tensor("ik", {N2, k}), right = ws_tensor("jk", {N2, k});
-    contract(Ten::make(Q, "iz", {N2, b}), Uk, left);
-    contract(Ten::make(Qt, "jz", {N2, b}), Vk, right);
-    Mr = ws_tensor("nk", {N2, k});
-    Nr = ws_tensor("kn", {k, N2});
-    contract(left, LL.as("ni"), Nr);                       // N = s^-1/2 U^T L_L^T
-    contract(LR.as("nj"), right, Mr);                      // M = L_R V s^-1/2
-    scale_leg(Nr.p, Nr.size(), N2, k, o.s_dev, 3);
-    scale_leg(Mr.p, Mr.size(), 1, k, o.s_dev, 3);
-    return true;
-}
+    // iteration count from the measured decay rho = s_b / s_chi: rho^(2p+1) < 1e-13
+    bool plan()
+    {
+        if (!read_back()) return false;
+        if (!(sh[chi - 1] > 1e-6 * sh[0])) return false;
+        const double rho = sh[b - 1] / sh[chi - 1];
+        const int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
+        more = std::max(1, std::min(need + 1, 80) - 2);    // two iterations are done
+        return true;
+    }
+    void phaseB()
+    {
+        for (int it = 0; it < more; ++it) {
+            const bool last = it == more - 1;
+            mulF(Qt, Q);                                   // Qt = orth(F^T Q) from the Ritz step / the loop
+            cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
+            if (!last) {
+                mulFt(Q, Qt);
+                cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
+            }
+        }
+        enqueue_ritz();
+    }
+    // M = L_R V s^-1/2, N = s^-1/2 U^T L_L^T from the converged triplets
+    bool phaseC()
+    {
+        if (!read_back()) return false;
+        k = num_rank(sh, chi);
+        if (k < chi) return false;
+        gap = rel_gap(sh, k);
+        scale_leg(Rb, (long long)k * b, b, k, sv, 1);      // columns of U
+        Ten Uk = Ten::make(Rb, "kz", {b, b}), Vk = Ten::make(V, "kz", {b, b});
+        Uk.legs[0].n = k;
+        Vk.legs[0].n = k;
+        Ten left = ws_tensor("ik", {N2, k}), right = ws_tensor("jk", {N2, k});
+        contract(Ten::make(Q, "iz", {N2, b}), Uk, left);
+        contract(Ten::make(Qt, "jz", {N2, b}), Vk, right);
+        Mr = ws_tensor("nk", {N2, k});
+        Nr = ws_tensor("kn", {k, N2});
+        contract(left, LL.as("ni"), Nr);
+        contract(LR.as("nj"), right, Mr);
+        scale_leg(Nr.p, Nr.size(), N2, k, sv, 3);
+        scale_leg(Mr.p, Mr.size(), 1, k, sv, 3);
+        return true;
+    }
+};
 
 // Orthonormal basis of the column space of the matricisation T2[(pqt); (c,b)] of T[c,p,q,t,b]
 // (nT x nk, nk = n0 * a), by two Cholesky-QR passes with explicit triangular inverses so that all
@@ -664,8 +777,17 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ten RX = ws_tensor("ab", {a, a}), RY = ws_tensor("ab", {a, a});
         contract(Xs.as("apqtg"), Xs.as("bpqtg"), RX);
         contract(Ys.as("apqtg"), Ys.as("bpqtg"), RY);
-        for (int i = 0; i < 4; ++i) {
-            // the symmetric PSD operator S = K K_w^T on the pair space (reading G6b)
+        for (int i = 0; i < 4; ++i) U[i] = ws_tensor("pqk", {n1, n2, kk});
+        struct IsoBack {   // page-locked read-back of one chain
+            int flag;
+            int pad;
+            double ratio[16];
+            double lam[64];
+        };
+        // One isometry: subspace iteration on the symmetric PSD operator S = K K_w^T on the pair space
+        // (reading G6b), then a Ritz step.  fast: asynchronous Cholesky-QR and one-CTA eigensolver, no
+        // host synchronisation (the caller checks the read-back); else the robust synchronous route.
+        auto iso_body = [&](int i, bool fast, IsoBack *back) {
             const Ten &Kt = (i == 0) ? A : (i == 1) ? Xs : (i == 2) ? Ys : D;
             const bool mid = (i == 0 || i == 3);
             const Ten &Rm = (i == 0) ? RX : RY;
@@ -680,27 +802,76 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                     contract(Kt.as("xpqta"), t1, Ten::make(out, "pqz", {n1, n2, kk}));
                 }
             };
+            int *flag = nullptr;
+            double *ratio = nullptr;
+            if (fast) {
+                flag = (int *)ws_alloc(sizeof(int));
+                TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+                ratio = ws_doubles(16);
+            }
+            int nqr = 0;
+            auto orth = [&](double *Y) {
+                if (fast) {
+                    cholqr_async(Y, n12, kk, 2, 0.0, flag, ratio + 2 * nqr, nullptr);
+                    ++nqr;
+                } else {
+                    double *Rtmp = ws_doubles((long long)kk * kk);
+                    tsqr(Y, n12, kk, Rtmp);
+                }
+            };
             Ten om = get_input(1 + i, n12, kk, cfg, "rz");
             Ten Qi = ws_tensor("rz", {n12, kk}), SQ = ws_tensor("ry", {n12, kk});
-            double *Rtmp = ws_doubles((long long)kk * kk);
             S_op(om.p, Qi.p);
-            tsqr(Qi.p, n12, kk, Rtmp);
+            orth(Qi.p);
             for (int it = 0; it < q; ++it) {
                 S_op(Qi.p, SQ.p);
                 d2d(Qi.p, SQ.p, n12 * kk);
-                tsqr(Qi.p, n12, kk, Rtmp);
+                orth(Qi.p);
             }
             S_op(Qi.p, SQ.p);
             Ten Hm = ws_tensor("zy", {kk, kk});
             contract(Qi, SQ, Hm);
             Ten Vt = ws_tensor("kz", {kk, kk});
             double *lam = ws_doubles(kk);
-            std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);
-            spec[2 + i].resize(kk);
-            for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
-            U[i] = ws_tensor("pqk", {n1, n2, kk});
+            if (fast) {
+                eig_small_async(Hm.p, kk, Vt.p, lam, flag);
+                back->pad = nqr;
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 2 * nqr * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(back->lam, lam, kk * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+            } else {
+                std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);
+                spec[2 + i].resize(kk);
+                for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
+            }
             contract(Ten::make(Qi.p, "pqz", {n1, n2, kk}), Vt, U[i]);
+        };
+        bool iso_done[4] = {false, false, false, false};
+        if (kk <= 64 && q + 1 <= 8 && n12 >= 16LL * kk) {   // the four isometries as concurrent chains
+            Fork fk(4);
+            for (int i = 0; i < 4; ++i) {
+                fk.enter(i);
+                iso_body(i, true, reinterpret_cast<IsoBack *>(fk.pinned(i)));
+                fk.leave();
+            }
+            for (int i = 0; i < 4; ++i) {
+                fk.sync(i);
+                const IsoBack *bk = reinterpret_cast<IsoBack *>(fk.pinned(i));
+                bool ok = bk->flag == 0;
+                for (int j = 0; j < bk->pad; ++j) ok = ok && bk->ratio[2 * j] > 1e-5 * bk->ratio[2 * j + 1];
+                if (!ok) continue;   // ill conditioned block or no convergence: redone below
+                spec[2 + i].resize(kk);
+                for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(bk->lam[j], 0.0));
+                iso_done[i] = true;
+            }
+            fk.join();
         }
+        for (int i = 0; i < 4; ++i)
+            if (!iso_done[i]) {
+                size_t mk = ws_mark();
+                iso_body(i, false, nullptr);
+                ws_release(mk);
+            }
     }
     kd = U[0].legs[2].n;
     stage_mark(3);
@@ -807,22 +978,81 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten Ms[3], Ns[3];
     int kq[3];
     for (int mu = 0; mu < 3; ++mu) {
-        const int N2 = (int)(nn[mu] * nn[mu]);
+        const long long N2 = nn[mu] * nn[mu];
         Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
         Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
+    }
+    // gauge (reading G12) P = N G_ref, then M W and W^T N into the step's squeezer buffers
+    auto finish = [&](int mu, const Ten &Mr, const Ten &Nr, const std::vector<double> &sh, int k) {
+        const long long N2 = nn[mu] * nn[mu];
+        kq[mu] = k;
+        spec[6 + mu].assign(sh.begin(), sh.begin() + k);
+        Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
+        Ten Pq = ws_tensor("kb", {k, k});
+        contract(Nr, rf, Pq);
+        Ten Wq = gauge_rotation(Pq.as("ab"), sh, k);
+        Ms[mu] = Ten::make(Ms[mu].p, "uok", {nn[mu], nn[mu], k});
+        Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
+        contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
+        contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
+    };
+    bool done[3] = {false, false, false};
+    {   // the three subspace-iteration squeezers as concurrent chains (large legs only)
+        SqChain ch[3];
+        int nact = 0;
+        for (int mu = 0; mu < 3; ++mu) {
+            const long long N2 = nn[mu] * nn[mu];
+            ch[mu].active = N2 >= 256 && chi < SqChain::b;
+            ch[mu].GLm = GL[mu];
+            ch[mu].GRm = GR[mu];
+            ch[mu].N2 = (int)N2;
+            ch[mu].chi = chi;
+            ch[mu].mu = mu;
+            nact += ch[mu].active;
+        }
+        if (nact > 0) {
+            Fork fk(3);
+            for (int mu = 0; mu < 3; ++mu)
+                if (ch[mu].active) {
+                    fk.enter(mu);
+                    ch[mu].phaseA(fk.pinned(mu));
+                    fk.leave();
+                }
+            for (int mu = 0; mu < 3; ++mu)
+                if (ch[mu].active) {
+                    fk.sync(mu);
+                    ch[mu].ok = ch[mu].plan();
+                }
+            for (int mu = 0; mu < 3; ++mu)
+                if (ch[mu].ok) {
+                    fk.enter(mu);
+                    ch[mu].phaseB();
+                    fk.leave();
+                }
+            for (int mu = 0; mu < 3; ++mu)
+                if (ch[mu].ok) {
+                    fk.sync(mu);
+                    fk.enter(mu);
+                    if (ch[mu].phaseC()) {
+                        gaps[1 + mu] = ch[mu].gap;
+                        finish(mu, ch[mu].Mr, ch[mu].Nr, ch[mu].sh, ch[mu].k);
+                        done[mu] = true;
+                    }
+                    fk.leave();
+                }
+            fk.join();
+        }
+    }
+    for (int mu = 0; mu < 3; ++mu) {
+        if (done[mu]) continue;
+        // dense route = the oracle's algorithm: eigendecompositions of both Grams, SVD of R1 R2
+        const int N2 = (int)(nn[mu] * nn[mu]);
         size_t mk = ws_mark();
         Ten Mr, Nr;
         std::vector<double> sh;
         double *sf;
         int k;
-        SqueezeOut so;
-        if (squeezer_subspace(GL[mu], GR[mu], N2, chi, mu, Mr, Nr, so)) {
-            k = so.k;
-            sh = so.s;
-            sf = so.s_dev;
-            gaps[1 + mu] = so.gap;
-        } else {
-            ws_release(mk);
+        {
             Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
             double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
             std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
@@ -855,17 +1085,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
             scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
         }
-        kq[mu] = k;
-        spec[6 + mu].assign(sh.begin(), sh.begin() + k);
-        // gauge (reading G12): P = N G_ref
-        Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
-        Ten Pq = ws_tensor("kb", {k, k});
-        contract(Nr, rf, Pq);
-        Ten Wq = gauge_rotation(Pq.as("ab"), sh, k);
-        Ms[mu] = Ten::make(Ms[mu].p, "uok", {nn[mu], nn[mu], k});
-        Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
-        contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
-        contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
+        finish(mu, Mr, Nr, sh, k);
         ws_release(mk);
     }
     stage_mark(6);

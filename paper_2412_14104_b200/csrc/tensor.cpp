@@ -2,7 +2,9 @@
 // (batch, rows, columns, summed), orders them by the operand's memory stride (so that the
 // kernel's loader walks the contiguous leg), merges legs that are adjacent in every tensor
 // involved, and emits the mixed-radix maps of one tensor_gemm launch.
-#include "tensor.h"
+#include "ctx.h"
+
+#include <chrono>
 
 #include <algorithm>
 #include <string.h>
@@ -178,7 +180,11 @@ void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accum
     long long bn0 = gn.empty() ? (1LL << 60) : gn[0].s[0];
     long long bk0 = gk.empty() ? (1LL << 60) : gk[0].s[1];
     p.b_kfast = bk0 < bn0;
+    const auto t0 = std::chrono::steady_clock::now();
     tensor_gemm(p);
+    Ctx &c = ctx();
+    c.host_contract_s += std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    c.host_contract_n += 1;
 }
 
 }  // namespace tatrg
