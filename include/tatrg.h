@@ -67,7 +67,9 @@ double log_Z_per_site(void);
 /* ---- plumbing (PyTorch owns memory and streams) ------------------------------------- */
 int tatrg_set_stream(void *cuda_stream);                     /* cudaStream_t; NULL = default */
 int tatrg_set_workspace(void *dev_ptr, size_t bytes);        /* device; 256-byte aligned */
-size_t tatrg_workspace_bytes(int chi, int r);                /* upper bound, steady state */
+size_t tatrg_workspace_bytes(int chi, int r);                /* upper bound, steady state, coarse_grain */
+size_t tatrg_workspace_bytes_atrg(int chi, int r);           /* the same for coarse_grain_atrg (adds the
+                                                              * chi^6-sized slices of the O(chi^9) contraction) */
 
 /* Caller-supplied Gaussian inputs for the NEXT coarse_grain call (consumed by it).
  * which: 0 swap sketch [(beta,J), l]; 1..4 isometry sketches A,X,Y,D [(p,q), k];

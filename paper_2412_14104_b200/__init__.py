@@ -18,7 +18,8 @@ _SO = os.path.join(_HERE, "libtatrg.so")
 
 EXPORTS = [
     "init_ising_tensor", "coarse_grain", "coarse_grain_atrg", "log_Z_per_site",
-    "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_peak",
+    "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_bytes_atrg",
+    "tatrg_workspace_peak",
     "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
@@ -56,6 +57,7 @@ def lib():
             "tatrg_set_stream": (c_i, [c_vp]),
             "tatrg_set_workspace": (c_i, [c_vp, c_sz]),
             "tatrg_workspace_bytes": (c_sz, [c_i, c_i]),
+            "tatrg_workspace_bytes_atrg": (c_sz, [c_i, c_i]),
             "tatrg_workspace_peak": (c_sz, []),
             "tatrg_set_sketch": (c_i, [c_i, c_vp, c_sz, c_i]),
             "tatrg_sketch_shape": (c_i, [c_i, c_i, c_i, c_i, ctypes.POINTER(c_i64), ctypes.POINTER(c_i64)]),

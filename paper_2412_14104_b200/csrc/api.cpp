@@ -1,6 +1,8 @@
 // api.cpp -- the C-ABI of libtatrg (include/tatrg.h): argument checking, the process-global
 // context, the caller-owned workspace (bump allocator), error reporting.
 #include <math.h>
+
+#include <algorithm>
 #include <stdarg.h>
 #include <string.h>
 
@@ -224,16 +226,32 @@ int tatrg_set_workspace(void *dev_ptr, size_t bytes)
     return TATRG_OK;
 }
 
+static double workspace_doubles(int chi, int r)
+{
+    // steady state, all legs = chi, in units of u = chi^5 doubles: two generations of the state (4 u),
+    // A, D (2 u), X sigma, Y (2 u), Y sigma (1 u) persist.  The largest transient sits on top of the first
+    // 8 u: the reduced bond swap (Q1_A, Q1_D, the r u sketch: 2.5 + r), or, when the reduced operator
+    // does not apply (ill-conditioned matricisation), the plain swap (sketch + two RSVD blocks + copies:
+    // 3.5 r) -- the latter is provisioned only while it costs less than 40 GB; beyond that a plain-swap
+    // fallback in the steady state fails with TATRG_ENOMEM.  The canonical form (3-4 u on 6 u) and the
+    // slabbed contraction (<= 1.1e9 doubles on 9 u) need less.  Plus the chi^4-sized triad / Gram /
+    // squeezer intermediates.
+    const double c5 = pow((double)chi, 5), c4 = pow((double)chi, 4);
+    const double swap_u = (c5 * 3.5 * r * 8.0 < 40e9) ? std::max(3.5 * r, 2.5 + r) : 2.5 + r;
+    return c5 * (8.0 + swap_u) + std::min(c5 * r * (1.0 + r), 1.1e9) + c4 * (12.0 * r * r + 40) + (1 << 23);
+}
+
 size_t tatrg_workspace_bytes(int chi, int r)
 {
     if (chi < 1 || r < 1) return 0;
-    // steady state, all legs = chi: a generous count of the live chi^5-sized tensors
-    // (state x2 generations, Q_Phi, Q_Psi, A, D, X, Y, Xs, Ys, G_ref, sketch + 3 RSVD blocks of
-    // r chi^5, TSQR stacks, P of r^2 chi^5, EM of r chi^5) plus the chi^4-sized Gram intermediates.
-    double c5 = pow((double)chi, 5), c4 = pow((double)chi, 4);
-    double doubles = c5 * (4 + 9 + 5.0 * r + 2.0 * r * r) + c4 * (16.0 * r * r + 64) + (1 << 22) +
-                     2.2 * c4 * chi * chi;   // the chi^6 slices of the plain ATRG contraction
-    return (size_t)(doubles * 8.0 * 1.1) + ((size_t)64 << 20);
+    return (size_t)(workspace_doubles(chi, r) * 8.0 * 1.05) + ((size_t)64 << 20);
+}
+
+size_t tatrg_workspace_bytes_atrg(int chi, int r)
+{
+    if (chi < 1 || r < 1) return 0;
+    const double c6 = pow((double)chi, 6);   // the chi^6 slices of the plain ATRG contraction
+    return (size_t)((workspace_doubles(chi, r) + 2.2 * c6) * 8.0 * 1.05) + ((size_t)64 << 20);
 }
 
 size_t tatrg_workspace_peak(void) { return ctx().peak; }

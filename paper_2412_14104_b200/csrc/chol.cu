@@ -288,6 +288,42 @@ bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full)
     return h == 0;
 }
 
+// out[0], out[1] = min, max of the diagonal of the n x n row-major matrix L (one CTA)
+__global__ void diag_minmax_kernel(const double *__restrict__ L, int n, double *__restrict__ out)
+{
+    __shared__ double lo_s[32], hi_s[32];
+    double lo = INFINITY, hi = -INFINITY;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const double d = L[(long long)i * n + i];
+        lo = fmin(lo, d);
+        hi = fmax(hi, d);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+        hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        lo_s[threadIdx.x >> 5] = lo;
+        hi_s[threadIdx.x >> 5] = hi;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int i = 1; i < (int)(blockDim.x >> 5); ++i) {
+            lo = fmin(lo, lo_s[i]);
+            hi = fmax(hi, hi_s[i]);
+        }
+        out[0] = lo;
+        out[1] = hi;
+    }
+}
+
+void diag_minmax(const double *L, int n, double *out)
+{
+    diag_minmax_kernel<<<1, 256, 0, stream()>>>(L, n, out);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
+
 void near_identity_chol(double *G, int n, double *Linv)
 {
     int blocks = (int)(((long long)n * n + 255) / 256 < 1184 ? ((long long)n * n + 255) / 256 : 1184);

@@ -139,6 +139,7 @@ bool cholesky_lower(double *A, int n, double shift_rel, double *Linv_full = null
 void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full, int *flag_dev);
 // G = I + E, |E| <~ 1e-8: in place lower Cholesky factor and its inverse by the first-order formulas (error O(|E|^2))
 void near_identity_chol(double *G, int n, double *Linv);
+void diag_minmax(const double *L, int n, double *out);   // out[0..1] = min, max of diag(L), L n x n row-major
 void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel = 0.0);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);

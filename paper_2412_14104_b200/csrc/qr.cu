@@ -252,6 +252,27 @@ void tsqr_impl(double *Y, long long m, int n, double *Rout)
 // unique qr+ factorisation as the Householder route whenever it applies.  It applies when the
 // first Cholesky factor exists and its diagonal ratio (a lower bound of cond(Y)) is below 1e5, so
 // that cond^2 eps << 1; otherwise nothing has been written and the caller falls back to TSQR.
+namespace {
+
+// C (n x n row-major, n <= 128) -> its lower Cholesky factor in place (after adding shift_rel * max
+// diag); returns L^-1 as a [d][c] view; mm (optional) receives min / max of diag(L).  Asynchronous.
+Ten chol_inv(Ten &C, int n, double shift_rel, int *flag, double *mm)
+{
+    if (n <= 64) {
+        double *Li = ws_doubles(64 * 64);
+        chol_block(C.p, n, n, Li, flag, mm, shift_rel);
+        Ten L = Ten::make(Li, "dc", {n, 64});
+        L.legs[1].n = n;
+        return L;
+    }
+    double *Li = ws_doubles((long long)n * n);
+    cholesky_lower_async(C.p, n, shift_rel, Li, flag);
+    if (mm) diag_minmax(C.p, n, mm);
+    return Ten::make(Li, "dc", {n, n});
+}
+
+}  // namespace
+
 bool cholqr2(double *Y, long long m, int n, double *Rout)
 {
     size_t mark = ws_mark();
@@ -260,9 +281,8 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
     TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten C1 = ws_tensor("cd", {n, n}), C2 = ws_tensor("cd", {n, n});
-    double *Li1 = ws_doubles(64 * 64), *Li2 = ws_doubles(64 * 64);
     contract(Ym, Ym.as("rd"), C1);
-    chol_block(C1.p, n, n, Li1, flag, mm);
+    Ten L1i = chol_inv(C1, n, 0.0, flag, mm);   // row d of L^-1; Q[r,d] = sum_c Y[r,c] Linv[d,c]
     struct {
         int f;
         double lo, hi;
@@ -275,13 +295,9 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
         return false;
     }
     Ten T = ws_tensor("rd", {m, n});
-    Ten L1i = Ten::make(Li1, "dc", {n, 64});   // row d of L^-1; Q[r,d] = sum_c Y[r,c] Linv[d,c]
-    L1i.legs[1].n = n;
     contract(Ym, L1i, T);
     contract(T.as("rc"), T, C2);
-    chol_block(C2.p, n, n, Li2, flag, nullptr);
-    Ten L2i = Ten::make(Li2, "dc", {n, 64});
-    L2i.legs[1].n = n;
+    Ten L2i = chol_inv(C2, n, 0.0, flag, nullptr);
     contract(T.as("rc"), L2i, Ym.as("rd"));
     // R = L2^T L1^T : R[i][j] = sum_k L2[k][i] L1[j][k]   (C1, C2 now hold L1, L2; upper parts zeroed)
     contract(C2.as("ki"), C1.as("jk"), Ten::make(Rout, "ij", {n, n}));
@@ -295,20 +311,17 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
                   double *Rout)
 {
-    if (n < 1 || n > 64 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
+    if (n < 1 || n > 128 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
     size_t mark = ws_mark();
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten T = ws_tensor("rd", {m, n});
     Ten C[3];
-    double *Li = ws_doubles(64 * 64);
     Ten cur = Ym, nxt = T;
     for (int p = 0; p < passes; ++p) {
         C[p] = ws_tensor("cd", {n, n});
         contract(cur.as("rc"), cur.as("rd"), C[p]);
-        chol_block(C[p].p, n, n, Li, flag_dev, p == 0 ? ratio_dev : nullptr, p == 0 ? shift_rel : 0.0);
-        Ten Linv = Ten::make(Li, "dc", {n, 64});   // Q[r,d] = sum_c Y[r,c] Linv[d,c]
-        Linv.legs[1].n = n;
-        contract(cur.as("rc"), Linv, nxt.as("rd"));
+        Ten Linv = chol_inv(C[p], n, p == 0 ? shift_rel : 0.0, flag_dev, p == 0 ? ratio_dev : nullptr);
+        contract(cur.as("rc"), Linv, nxt.as("rd"));       // Q[r,d] = sum_c Y[r,c] Linv[d,c]
         std::swap(cur, nxt);
     }
     if (cur.p != Y) TATRG_CUDA_CHECK(cudaMemcpyAsync(Y, cur.p, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, stream()));
@@ -328,12 +341,48 @@ void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, i
     ws_release(mark);
 }
 
+namespace {
+
+// n > 64: block Gram-Schmidt with reorthogonalisation over two column halves of at most 64 columns,
+// each factored by tsqr (the robust route for blocks that are not tall or too ill conditioned for
+// Cholesky-QR): Y = [Q1 Q2] [[R11, R12], [0, R22]].
+void tsqr_split(double *Y, long long m, int n, double *Rout)
+{
+    size_t mark = ws_mark();
+    const int h1 = n / 2, h2 = n - h1;
+    Ten Y1 = ws_tensor("rc", {m, h1}), Y2 = ws_tensor("rd", {m, h2});
+    const size_t pitch = sizeof(double) * n;
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y1.p, sizeof(double) * h1, Y, pitch, sizeof(double) * h1, m, cudaMemcpyDeviceToDevice, stream()));
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y2.p, sizeof(double) * h2, Y + h1, pitch, sizeof(double) * h2, m, cudaMemcpyDeviceToDevice, stream()));
+    Ten R11 = ws_tensor("ce", {h1, h1}), R22 = ws_tensor("df", {h2, h2});
+    Ten R12 = ws_tensor("cd", {h1, h2}), Rb = ws_tensor("ed", {h1, h2}), Id = ws_tensor("ce", {h1, h1});
+    tsqr(Y1.p, m, h1, R11.p);
+    contract(Y1, Y2, R12);                       // R12 = Q1^T Y2
+    contract(Y1, R12, Y2, -1.0, true);           // Y2 -= Q1 R12
+    contract(Y1.as("re"), Y2, Rb);               // second pass
+    contract(Y1.as("re"), Rb, Y2, -1.0, true);
+    fill_identity(Id.p, h1);
+    contract(Id, Rb, R12, 1.0, true);            // R12 += Rb
+    tsqr(Y2.p, m, h2, R22.p);
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y, pitch, Y1.p, sizeof(double) * h1, sizeof(double) * h1, m, cudaMemcpyDeviceToDevice, stream()));
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y + h1, pitch, Y2.p, sizeof(double) * h2, sizeof(double) * h2, m, cudaMemcpyDeviceToDevice, stream()));
+    fill_zero(Rout, (long long)n * n);
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Rout, pitch, R11.p, sizeof(double) * h1, sizeof(double) * h1, h1, cudaMemcpyDeviceToDevice, stream()));
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Rout + h1, pitch, R12.p, sizeof(double) * h2, sizeof(double) * h2, h1, cudaMemcpyDeviceToDevice, stream()));
+    TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Rout + (long long)h1 * n + h1, pitch, R22.p, sizeof(double) * h2, sizeof(double) * h2, h2, cudaMemcpyDeviceToDevice, stream()));
+    ws_release(mark);
+}
+
+}  // namespace
+
 void tsqr(double *Y, long long m, int n, double *Rout)
 {
     if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");
-    if (n <= 64 && m >= 16LL * n && m >= 512 && cholqr2(Y, m, n, Rout)) return;
-    if (n > 64) fail(-22, "tsqr: n = %d > 64 not supported yet", n);
-    if (n > 32)
+    if (n > 128) fail(-22, "tsqr: n = %d > 128 not supported", n);
+    if (m >= 16LL * n && m >= 512 && cholqr2(Y, m, n, Rout)) return;
+    if (n > 64)
+        tsqr_split(Y, m, n, Rout);
+    else if (n > 32)
         tsqr_impl<64>(Y, m, n, Rout);
     else if (n > 16)
         tsqr_impl<32>(Y, m, n, Rout);

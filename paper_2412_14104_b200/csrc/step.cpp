@@ -294,12 +294,12 @@ Ten solver_start_block(long long rows, long long cols, int tag, const char *name
 // after synchronising the chain's stream), so that the three squeezers of a step run concurrently
 // on three streams (Fork).
 struct SqChain {
-    static constexpr int b = 64;
+    int b = 64;            // block width of the subspace iteration (> chi): 64, or 128 for chi >= 64
     struct Back {          // page-locked read-back
         int flag;
         int pad;
         double ratio[4];
-        double s[b];
+        double s[128];
     };
     Ten GLm, GRm;
     int N2 = 0, chi = 0, mu = 0;
@@ -328,7 +328,10 @@ struct SqChain {
     {
         mulFt(Q, Qt);
         cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
-        svd_small_async(Rb, b, b, V, sv, flag);
+        if (b <= 64)
+            svd_small_async(Rb, b, b, V, sv, flag);
+        else
+            jacobi_svd(Rb, b, b, V, sv, 1, 0, 0, 0);       // multi-launch Jacobi (synchronises this chain)
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(back->s, sv, b * sizeof(double), cudaMemcpyDeviceToHost, stream()));
@@ -569,7 +572,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ctx &c = ctx();
     if (!c.inited) fail(-1, "coarse_grain: call init_ising_tensor first");
     if (direction < 1 || direction > 4 || chi < 1 || r < 1 || q < 0) fail(-22, "coarse_grain: bad arguments");
-    if ((long long)r * chi > 64) fail(-22, "coarse_grain: r*chi = %d > 64 not supported yet", r * chi);
+    if ((long long)r * chi > 128 || chi > 64) fail(-22, "coarse_grain: r*chi = %d > 128 (or chi > 64) not supported", r * chi);
     StepCfg cfg{seed, c.step};
     c.prof_rec.clear();
 
@@ -617,6 +620,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
 
     stage_mark(0);
     // =================== O2 canonical form ===================
+    // A, D and sigma^T outlive this stage; everything else of it (the chi^5-sized Q factors included)
+    // is released once A and D are formed
+    double *Abuf = ws_doubles(R * g0), *Dbuf = ws_doubles(R * g0);
+    double *sT = ws_doubles(g0);
+    const size_t canon_mark = ws_mark();
     Ten Qp = ws_tensor("rg", {R, g0}), Qs = ws_tensor("rg", {R, g0});
     d2d(Qp.p, c.phi, R * g0);
     d2d(Qs.p, c.psi, R * g0);
@@ -627,7 +635,6 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten Cm = ws_tensor("hg", {g0, g0});
     contract(Rs, Rp, Cm);
     Ten Vc = ws_tensor("ah", {g0, g0});    // rows = right singular vectors v_a[h]
-    double *sT = ws_doubles(g0);
     jacobi_svd(Cm.p, g0, g0, Vc.p, sT, 1, 0, 0, 0);   // C V = U diag(sT); Cm rows -> u_a[g] sT_a
     spec[0] = d2h(sT, g0);
     const int a = num_rank(spec[0], -1);
@@ -648,9 +655,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten u2 = ws_tensor("bg", {a, g0}), v2 = ws_tensor("bg", {a, g0});
     contract(Wg, u, u2);                    // u2[b][g] = sum_a W[a,b] u[a][g]
     contract(Wg, v.as("ag"), v2);
-    Ten A = ws_tensor("xpqta", {n0, n1, n2, n3, a}), D = ws_tensor("xpqta", {n0, n1, n2, n3, a});
+    Ten A = Ten::make(Abuf, "xpqta", {n0, n1, n2, n3, a}), D = Ten::make(Dbuf, "xpqta", {n0, n1, n2, n3, a});
     contract(QpR.as("xpqtg"), u2.as("ag"), A);
     contract(QsR.as("xpqtg"), v2.as("ag"), D);
+    ws_release(canon_mark);
     stage_mark(1);
 
     // =================== O3 bond swap (Table 1 row 1) ===================
@@ -749,8 +757,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     }
     Ten X = Ten::make(Xbuf, "apqtg", {a, n1, n2, n3, gs});
     Ten Y = Ten::make(Ybuf, "buvwg", {a, n1, n2, n3, gs});
-    Ten Xs = ws_tensor("apqtg", {a, n1, n2, n3, gs}), Ys = ws_tensor("buvwg", {a, n1, n2, n3, gs});
-    d2d(Xs.p, X.p, X.size());
+    // X enters the rest of the step only as X sigma (Eq. 5): scaled in place; Y is needed both ways
+    Ten Xs = X, Ys = ws_tensor("buvwg", {a, n1, n2, n3, gs});
     d2d(Ys.p, Y.p, Y.size());
     scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
     scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
@@ -1002,7 +1010,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         int nact = 0;
         for (int mu = 0; mu < 3; ++mu) {
             const long long N2 = nn[mu] * nn[mu];
-            ch[mu].active = N2 >= 256 && chi < SqChain::b;
+            ch[mu].b = chi < 64 ? 64 : 128;
+            ch[mu].active = N2 >= 4 * ch[mu].b && chi < ch[mu].b;
             ch[mu].GLm = GL[mu];
             ch[mu].GRm = GR[mu];
             ch[mu].N2 = (int)N2;
@@ -1118,18 +1127,31 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(U[3].as("PQl"), Ns[1].as("nqQ"), V2);
         }
         contract(W1, V2, Qt);
-        Ten EM = ws_tensor("xkaTw", {n0, kd, a, n3, m3});
-        Ten Pt = ws_tensor("xkwlg", {n0, kd, m3, kd, gs});
-        Ten out = new_view(side == 0 ? phi_new : psi_new);
-        if (side == 0) {
-            contract(E.as("xkta"), Ms[2].as("tTw"), EM);
-            contract(EM, F.as("alTg"), Pt);
-            contract(Pt, Qt, out.as("xmnwg"));
-        } else {
-            // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
-            contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkatw"));
-            contract(EM.as("xkatw"), G.as("altg"), Pt);   // Pt[x, kD, w, kY, g]
-            contract(Pt.as("xlwkg"), Qt, out.as("xmnwg"));
+        // (i)-(ii)-(iv) of Eqs. 13-14 in slabs of the direction-0 leg so that E M^(4) (r chi^5) and
+        // P (r^2 chi^5) stay below ~8 GB (one slab = the whole tensor up to chi ~ 40)
+        const double per_x = 8.0 * ((double)kd * a * n3 * m3 + (double)kd * m3 * kd * gs);
+        const long long xc = std::max<long long>(1, std::min<long long>(n0, (long long)(8.0e9 / per_x)));
+        Ten EM = ws_tensor("xkaTw", {xc, kd, a, n3, m3});
+        Ten Pt = ws_tensor("xkwlg", {xc, kd, m3, kd, gs});
+        Ten out = new_view(side == 0 ? phi_new : psi_new).as("xmnwg");
+        auto slab = [](Ten t, long long x0, long long cnt) {   // legs[0] is the direction-0 leg
+            t.p += x0 * t.legs[0].stride;
+            t.legs[0].n = cnt;
+            return t;
+        };
+        for (long long x0 = 0; x0 < n0; x0 += xc) {
+            const long long cnt = std::min(xc, n0 - x0);
+            Ten EMs = slab(EM, 0, cnt), Pts = slab(Pt, 0, cnt), outs = slab(out, x0, cnt);
+            if (side == 0) {
+                contract(slab(E.as("xkta"), x0, cnt), Ms[2].as("tTw"), EMs);
+                contract(EMs, F.as("alTg"), Pts);
+                contract(Pts, Qt, outs);
+            } else {
+                // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
+                contract(slab(H.as("xkTa"), x0, cnt), Ns[2].as("wtT"), EMs.as("xkatw"));
+                contract(EMs.as("xkatw"), G.as("altg"), Pts);   // Pt[x, kD, w, kY, g]
+                contract(Pts.as("xlwkg"), Qt, outs);
+            }
         }
         ws_release(mk);
     }

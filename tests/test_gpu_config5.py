@@ -1,0 +1,64 @@
+"""BASELINE.json configs[4] (T=6.5, h=0.01, chi=64, r=2, q=3): the largest sizes the library takes
+(r*chi = 128 sketch columns, 128-wide squeezer blocks, chi^5 = 8.6 GB tensors).
+
+The oracle cannot follow this config into its steady state (one step is ~4.6e14 flop), so parity is
+checked element by element on the first four steps (legs 2 -> 4 -> 16 -> 64; the fourth already runs
+the 128-column RSVD, the reduced bond swap and 16x16-leg squeezers), and the first step with all
+legs = 64 (workspace ~135 GB, chi^9-free O(r^2 chi^7) contraction in slabs) is checked through
+properties that hold at any size: unit-norm state, dims, descending positive spectra, and a free
+energy that agrees with the chi = 32 run of the same lattice to truncation level."""
+import numpy as np
+import pytest
+
+from oracle import driver
+from oracle import tatrg_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+BETA, H, CHI, R, Q, SEED = 1 / 6.5, 0.01, 64, 2, 3, 20241218
+
+
+def test_config5_first_steps_parity_then_full_size_step():
+    import torch
+    import paper_2412_14104_b200 as tt
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    free, _ = torch.cuda.mem_get_info()
+    need = tt.workspace_bytes(CHI, R)
+    full = free > need + (4 << 30)
+    tt.set_workspace(nbytes=need if full else 8 << 30)
+    tt.set_stream()
+    try:
+        st = orc.init_ising_tensor(BETA, H)
+        tt.init_ising_tensor(BETA, H)
+        for m in range(4):
+            rec = orc.coarse_grain(st, m + 1, CHI, R, Q, driver.seeded_inputs_for(SEED, m))
+            tt.coarse_grain(m + 1, CHI, R, Q, SEED)
+            assert tuple(st.dims) == tuple(tt.get_dims()[:5])
+            lo, lg = orc.log_Z_per_site(st), tt.log_Z_per_site()
+            assert abs(lg / lo - 1) <= 1e-10, (m, lg, lo)
+            for name in ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3"):
+                so = np.asarray(rec[name]) if name in rec else np.zeros(0)
+                sg = tt.get_spectrum(name)
+                assert len(so) == len(sg), (m, name, len(so), len(sg))
+                if len(so):
+                    assert np.abs(so - sg).max() <= 1e-9 * so[0], (m, name)
+        assert tuple(tt.get_dims()[:5]) == (64, 64, 64, 64, 64)
+        if not full:
+            pytest.skip("not enough free device memory for the chi = 64 steady-state workspace")
+        lnz4 = tt.log_Z_per_site()
+        tt.coarse_grain(1, CHI, R, Q, SEED)      # all legs = 64
+        assert tuple(tt.get_dims()[:5]) == (64, 64, 64, 64, 64)
+        lnz5 = tt.log_Z_per_site()
+        assert np.isfinite(lnz5) and 0.5 < lnz5 < lnz4      # ln Z / V decreases towards its bulk value
+        for name in ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3"):
+            s = tt.get_spectrum(name)
+            assert len(s) in (64, 128) and np.all(s > 0) and np.all(np.diff(s) <= 1e-12 * s[0]), name
+        # the same five steps at chi = 32: the free energies agree to the truncation level this early
+        # stage has (the oracle's own values for chi = 12, 16, 24 at this point scatter by 1-2.5e-3)
+        tt.init_ising_tensor(BETA, H)
+        for m in range(5):
+            tt.coarse_grain(m % 4 + 1, 32, R, 2, SEED)
+        assert abs(tt.log_Z_per_site() / lnz5 - 1) < 1e-2
+    finally:
+        tt.destroy()
