@@ -118,9 +118,10 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------ inputs
-def pinned_sketches(tt, cfg, step_index, direction):
+def pinned_sketches(tt, cfg, step_index, direction, reuse=None):
     """Host (pinned) seeded Gaussian sketches of one step: {which: torch tensor}; shapes asked from
-    the library for the current state (rows, cols per DESIGN.md 'Input recipe')."""
+    the library for the current state (rows, cols per DESIGN.md 'Input recipe').  reuse: buffers of a
+    previous call to fill again (large configs)."""
     import torch
     import seeded_inputs as si
     out = {}
@@ -128,14 +129,21 @@ def pinned_sketches(tt, cfg, step_index, direction):
         rows, cols = tt.sketch_shape(which, direction, cfg["chi"], cfg["r"])
         if rows * cols == 0:
             continue
-        t = torch.empty(rows * cols, dtype=torch.float64, pin_memory=True)
+        if reuse is not None and which in reuse and reuse[which].numel() == rows * cols:
+            t = reuse[which]
+        else:
+            t = torch.empty(rows * cols, dtype=torch.float64, pin_memory=True)
         si.gauss(si.subseed(cfg["seed"], step_index, which), rows * cols, out=t.numpy())
         out[which] = t
     return out
 
 
+_REF_CACHE = {}
+
+
 def gauge_refs(tt, cfg, direction):
-    """Step-independent gauge reference matrices (reading G12), device resident."""
+    """Step-independent gauge reference matrices (reading G12), device resident.  They depend on
+    (seed, which, shape) only, so directions with equal shapes share one tensor."""
     import torch
     import seeded_inputs as si
     out = {}
@@ -143,8 +151,10 @@ def gauge_refs(tt, cfg, direction):
         rows, cols = tt.sketch_shape(which, direction, cfg["chi"], cfg["r"])
         if rows * cols == 0:
             continue
-        t = torch.from_numpy(si.gauss(si.subseed(cfg["seed"], 0, which), rows * cols))
-        out[which] = t.cuda()
+        key = (cfg["seed"], which, rows, cols)
+        if key not in _REF_CACHE:
+            _REF_CACHE[key] = torch.from_numpy(si.gauss(si.subseed(cfg["seed"], 0, which), rows * cols)).cuda()
+        out[which] = _REF_CACHE[key]
     return out
 
 
@@ -249,6 +259,8 @@ def run_ours(args, cfg, name):
     tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
     m = 0
     for _ in range(cfg["ramp"]):                       # untimed ramp-up to the steady state
+        for which, t in gauge_refs(tt, cfg, m % 4 + 1).items():
+            tt.set_sketch(which, t)
         tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
         m += 1
     dims = tt.get_dims()
@@ -262,28 +274,56 @@ def run_ours(args, cfg, name):
         for which, t in refs[d].items():
             tt.set_sketch(which, t)
 
-    # ---- pass 1: sketches resident in HBM before the timed region
-    host = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(W + K)]
-    dev = [{w: t.cuda() for w, t in sk.items()} for sk in host]
-    torch.cuda.synchronize()
+    # ---- pass 1: sketches resident in HBM before the timed region.  Small configs: all W + K steps
+    # sketches are uploaded first and one event pair brackets the K steps.  Large configs (chi = 64: 17 GB
+    # of sketch per step): one device buffer set, refilled between steps outside the per-step event
+    # pairs, whose times are summed.
+    per_step_bytes = sum(a * b * 8 for a, b in (tt.sketch_shape(w, 1, chi, r) for w in range(5)))
+    streamed = per_step_bytes * (W + K) > (20 << 30)
+    if streamed:
+        host = pinned_sketches(tt, cfg, m, m % 4 + 1)
+        dev1 = {w: torch.empty_like(t, device="cuda") for w, t in host.items()}
+
+        def inputs_for(i):
+            pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1, reuse=host)
+            for w, t in host.items():
+                dev1[w].copy_(t)
+            torch.cuda.synchronize()
+            return dev1
+    else:
+        hosts = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(W + K)]
+        dev = [{w: t.cuda() for w, t in sk.items()} for sk in hosts]
+        torch.cuda.synchronize()
+
+        def inputs_for(i):
+            return dev[i]
     for i in range(W):
-        set_inputs(dev[i], (m + i) % 4 + 1)
+        set_inputs(inputs_for(i), (m + i) % 4 + 1)
         tt.coarse_grain((m + i) % 4 + 1, chi, r, q, seed)
     tt.set_profile(2 if args.profile_all else 1)
     tt.launch_count(reset=True)
     tt.gemm_flops(reset=True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     vis = os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")
     sampler = ClockSampler(vis[local] if local < len(vis) and vis[local].strip().isdigit() else local)
     stages = {}
     gprof = {}
+    pairs = []
     barrier()
     sampler.start()
-    e0.record(stream)
+    if not streamed:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        pairs.append((e0, e1))
     for i in range(W, W + K):
         d = (m + i) % 4 + 1
-        set_inputs(dev[i], d)
+        sk = inputs_for(i)
+        if streamed:
+            pairs.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
+            pairs[-1][0].record(stream)
+        set_inputs(sk, d)
         tt.coarse_grain(d, chi, r, q, seed)
+        if streamed:
+            pairs[-1][1].record(stream)
         for k, v in tt.stage_ms().items():
             stages[k] = stages.get(k, 0.0) + v / K
         for k, v in tt.gemm_profile().items():
@@ -292,34 +332,56 @@ def run_ours(args, cfg, name):
                 g["ms"][j] += v["ms"][j]
                 g["flops"][j] += v["flops"][j]
                 g["launches"][j] += v["launches"][j]
-    e1.record(stream)
+    if not streamed:
+        pairs[0][1].record(stream)
     barrier()
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
+    ms = sum(a.elapsed_time(b) for a, b in pairs)
     launches = tt.launch_count(reset=True)
     flops = tt.gemm_flops(reset=True)
     tt.set_profile(False)
     m += W + K
     lnz = tt.log_Z_per_site()
-    del dev
+    if streamed:
+        del dev1
+    else:
+        del dev
+        hosts = None
     torch.cuda.empty_cache()
 
     # ---- pass 2: end to end through the C-ABI with host sketch buffers + ln Z read-back
     Ke = K
     h2d = 0
-    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    host2 = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(Ke)]
-    barrier()
-    e2.record(stream)
-    for i in range(Ke):
-        d = (m + i) % 4 + 1
-        set_inputs(host2[i], d)                      # host pointers: copied inside coarse_grain
-        tt.coarse_grain(d, chi, r, q, seed)
-        lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
-        h2d += sum(t.numel() * 8 for t in host2[i].values())
-    e3.record(stream)
-    barrier()
-    ms_e2e = e2.elapsed_time(e3)
+    pairs2 = []
+    if streamed:
+        barrier()
+        for i in range(Ke):
+            d = (m + i) % 4 + 1
+            pinned_sketches(tt, cfg, m + i, d, reuse=host)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            set_inputs(host, d)                          # host pointers: copied inside coarse_grain
+            tt.coarse_grain(d, chi, r, q, seed)
+            lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
+            b.record(stream)
+            pairs2.append((a, b))
+            h2d += sum(t.numel() * 8 for t in host.values())
+        barrier()
+    else:
+        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        host2 = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(Ke)]
+        barrier()
+        e2.record(stream)
+        for i in range(Ke):
+            d = (m + i) % 4 + 1
+            set_inputs(host2[i], d)                      # host pointers: copied inside coarse_grain
+            tt.coarse_grain(d, chi, r, q, seed)
+            lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
+            h2d += sum(t.numel() * 8 for t in host2[i].values())
+        e3.record(stream)
+        barrier()
+        pairs2.append((e2, e3))
+    ms_e2e = sum(a.elapsed_time(b) for a, b in pairs2)
     m += Ke
 
     # ---- max over ranks
@@ -366,7 +428,9 @@ def run_ours(args, cfg, name):
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload_name(name, cfg), "chi": chi, "r": r, "q": q,
                            "steady_state": steady, "dims": list(dims[:5]),
-                           "l2": "inputs larger than L2 (Phi, Psi, A, D, X, Y are 268 MB each at chi=32)",
+                           "l2": "inputs larger than L2 (Phi, Psi, A, D, X, Y are %.0f MB each)" % (8e-6 * chi ** 5),
+                           "timed_region": ("per-step event pairs summed, sketch refilled between steps"
+                                            if streamed else "one event pair around the K steps"),
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
                 "e2e": {"value": world * Ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke,
                         "d2h_bytes_per_step": 8, "steps": Ke},
