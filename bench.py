@@ -231,6 +231,24 @@ def run_reference(args, cfg, name):
 
 
 # ------------------------------------------------------------------------------ our arm
+def reduce_over_ranks(max_values, sum_values, dist, device):
+    """Replicas only: the job's time is the slowest replica's (MAX over ranks),
+    counters add up.  dist = torch.distributed or None for a single process."""
+    if dist is None:
+        return list(max_values), list(sum_values)
+    import torch
+    t = torch.tensor(list(max_values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([float(v) for v in sum_values], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t], [float(x) for x in u]
+
+
+def job_value(world, steps, ms):
+    """Whole-job steps/s of `world` independent replicas that each did `steps` steps in (max) `ms`."""
+    return world * steps / (ms * 1e-3)
+
+
 def run_ours(args, cfg, name):
     import torch
     import paper_2412_14104_b200 as tt
@@ -385,13 +403,8 @@ def run_ours(args, cfg, name):
     m += Ke
 
     # ---- max over ranks
-    if dist is not None:
-        t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, ms_e2e = float(t[0]), float(t[1])
-        ln = torch.tensor([float(launches)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(ln)
-        launches = int(ln[0])
+    (ms, ms_e2e), (launches,) = reduce_over_ranks([ms, ms_e2e], [launches], dist, "cuda")
+    launches = int(launches)
 
     # ---- roofline of the dominant kernel (tensor-GEMM, 128x128 DMMA tile)
     peaks, how = measured_peaks()
@@ -423,7 +436,7 @@ def run_ours(args, cfg, name):
 
     line = None
     if rank == 0:
-        line = {"metric": METRIC, "value": world * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+        line = {"metric": METRIC, "value": job_value(world, K, ms), "unit": UNIT, "n_gpus": world, "steps": K,
                 "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload_name(name, cfg), "chi": chi, "r": r, "q": q,
@@ -432,7 +445,7 @@ def run_ours(args, cfg, name):
                            "timed_region": ("per-step event pairs summed, sketch refilled between steps"
                                             if streamed else "one event pair around the K steps"),
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
-                "e2e": {"value": world * Ke / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke,
+                "e2e": {"value": job_value(world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke,
                         "d2h_bytes_per_step": 8, "steps": Ke},
                 "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
                 "stages_ms_per_step": stages, "stages_gemm": per_stage, "ln_Z_per_site": lnz}

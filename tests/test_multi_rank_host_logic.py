@@ -1,0 +1,53 @@
+"""N > 1 is "replicas only": no data-path collective exists.  What N > 1 adds is host
+logic in bench.py -- MAX over ranks of the device times, SUM of the counters, whole-job value, rank-0-only
+output of the reference arm -- covered here with world_size 2 over gloo on CPU."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch, torch.distributed as dist
+import bench
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%%s" %% os.environ["PORT"],
+                        rank=int(os.environ["RANK"]), world_size=2)
+rank = dist.get_rank()
+mx, sm = bench.reduce_over_ranks([100.0 + 50.0 * rank, 7.0 - rank], [1000 + rank], dist, "cpu")
+print(json.dumps({"rank": rank, "max": mx, "sum": sm, "value": bench.job_value(2, 8, mx[0])}))
+dist.destroy_process_group()
+""" % ROOT
+
+
+def test_reduce_over_ranks_world2_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    port = str(29500 + os.getpid() % 2000)
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), PORT=port)
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs)
+    for out in outs:
+        d = json.loads(out.strip().splitlines()[-1])
+        assert d["max"] == [150.0, 7.0]          # slowest replica, per quantity
+        assert d["sum"] == [2001.0]
+        assert abs(d["value"] - 2 * 8 / 0.150) < 1e-9
+
+
+def test_single_process_passthrough():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.reduce_over_ranks([3.0, 4.0], [5], None, "cpu") == ([3.0, 4.0], [5])
+    assert bench.job_value(1, 8, 1000.0) == 8.0
+
+
+def test_reference_arm_runs_on_rank0_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                          "--steps", "1", "--warmup", "1"], env=env, capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0 and out.stdout.strip() == ""
