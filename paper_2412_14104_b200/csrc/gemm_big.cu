@@ -23,9 +23,8 @@ namespace tatrg {
 
 namespace {
 
-constexpr int BM = 128, BK = 16, STAGES = 4;
-constexpr int LD_F = BM + 4;   // [k][m] layout
-constexpr int LD_K = BK + 4;   // [m][k] layout
+constexpr int BM = 128;
+constexpr int LD_F = BM + 4;   // [k][m] layout; the [m][k] layout has leading dimension BK + 4
 constexpr int RASTER_W = 12;
 
 __device__ __forceinline__ void cp_async(double *smem_dst, const double *gsrc, int bytes, int vec)
@@ -49,10 +48,11 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
                  : "d"(a), "d"(b));
 }
 
-// Loader of one ROWS x 16 operand tile by NT threads.  KF: k is the contiguous index in global
+// Loader of one ROWS x BK operand tile by NT threads.  KF: k is the contiguous index in global
 // memory.  VEC: 16-byte copies (pairs along the contiguous index), else 8-byte copies.
-template <bool KF, bool VEC, int ROWS, int NT>
+template <bool KF, bool VEC, int ROWS, int NT, int BK>
 struct TileLoader {
+    static constexpr int LD_K = BK + 4;
     static constexpr int W = VEC ? 2 : 1;             // elements per copy
     static constexpr int PER = ROWS * BK / (NT * W);  // copies per thread per tile
     static constexpr int TPR = NT / BK;               // !KF: threads along the free index per k row
@@ -69,7 +69,7 @@ struct TileLoader {
         base = b;
         if (KF) {
             // k pairs (VEC) or singles along the 16-wide k; free index strided over threads
-            constexpr int KT = VEC ? 8 : 16;          // threads along k
+            constexpr int KT = BK / W;                // threads along k
             kl = (t % KT) * (VEC ? 2 : 1);
 #pragma unroll
             for (int j = 0; j < PER; ++j) {
@@ -108,9 +108,10 @@ struct TileLoader {
     }
 };
 
-template <bool A_KF, bool B_KF, bool VEC, int BN, int WN>
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES>
 __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_kernel(const __grid_constant__ GemmParams p)
 {
+    constexpr int LD_K = BK + 4;
     constexpr int NT = 128 * BN / WN;                 // (BM / 32) * (BN / WN) warps
     constexpr int LD_FB = BN + 4;                     // [k][n] layout of the B tile
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
@@ -136,15 +137,16 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
     const int split = bz / p.batch;
     bz -= split * p.batch;
 
-    int kt0 = 0, kt1 = (p.K + BK - 1) / BK;
+    // this CTA's range of the summed index (split-K ranges are given in units of 16)
+    int k_begin = 0, k_end = p.K;
     if (p.ksplit > 1) {
-        kt0 = split * p.ktiles_per_split;
-        kt1 = min(kt1, kt0 + p.ktiles_per_split);
+        k_begin = min(p.K, split * p.ktiles_per_split * 16);
+        k_end = min(p.K, k_begin + p.ktiles_per_split * 16);
     }
-    const int nkt = max(kt1 - kt0, 0);
+    const int nkt = (k_end - k_begin + BK - 1) / BK;
 
-    TileLoader<A_KF, VEC, BM, NT> la;
-    TileLoader<B_KF, VEC, BN, NT> lb;
+    TileLoader<A_KF, VEC, BM, NT, BK> la;
+    TileLoader<B_KF, VEC, BN, NT, BK> lb;
     la.init(p.A + map_off(p.ab, bz), p.am, m0, p.M, t);
     lb.init(p.B + map_off(p.bb, bz), p.bn, n0, p.N, t);
 
@@ -167,8 +169,8 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
 #pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
         if (s < nkt) {
-            la.load(As + s * A_STAGE, p.ak, (kt0 + s) * BK, p.K);
-            lb.load(Bs + s * B_STAGE, p.bk, (kt0 + s) * BK, p.K);
+            la.load(As + s * A_STAGE, p.ak, k_begin + s * BK, k_end);
+            lb.load(Bs + s * B_STAGE, p.bk, k_begin + s * BK, k_end);
         }
         cp_async_commit();
     }
@@ -178,8 +180,8 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
         {
             const int nx = it + STAGES - 1;
             if (nx < nkt) {
-                la.load(As + (nx % STAGES) * A_STAGE, p.ak, (kt0 + nx) * BK, p.K);
-                lb.load(Bs + (nx % STAGES) * B_STAGE, p.bk, (kt0 + nx) * BK, p.K);
+                la.load(As + (nx % STAGES) * A_STAGE, p.ak, k_begin + nx * BK, k_end);
+                lb.load(Bs + (nx % STAGES) * B_STAGE, p.bk, k_begin + nx * BK, k_end);
             }
             cp_async_commit();
         }
@@ -249,15 +251,16 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
     }
 }
 
-template <bool A_KF, bool B_KF, bool VEC, int BN, int WN>
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES>
 void launch_big(const GemmParams &p_in)
 {
     constexpr int NT = 128 * BN / WN;
+    constexpr int LD_K = BK + 4;
     constexpr int A_STAGE = A_KF ? BM * LD_K : BK * LD_F;
     constexpr int B_STAGE = B_KF ? BN * LD_K : BK * (BN + 4);
     constexpr size_t smem = (size_t)STAGES * (A_STAGE + B_STAGE) * sizeof(double);
     static bool attr_done = false;
-    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN, WN>;
+    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN, WN, BK, STAGES>;
     if (!attr_done) {
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
@@ -288,7 +291,7 @@ bool vec_ok(const double *base, const Map4 &fast, const Map4 &slow, const Map4 &
            all_even(batch);
 }
 
-template <int BN, int WN>
+template <int BN, int WN, int BK, int STAGES>
 void dispatch_big(const GemmParams &p)
 {
     const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;
@@ -297,14 +300,14 @@ void dispatch_big(const GemmParams &p)
     const bool vec = va && vb;
     if (akf) {
         if (bkf)
-            vec ? launch_big<true, true, true, BN, WN>(p) : launch_big<true, true, false, BN, WN>(p);
+            vec ? launch_big<true, true, true, BN, WN, BK, STAGES>(p) : launch_big<true, true, false, BN, WN, BK, STAGES>(p);
         else
-            vec ? launch_big<true, false, true, BN, WN>(p) : launch_big<true, false, false, BN, WN>(p);
+            vec ? launch_big<true, false, true, BN, WN, BK, STAGES>(p) : launch_big<true, false, false, BN, WN, BK, STAGES>(p);
     } else {
         if (bkf)
-            vec ? launch_big<false, true, true, BN, WN>(p) : launch_big<false, true, false, BN, WN>(p);
+            vec ? launch_big<false, true, true, BN, WN, BK, STAGES>(p) : launch_big<false, true, false, BN, WN, BK, STAGES>(p);
         else
-            vec ? launch_big<false, false, true, BN, WN>(p) : launch_big<false, false, false, BN, WN>(p);
+            vec ? launch_big<false, false, true, BN, WN, BK, STAGES>(p) : launch_big<false, false, false, BN, WN, BK, STAGES>(p);
     }
 }
 
@@ -316,12 +319,15 @@ void tensor_gemm_big(const GemmParams &p, int bn)
     // (four warps per scheduler keep the DMMA pipe fed across the per-k-tile barrier);
     // TATRG_GEMM_WN64 selects the 8-warp variant for comparison
     static const bool wn64 = getenv("TATRG_GEMM_WN64") != nullptr;
+    static const bool bk16 = getenv("TATRG_GEMM_BK16") != nullptr;   // comparison: BK = 16, 4 stages
     if (bn == 64)
-        dispatch_big<64, 64>(p);
+        dispatch_big<64, 64, 16, 4>(p);
     else if (wn64)
-        dispatch_big<128, 64>(p);
+        dispatch_big<128, 64, 16, 4>(p);
+    else if (bk16)
+        dispatch_big<128, 32, 16, 4>(p);
     else
-        dispatch_big<128, 32>(p);
+        dispatch_big<128, 32, 32, 3>(p);
 }
 
 }  // namespace tatrg
