@@ -232,17 +232,49 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
     double *Rtmp = ws_doubles((long long)ell * ell);
     Ten Yb = ws_tensor("rz", {rows, ell});
     Ten Yt = ws_tensor("rz", {cols, ell});
-    apply(omega.p, Yb.p);
-    tsqr(Yb.p, rows, ell, Rtmp);
-    for (int it = 0; it < q; ++it) {
-        apply_t(Yb.p, Yt.p);
-        tsqr(Yt.p, cols, ell, Rtmp);
-        apply(Yt.p, Yb.p);
-        tsqr(Yb.p, rows, ell, Rtmp);
-    }
-    apply_t(Yb.p, Yt.p);             // B^T = Op^T Q
     double *Rb = ws_doubles((long long)ell * ell);
-    tsqr(Yt.p, cols, ell, Rb);       // B^T = Q_B R_B; the row-major R_B buffer is R_B^T column-major
+    // Fast route for tall blocks: asynchronous Cholesky-QR -- between iterations one shifted pass (only
+    // the span is carried on), two passes for the two blocks that define the result (Q and Q_B); the
+    // flags / condition estimates are read once at the end, and if they are bad everything is redone
+    // with the robust synchronous QR.
+    bool done = false;
+    if (ell <= 128 && rows >= 16LL * ell && cols >= 16LL * ell && rows >= 512 && cols >= 512) {
+        int *flag = (int *)ws_alloc(sizeof(int));
+        double *ratio = ws_doubles(4);
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+        const double it_shift = 1e-13;
+        apply(omega.p, Yb.p);
+        cholqr_async(Yb.p, rows, ell, q == 0 ? 2 : 1, q == 0 ? 0.0 : it_shift, flag, q == 0 ? ratio : nullptr, nullptr);
+        for (int it = 0; it < q; ++it) {
+            const bool last = it == q - 1;
+            apply_t(Yb.p, Yt.p);
+            cholqr_async(Yt.p, cols, ell, 1, it_shift, flag, nullptr, nullptr);
+            apply(Yt.p, Yb.p);
+            cholqr_async(Yb.p, rows, ell, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
+        }
+        apply_t(Yb.p, Yt.p);             // B^T = Op^T Q
+        cholqr_async(Yt.p, cols, ell, 2, 0.0, flag, ratio + 2, Rb);
+        struct {
+            int f;
+            double r[4];
+        } h;
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(h.r, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+        done = h.f == 0 && h.r[0] > 1e-5 * h.r[1] && h.r[2] > 1e-5 * h.r[3];
+    }
+    if (!done) {
+        apply(omega.p, Yb.p);
+        tsqr(Yb.p, rows, ell, Rtmp);
+        for (int it = 0; it < q; ++it) {
+            apply_t(Yb.p, Yt.p);
+            tsqr(Yt.p, cols, ell, Rtmp);
+            apply(Yt.p, Yb.p);
+            tsqr(Yb.p, rows, ell, Rtmp);
+        }
+        apply_t(Yb.p, Yt.p);             // B^T = Op^T Q
+        tsqr(Yt.p, cols, ell, Rb);       // B^T = Q_B R_B; the row-major R_B buffer is R_B^T column-major
+    }
     double *V = ws_doubles((long long)ell * ell);
     double *s = ws_doubles(ell);
     jacobi_svd(Rb, ell, ell, V, s, 1, 0, 0, 0);   // R_B^T V = U diag(s)
@@ -436,42 +468,87 @@ struct RedBasis {
     Ten L2inv;   // [k,l] lower triangular: Q = Q1 L2inv^T
 };
 
-bool ortho_factor(const Ten &T, RedBasis &o)
+// Two phases: phase 1 enqueues everything up to |G2 - I| and its read-back, phase 2 (after the host has
+// looked at it) the second factor and R.
+struct OrthoChain {
+    Ten T;
+    RedBasis o;
+    long long nk = 0;
+    Ten G1, G2;
+    struct Back {
+        int flag;
+        int pad;
+        double err;
+    } *back = nullptr;
+    double err = INFINITY;
+
+    void alloc(const Ten &T_)   // on the main stream: what outlives the fork
+    {
+        T = T_;
+        const long long n0 = T.legs[0].n, n1 = T.legs[1].n, n2 = T.legs[2].n, n3 = T.legs[3].n, a = T.legs[4].n;
+        nk = n0 * a;
+        o.Q1 = ws_tensor("pqtk", {n1, n2, n3, nk});
+        o.R = ws_tensor("kcb", {nk, n0, a});
+        o.L2inv = ws_tensor("kl", {nk, nk});
+    }
+    void phase1(char *pinned)
+    {
+        back = reinterpret_cast<Back *>(pinned);
+        const long long n0 = T.legs[0].n, a = T.legs[4].n;
+        int *flag = (int *)ws_alloc(sizeof(int));
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+        G1 = ws_tensor("cbde", {n0, a, n0, a});
+        Ten L1inv = ws_tensor("kcb", {nk, n0, a});
+        contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true);
+        cholesky_lower_async(G1.p, (int)nk, 0.0, L1inv.p, flag);
+        contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
+        G2 = ws_tensor("kl", {nk, nk});
+        contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
+        double *dev = ws_doubles(1);
+        max_dev_identity(G2.p, (int)nk, dev);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->err, dev, sizeof(double), cudaMemcpyDeviceToHost, stream()));
+    }
+    bool usable()   // after the chain's stream has been synchronised
+    {
+        err = back->err;
+        return back->flag == 0 && err < 0.05;
+    }
+    bool phase2()
+    {
+        if (err < 1e-8)
+            near_identity_chol(G2.p, (int)nk, o.L2inv.p);
+        else if (!cholesky_lower(G2.p, (int)nk, 0.0, o.L2inv.p))
+            return false;
+        // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
+        contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
+        return true;
+    }
+};
+
+// Both bases of the reduced bond swap; false when either matricisation is rank deficient or too
+// ill conditioned for two Cholesky-QR passes (|G2 - I| > 0.05).  One after the other on the caller's
+// stream: the work is dominated by machine-filling GEMMs, which gain nothing from overlapping (and
+// whose per-launch timing would be blurred by it).
+bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
 {
-    const long long n0 = T.legs[0].n, n1 = T.legs[1].n, n2 = T.legs[2].n, n3 = T.legs[3].n, a = T.legs[4].n;
-    const long long nk = n0 * a;
-    if (nk > 0x7fffffff) return false;
-    o.Q1 = ws_tensor("pqtk", {n1, n2, n3, nk});
-    o.R = ws_tensor("kcb", {nk, n0, a});
-    o.L2inv = ws_tensor("kl", {nk, nk});
-    size_t mk = ws_mark();
-    Ten G1 = ws_tensor("cbde", {n0, a, n0, a});
-    Ten L1inv = ws_tensor("kcb", {nk, n0, a});
-    contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true);
-    if (!cholesky_lower(G1.p, (int)nk, 0.0, L1inv.p)) {
+    Ctx &c = ctx();
+    if (!c.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c.pinned, Ctx::PINNED_BYTES));
+    OrthoChain ch[2];
+    ch[0].alloc(A);
+    ch[1].alloc(D);
+    if (ch[0].nk > 0x7fffffff) return false;
+    bool ok = true;
+    for (int i = 0; i < 2 && ok; ++i) {
+        size_t mk = ws_mark();
+        ch[i].phase1(c.pinned);
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+        ok = ch[i].usable() && ch[i].phase2();
         ws_release(mk);
-        return false;
     }
-    contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
-    Ten G2 = ws_tensor("kl", {nk, nk});
-    contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
-    double *dev = ws_doubles(1);
-    max_dev_identity(G2.p, (int)nk, dev);
-    const double err = d2h(dev, 1)[0];
-    if (!(err < 0.05)) {
-        ws_release(mk);
-        return false;
-    }
-    if (err < 1e-8) {
-        near_identity_chol(G2.p, (int)nk, o.L2inv.p);
-    } else if (!cholesky_lower(G2.p, (int)nk, 0.0, o.L2inv.p)) {
-        ws_release(mk);
-        return false;
-    }
-    // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
-    contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
-    ws_release(mk);
-    return true;
+    bA = ch[0].o;
+    bD = ch[1].o;
+    return ok;
 }
 
 }  // namespace
@@ -626,11 +703,46 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     double *sT = ws_doubles(g0);
     const size_t canon_mark = ws_mark();
     Ten Qp = ws_tensor("rg", {R, g0}), Qs = ws_tensor("rg", {R, g0});
-    d2d(Qp.p, c.phi, R * g0);
-    d2d(Qs.p, c.psi, R * g0);
     Ten Rp = ws_tensor("gr", {g0, g0}), Rs = ws_tensor("hr", {g0, g0});
-    tsqr(Qp.p, R, g0, Rp.p);
-    tsqr(Qs.p, R, g0, Rs.p);
+    {
+        // the two tall QRs are independent: asynchronous Cholesky-QR2 on two streams; a side that is
+        // rank deficient or too ill conditioned for it (the early steps) is redone by the robust route
+        bool qr_done[2] = {false, false};
+        double *Yq[2] = {Qp.p, Qs.p};
+        const double *src[2] = {c.phi, c.psi};
+        double *Rq[2] = {Rp.p, Rs.p};
+        if (R >= 16LL * g0 && R >= 512) {
+            struct QrBack {
+                int flag;
+                int pad;
+                double ratio[2];
+            };
+            Fork fk(2);
+            for (int i = 0; i < 2; ++i) {
+                fk.enter(i);
+                QrBack *bk = reinterpret_cast<QrBack *>(fk.pinned(i));
+                d2d(Yq[i], src[i], R * g0);
+                int *flag = (int *)ws_alloc(sizeof(int));
+                double *ratio = ws_doubles(2);
+                TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+                cholqr_async(Yq[i], R, g0, 2, 0.0, flag, ratio, Rq[i]);
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(&bk->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(bk->ratio, ratio, 2 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+                fk.leave();
+            }
+            for (int i = 0; i < 2; ++i) {
+                fk.sync(i);
+                const QrBack *bk = reinterpret_cast<QrBack *>(fk.pinned(i));
+                qr_done[i] = bk->flag == 0 && bk->ratio[0] > 1e-5 * bk->ratio[1];
+            }
+            fk.join();
+        }
+        for (int i = 0; i < 2; ++i)
+            if (!qr_done[i]) {
+                d2d(Yq[i], src[i], R * g0);
+                tsqr(Yq[i], R, g0, Rq[i]);
+            }
+    }
     // C = R_Phi R_Psi^T, stored transposed ([h][g]) so that the buffer is column-major C
     Ten Cm = ws_tensor("hg", {g0, g0});
     contract(Rs, Rp, Cm);
@@ -678,7 +790,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     if (nT >= 2 * nk && nk >= 16) {
         size_t mk = ws_mark();
         RedBasis bA, bD;
-        if (ortho_factor(A, bA) && ortho_factor(D, bD)) {
+        if (ortho_factor_pair(A, D, bA, bD)) {
             const long long rdim = a * nk;
             const int ellr = (int)std::min<long long>(ell, rdim);
             // Omega_red[b,l,z] = sum_l' L2inv_D[l,l'] sum_uvw Q1_D[uvw,l'] Omega[b,uvw,z]
