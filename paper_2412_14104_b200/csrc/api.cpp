@@ -510,6 +510,10 @@ void tatrg_destroy(void)
         for (auto &e : c.join_ev) cudaEventDestroy(e);
         cudaEventDestroy(c.fork_ev);
     }
+    if (c.copy_stream) {
+        cudaStreamDestroy(c.copy_stream);
+        for (auto &e : c.pre_ev) cudaEventDestroy(e);
+    }
     if (c.pinned) cudaFreeHost(c.pinned);
     for (auto &b : c.start_blk)
         if (b) cudaFreeHost(b);

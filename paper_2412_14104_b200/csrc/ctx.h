@@ -43,6 +43,13 @@ struct Ctx {
     double *start_blk[4] = {};              // page-locked start blocks of the iterative solvers
     long long start_blk_n[4] = {};
 
+    // host-resident inputs of a step are uploaded by a copy stream from the start of the step on
+    // (step.cpp: prefetch_inputs), overlapping the canonical form; get_input waits for the event
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t pre_ev[9] = {};
+    double *pre[9] = {};
+    size_t pre_n[9] = {};
+
     Input in[9];
     std::vector<double> spec[10];
     double gaps[4] = {0, 0, 0, 0};

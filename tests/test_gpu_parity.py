@@ -109,3 +109,60 @@ def test_config4_atrg_chi24_vs_triad(tt):
             fn(m % 4 + 1, 24, 2, 2, 20241217)
         out.append(tt.log_Z_per_site())
     assert abs(out[0] / out[1] - 1) < 1e-4, out
+
+
+def _supply(tt, where, seed, m, d, chi, r, only=None):
+    import torch
+    import seeded_inputs as si
+    keep = []
+    for which in range(9):
+        if only is not None and which not in only:
+            continue
+        rows, cols = tt.sketch_shape(which, d, chi, r)
+        if rows * cols == 0:
+            continue
+        g = si.gauss(si.subseed(seed, 0 if which >= 5 else m, which), rows * cols)
+        if where == "host_pageable":
+            buf = g
+        else:
+            buf = torch.from_numpy(g)
+            buf = buf.cuda() if where == "device" else buf.pin_memory()
+        keep.append(buf)
+        tt.set_sketch(which, buf)
+    return keep
+
+
+@pytest.mark.parametrize("where", ["host_pinned", "host_pageable", "device"])
+def test_caller_supplied_inputs(tt, where):
+    """Sketches and gauge references handed over through tatrg_set_sketch (host buffers are uploaded
+    by the library's copy stream while the step's first stage runs; device buffers are used in place)
+    give the oracle's result like the internally generated ones: same generator, same sub-seeds."""
+    beta, chi, r, q, seed = 1 / 6.0, 6, 2, 2, 20241214      # config 1: no cut through a degenerate multiplet
+    st = orc.init_ising_tensor(beta, 0.0)
+    tt.init_ising_tensor(beta, 0.0)
+    for m in range(7):
+        d = m % 4 + 1
+        keep = _supply(tt, where, seed, m, d, chi, r)
+        rec = orc.coarse_grain(st, d, chi, r, q, driver.seeded_inputs_for(seed, m))
+        tt.coarse_grain(d, chi, r, q, seed)
+        del keep
+        lo, lg = orc.log_Z_per_site(st), tt.log_Z_per_site()
+        assert abs(lg / lo - 1) <= LNZ_RTOL, (m, lg, lo)
+        for name in ("sigma_swap", "s1", "s2", "s3"):
+            so, sg = np.asarray(rec[name]), tt.get_spectrum(name)
+            assert len(so) == len(sg) and np.abs(so - sg).max() <= SPEC_TOL * so[0], (m, name)
+
+
+@pytest.mark.parametrize("where", ["host_pinned", "device"])
+def test_caller_supplied_sketch_is_the_one_used(tt, where):
+    """A swap sketch from another stream changes the step at truncation level (and only there)."""
+    beta, chi, r, q, seed = 1 / 6.0, 6, 2, 2, 20241214
+    out = []
+    for other in (False, True):
+        tt.init_ising_tensor(beta, 0.0)
+        for m in range(6):
+            keep = _supply(tt, where, seed + 17, m, m % 4 + 1, chi, r, only=(0,)) if (other and m == 5) else None
+            tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
+            del keep
+        out.append(tt.log_Z_per_site())
+    assert 1e-13 < abs(out[0] / out[1] - 1) < 1e-3, out
