@@ -166,3 +166,17 @@ def test_caller_supplied_sketch_is_the_one_used(tt, where):
             del keep
         out.append(tt.log_Z_per_site())
     assert 1e-13 < abs(out[0] / out[1] - 1) < 1e-3, out
+
+
+def test_order_parameter_matches_oracle(tt):
+    """X^(m) = (Tr A)^2 / Tr(A^2) from the device-resident (Phi, Psi)
+    against the oracle's, every leg, along the config-1 schedule."""
+    beta, chi, r, q, seed = 1 / 6.0, 6, 2, 2, 20241214
+    st = orc.init_ising_tensor(beta, 0.0)
+    tt.init_ising_tensor(beta, 0.0)
+    for m in range(6):
+        orc.coarse_grain(st, m % 4 + 1, chi, r, q, driver.seeded_inputs_for(seed, m))
+        tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
+        for leg in range(4):
+            xo, xg = orc.order_parameter_X(st, leg), tt.order_parameter(leg + 1)
+            assert abs(xg / xo - 1) < 1e-9, (m, leg, xg, xo)

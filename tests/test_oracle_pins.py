@@ -330,3 +330,33 @@ def test_bad_arguments():
     st = orc.init_ising_tensor(BETA)
     with pytest.raises(ValueError):
         orc.coarse_grain(st, 5, 4, 2, 2, driver.seeded_inputs_for(1, 0))
+
+
+# --------------------------------------------------------------------------- order parameter
+def test_order_parameter_definition_on_the_dense_tensor():
+    """X = (Tr A)^2 / Tr(A^2), A_kl = sum_{i1 i2 i3} T_{i1 i2 i3 k; i1 i2 i3 l} written out
+    with explicit loops on the dense initial tensor T = Phi Psi^T (2^8 elements), for every open leg."""
+    beta, h = 0.3, 0.07
+    st = orc.init_ising_tensor(beta, h)
+    T = np.tensordot(st.phi, st.psi, axes=([4], [4]))          # T[i1..i4, j1..j4]
+    for leg in range(4):
+        A = np.zeros((2, 2))
+        for idx in np.ndindex(2, 2, 2, 2):
+            for l in range(2):
+                jdx = list(idx)
+                jdx[leg] = l
+                A[idx[leg], l] += T[idx + tuple(jdx)]
+        X = np.trace(A) ** 2 / np.trace(A @ A)
+        assert abs(orc.order_parameter_X(st, leg) - X) < 1e-13
+
+
+def test_order_parameter_counts_degenerate_ground_states():
+    """Deep in the ordered phase (T = 3 << T_c = 6.65, h = 0) two degenerate states dominate: X -> 2;
+    deep in the disordered phase (T = 12) one: X -> 1."""
+    def X_after(T, steps):
+        st = orc.init_ising_tensor(1 / T, 0.0)
+        for m in range(steps):
+            orc.coarse_grain(st, m % 4 + 1, 4, 2, 2, driver.seeded_inputs_for(7, m))
+        return orc.order_parameter_X(st, 3)
+    assert abs(X_after(3.0, 8) - 2.0) < 1e-2
+    assert abs(X_after(12.0, 16) - 1.0) < 2e-2
