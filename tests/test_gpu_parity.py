@@ -21,7 +21,7 @@ def tt():
     import paper_2412_14104_b200 as t
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
-    t.set_workspace(nbytes=6 << 30)
+    t.set_workspace(nbytes=8 << 30)
     t.set_stream()
     yield t
     t.destroy()
@@ -79,6 +79,14 @@ def test_config2_chi16_first_steps(tt):
     """BASELINE.json configs[1] (T=6.65, chi=16, r=2, q=2): the first 10 of its 40 steps (the oracle
     needs ~seconds per step at chi=16)."""
     check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 10, 20241215))
+
+
+def test_config3_chi32_first_steps_incl_one_full_size_step(tt):
+    """BASELINE.json configs[2] (the headline config: T=6.65, chi=32, r=2, q=2), the first 5 of its 40
+    steps.  Step 5 has all legs and the bond = 32 on input: the launch configuration bench.py times
+    (reduced bond swap, concurrent isometry / squeezer chains, 64-column sketches); the oracle needs
+    about a minute for it."""
+    check(run_both(tt, 1 / 6.65, 0.0, 32, 2, 2, 5, 20241216))
 
 
 def test_plain_atrg_parity(tt):
