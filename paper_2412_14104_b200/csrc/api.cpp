@@ -45,6 +45,17 @@ void fail(int code, const char *fmt, ...)
     throw Err{code};
 }
 
+void trace_mark(const char *label)
+{
+    static const bool trace = getenv("TATRG_TRACE") != nullptr;
+    if (!trace) return;
+    Ctx &c = ctx();
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    cudaEventRecord(e, c.stream);
+    c.tmarks.emplace_back(label, e);
+}
+
 int prof_begin(double flops, int big)
 {
     Ctx &c = ctx();
@@ -102,6 +113,15 @@ void prof_collect()
         c.gemm_n[r.stage][r.big] += 1;
     }
     c.prof_rec.clear();
+    if (trace && !c.tmarks.empty()) {
+        for (size_t i = 1; i < c.tmarks.size(); ++i) {
+            float ms = 0;
+            cudaEventElapsedTime(&ms, c.tmarks[i - 1].second, c.tmarks[i].second);
+            fprintf(stderr, "tatrg-trace mark %-28s %.3f ms\n", c.tmarks[i].first.c_str(), ms);
+        }
+        for (auto &m : c.tmarks) cudaEventDestroy(m.second);
+        c.tmarks.clear();
+    }
     if (trace) {
         fprintf(stderr, "tatrg-trace host: %lld tensor_gemm calls, %.3f ms on the host (%.2f us each)\n", c.host_contract_n,
                 1e3 * c.host_contract_s, c.host_contract_n ? 1e6 * c.host_contract_s / c.host_contract_n : 0.0);

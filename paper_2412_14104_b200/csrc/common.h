@@ -65,6 +65,7 @@ inline double gemm_flops(const GemmParams &p)
 cudaStream_t stream();
 void count_launch(int n = 1);
 void count_flops(double f);
+void trace_mark(const char *label);   // TATRG_TRACE: labelled timestamp on the main stream
 int prof_begin(double flops, int big);
 void prof_end(int slot);
 void prof_shape(int M, int N, int K, int batch, int ksplit);   // shape of the next profiled launch (trace)
@@ -95,6 +96,7 @@ struct Err {
 // gemm.cu
 void tensor_gemm(GemmParams p);
 void tensor_gemm_big(const GemmParams &p, int bn);   // gemm_big.cu: the 128 x bn CTA tile, bn = 128 or 64
+bool tensor_gemm_ts(const GemmParams &p);   // ts.cu: HBM-bound tall-and-skinny shapes; false = not taken
 double probe_fp64_peak(int mode, int iters);
 // qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
 // Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).

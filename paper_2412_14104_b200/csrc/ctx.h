@@ -74,6 +74,7 @@ struct Ctx {
         int shape[5];   // M, N, K, batch, ksplit
     };
     int prof_shape[5] = {0, 0, 0, 0, 0};
+    std::vector<std::pair<std::string, cudaEvent_t>> tmarks;   // TATRG_TRACE: labelled events inside a step
     double host_contract_s = 0;   // host seconds spent inside contract() (trace only)
     long long host_contract_n = 0;
     std::vector<ProfRec> prof_rec;

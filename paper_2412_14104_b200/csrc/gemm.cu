@@ -301,6 +301,7 @@ void tensor_gemm(GemmParams p)
         TATRG_CUDA_CHECK(cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev));
     }
     count_flops(gemm_flops(p));
+    if (tensor_gemm_ts(p)) return;   // tall-and-skinny: streaming kernels (HBM-bound)
     // tile choice: 128x128 when it fills the machine (with split-K when the summed index is long),
     // 128x64 for outputs at most 64 columns wide with enough rows, else the 64x64 tile
     int ktiles = (p.K + BK - 1) / BK;

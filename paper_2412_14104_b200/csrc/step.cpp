@@ -726,6 +726,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     double gaps[4] = {INFINITY, INFINITY, INFINITY, INFINITY};
 
     stage_mark(0);
+    trace_mark("step begin");
     // =================== O2 canonical form ===================
     // A, D and sigma^T outlive this stage; everything else of it (the chi^5-sized Q factors included)
     // is released once A and D are formed
@@ -773,6 +774,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 tsqr(Yq[i], R, g0, Rq[i]);
             }
     }
+    trace_mark("canon: two tall QRs");
     // C = R_Phi R_Psi^T, stored transposed ([h][g]) so that the buffer is column-major C
     Ten Cm = ws_tensor("hg", {g0, g0});
     contract(Rs, Rp, Cm);
@@ -785,6 +787,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     scale_leg(Cm.p, (long long)a * g0, g0, a, sT, 1);
     Ten u = Ten::make(Cm.p, "ag", {a, g0});   // u[a][g] = u_a[g]
     Ten v = Ten::make(Vc.p, "ah", {a, g0});
+    trace_mark("canon: core svd");
     // gauge (reading G12): P = A^T G_ref = u^T (Q_Phi^T G_ref)
     Ten QpR = rot_view(Qp.p, g0), QsR = rot_view(Qs.p, g0);
     Ten ref = get_input(5, R, a, cfg, "rb");
@@ -797,9 +800,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten u2 = ws_tensor("bg", {a, g0}), v2 = ws_tensor("bg", {a, g0});
     contract(Wg, u, u2);                    // u2[b][g] = sum_a W[a,b] u[a][g]
     contract(Wg, v.as("ag"), v2);
+    trace_mark("canon: gauge");
     Ten A = Ten::make(Abuf, "xpqta", {n0, n1, n2, n3, a}), D = Ten::make(Dbuf, "xpqta", {n0, n1, n2, n3, a});
     contract(QpR.as("xpqtg"), u2.as("ag"), A);
     contract(QsR.as("xpqtg"), v2.as("ag"), D);
+    trace_mark("canon: A, D");
     ws_release(canon_mark);
     stage_mark(1);
 
@@ -821,6 +826,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         size_t mk = ws_mark();
         RedBasis bA, bD;
         if (ortho_factor_pair(A, D, bA, bD)) {
+            trace_mark("swap: bases of A, D");
             const long long rdim = a * nk;
             const int ellr = (int)std::min<long long>(ell, rdim);
             // Omega_red[b,l,z] = sum_l' L2inv_D[l,l'] sum_uvw Q1_D[uvw,l'] Omega[b,uvw,z]
@@ -833,6 +839,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 contract(bD.L2inv.as("lm"), t1, om_red);
                 ws_release(mk2);
             }
+            trace_mark("swap: sketch projection");
             Ten Z = ws_tensor("cabz", {n0, a, a, ell});
             auto apply = [&](const double *w, double *out) {     // m w : [(b,l), z] -> [(a,k), z]
                 contract(bD.R.as("lca"), Ten::make(const_cast<double *>(w), "blz", {a, nk, ell}), Z);
@@ -854,6 +861,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 spec[1].assign(ro.s_full.begin(), ro.s_full.begin() + gs);
                 gaps[0] = rel_gap(ro.s_full, gs);
                 ws_release(mk2);
+                trace_mark("swap: rsvd of the core");
                 // expand: X[a,pqt,g] = sum_m Q1_A[pqt,m] sum_k L2inv_A[k,m] x[a,k,g]
                 Ten t2 = ws_tensor("amg", {a, nk, gs});
                 contract(bA.L2inv.as("km"), Ten::make(xr, "akg", {a, nk, gs}), t2);
@@ -904,6 +912,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     d2d(Ys.p, Y.p, Y.size());
     scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
     scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
+    trace_mark("swap: expansion, scaling");
     stage_mark(2);
 
     Ten U[4];   // A, X, Y, D : [p,q,k]

@@ -224,3 +224,28 @@ def test_tensor_gemm_tile_variants(tt, M, N, K):
     tt.tensor_gemm(dA, dB, dC, M, N, K, maps)
     torch.cuda.synchronize()
     np.testing.assert_allclose(dC.cpu().numpy(), A @ B, rtol=0, atol=1e-11 * np.sqrt(K))
+
+
+@pytest.mark.parametrize("M,N,K", [(20000, 32, 32), (16384, 64, 64), (70001, 17, 33), (33000, 6, 6),
+                                   (32, 32, 50000), (64, 64, 16384), (13, 40, 70001), (6, 6, 20000)])
+def test_tensor_gemm_tall_skinny_streaming(tt, M, N, K):
+    """The HBM-bound tall-and-skinny shapes (ts.cu): rows x K times K x N with <= 64 columns, and the
+    (M x rows)(rows x N) products behind the Gram matrices of the Cholesky-QR passes."""
+    import torch
+    rng = np.random.default_rng(M + 3 * N + 7 * K)
+    A, B = rng.standard_normal((M, K)), rng.standard_normal((K, N))
+    dA, dB = _dev(A), _dev(B)
+    dC = torch.full((M, N), 7.0, dtype=torch.float64, device="cuda")
+    maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+    tt.tensor_gemm(dA, dB, dC, M, N, K, maps)
+    torch.cuda.synchronize()
+    np.testing.assert_allclose(dC.cpu().numpy(), A @ B, rtol=0, atol=1e-11 * np.sqrt(K))
+    # A^T as the left operand (its small index contiguous): C2 = A^T-layout product, plus accumulate
+    if M <= 64:
+        At = np.ascontiguousarray(A.T)                      # K x M, element (k, m) at k*M + m
+        dAt = _dev(At)
+        dC2 = torch.full((M, N), 1.0, dtype=torch.float64, device="cuda")
+        maps2 = dict(am=[(M, 1)], ak=[(K, M)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+        tt.tensor_gemm(dAt, dB, dC2, M, N, K, maps2, alpha=0.5, accumulate=True)
+        torch.cuda.synchronize()
+        np.testing.assert_allclose(dC2.cpu().numpy(), 1.0 + 0.5 * (A @ B), rtol=0, atol=1e-11 * np.sqrt(K))
