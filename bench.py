@@ -40,6 +40,7 @@ CONFIGS = {
     "c1": dict(T=6.0, h=0.0, chi=6, r=2, q=2, seed=20241214, ramp=4),
     "c2": dict(T=6.65, h=0.0, chi=16, r=2, q=2, seed=20241215, ramp=8),
     "c3": dict(T=6.65, h=0.0, chi=32, r=2, q=2, seed=20241216, ramp=8),
+    "c4": dict(T=6.65, h=0.0, chi=24, r=2, q=2, seed=20241217, ramp=8, atrg=True),   # plain ATRG, O(chi^9)
     "c5": dict(T=6.5, h=0.01, chi=64, r=2, q=3, seed=20241218, ramp=8),
 }
 # DRAM traffic of one launch of the dominant kernel, from the committed `ncu --set full` capture
@@ -53,8 +54,10 @@ FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
 
 
 def workload_name(name, c):
-    return ("%s: 4D Ising T=%.2f h=%g, Triad-ATRG chi=%d r=%d q=%d, steady-state coarse-grain steps "
-            "(all legs = chi), directions cycling 1..4" % (name, c["T"], c["h"], c["chi"], c["r"], c["q"]))
+    return ("%s: 4D Ising T=%.2f h=%g, %s chi=%d r=%d q=%d, steady-state coarse-grain steps "
+            "(all legs = chi), directions cycling 1..4" % (name, c["T"], c["h"],
+                                                            "plain ATRG (O(chi^9) contraction)" if c.get("atrg") else "Triad-ATRG",
+                                                            c["chi"], c["r"], c["q"]))
 
 
 def measured_peaks():
@@ -173,7 +176,8 @@ def oracle_sample(cfg):
     from oracle import tatrg_oracle as orc
     st = orc.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
     for m in range(3):
-        orc.coarse_grain(st, m + 1, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], m))
+        orc.coarse_grain(st, m + 1, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], m),
+                         mode="atrg" if cfg.get("atrg") else "triad")
     return st
 
 
@@ -183,7 +187,8 @@ def oracle_time_one(cfg, st0):
     from oracle import tatrg_oracle as orc
     st = copy.deepcopy(st0)
     t0 = time.perf_counter()
-    orc.coarse_grain(st, 4, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], 3))
+    orc.coarse_grain(st, 4, cfg["chi"], cfg["r"], cfg["q"], driver.seeded_inputs_for(cfg["seed"], 3),
+                     mode="atrg" if cfg.get("atrg") else "triad")
     dt = time.perf_counter() - t0
     return dt, st
 
@@ -277,7 +282,8 @@ def run_ours(args, cfg, name):
 
     chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
     K, W = args.steps, max(args.warmup, 0)
-    tt.set_workspace(chi=chi, r=r, device="cuda:%d" % local)
+    tt.set_workspace(chi=chi, r=r, device="cuda:%d" % local, atrg=bool(cfg.get("atrg")))
+    step_fn = tt.coarse_grain_atrg if cfg.get("atrg") else tt.coarse_grain
     stream = torch.cuda.Stream()
     tt.set_stream(stream)
     tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
@@ -285,7 +291,7 @@ def run_ours(args, cfg, name):
     for _ in range(cfg["ramp"]):                       # untimed ramp-up to the steady state
         for which, t in gauge_refs(tt, cfg, m % 4 + 1).items():
             tt.set_sketch(which, t)
-        tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
+        step_fn(m % 4 + 1, chi, r, q, seed)
         m += 1
     dims = tt.get_dims()
     steady = all(d == chi for d in dims[:5])
@@ -323,7 +329,7 @@ def run_ours(args, cfg, name):
             return dev[i]
     for i in range(W):
         set_inputs(inputs_for(i), (m + i) % 4 + 1)
-        tt.coarse_grain((m + i) % 4 + 1, chi, r, q, seed)
+        step_fn((m + i) % 4 + 1, chi, r, q, seed)
     tt.set_profile(2 if args.profile_all else 1)
     tt.launch_count(reset=True)
     tt.gemm_flops(reset=True)
@@ -345,7 +351,7 @@ def run_ours(args, cfg, name):
             pairs.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
             pairs[-1][0].record(stream)
         set_inputs(sk, d)
-        tt.coarse_grain(d, chi, r, q, seed)
+        step_fn(d, chi, r, q, seed)
         if streamed:
             pairs[-1][1].record(stream)
         for k, v in tt.stage_ms().items():
@@ -385,7 +391,7 @@ def run_ours(args, cfg, name):
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
             set_inputs(host, d)                          # host pointers: copied inside coarse_grain
-            tt.coarse_grain(d, chi, r, q, seed)
+            step_fn(d, chi, r, q, seed)
             lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
             b.record(stream)
             pairs2.append((a, b))
@@ -399,7 +405,7 @@ def run_ours(args, cfg, name):
         for i in range(Ke):
             d = (m + i) % 4 + 1
             set_inputs(host2[i], d)                      # host pointers: copied inside coarse_grain
-            tt.coarse_grain(d, chi, r, q, seed)
+            step_fn(d, chi, r, q, seed)
             lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
             h2d += sum(t.numel() * 8 for t in host2[i].values())
         e3.record(stream)

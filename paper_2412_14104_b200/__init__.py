@@ -105,11 +105,13 @@ def _require_cuda():
 
 
 # ------------------------------------------------------------------ plumbing
-def set_workspace(nbytes: int | None = None, chi: int | None = None, r: int = 2, device="cuda:0"):
-    """Allocates the workspace as a torch tensor (PyTorch owns device memory) and hands it over."""
+def set_workspace(nbytes: int | None = None, chi: int | None = None, r: int = 2, device="cuda:0", atrg: bool = False):
+    """Allocates the workspace as a torch tensor (PyTorch owns device memory) and hands it over.
+    atrg: size it for coarse_grain_atrg (the chi^6 slices of the plain ATRG contraction)."""
     torch = _require_cuda()
     if nbytes is None:
-        nbytes = int(lib().tatrg_workspace_bytes(int(chi), int(r)))
+        f = lib().tatrg_workspace_bytes_atrg if atrg else lib().tatrg_workspace_bytes
+        nbytes = int(f(int(chi), int(r)))
     buf = torch.empty((nbytes + 255) // 256 * 32, dtype=torch.float64, device=device)
     _keep["ws"] = buf
     _check(lib().tatrg_set_workspace(buf.data_ptr(), buf.numel() * 8))

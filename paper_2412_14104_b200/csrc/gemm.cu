@@ -10,6 +10,7 @@
 // memory as [k][m] / [k][n] with a leading dimension = 4 (mod 16) doubles, which makes the
 // 8-byte DMMA fragment loads bank-conflict free, through a STAGES-deep cp.async pipeline.
 #include <math.h>
+#include <stdlib.h>
 
 #include <algorithm>
 
@@ -309,7 +310,7 @@ void tensor_gemm(GemmParams p)
     const int max_split = ktiles / 8 < 512 ? ktiles / 8 : 512;
     bool big = p.M >= 96 && p.N >= 96 &&
                (big_tiles * 5 >= 4LL * g_num_sms || big_tiles * (long long)(max_split > 1 ? max_split : 1) >= 2LL * g_num_sms);
-    const bool mid = !big && p.N <= 64 && p.N >= 33 && p.M >= 96;
+    const bool mid = !big && p.N <= 64 && p.N >= 17 && p.M >= 96;
     long long tiles = big ? big_tiles
                           : mid ? (long long)((p.M + 127) / 128) * p.batch
                                 : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
