@@ -5,8 +5,10 @@
 // swap (Table 1) and the O(r^2 chi^7) triad contraction (Eqs. 13-14)
 // run on.
 //
-// 128x128: 16 warps, warp tile 32 x 32 (32 FP64 accumulators per thread); 128x64: 4 warps, warp tile
-// 32 x 64.  BK = 16, 4-stage cp.async pipeline.
+// 128x128: 16 warps, warp tile 32 x 32 (32 FP64 accumulators per thread), BK = 32, 3-stage cp.async
+// pipeline synchronised by per-stage mbarriers ("full": the copies of all threads have landed, "empty":
+// all threads are done reading) instead of a CTA-wide barrier per k tile.  128x64: 4 warps, warp tile
+// 32 x 64, BK = 16, 4 stages, __syncthreads.
 // The shared-memory layout of an operand tile follows the operand's contiguous index in global
 // memory, so that 16-byte cp.async copies land on 16 consecutive bytes of shared memory:
 //   contiguous index = the free index (m or n):  tile stored [k][m], leading dimension 128 + 4
@@ -41,6 +43,36 @@ __device__ __forceinline__ void cp_async_wait()
 {
     asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
 }
+// ---- mbarrier helpers (shared::cta): per-stage "full" / "empty" barriers of the decoupled pipeline
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar))
+                 : "memory");
+}
+// arrives on `bar` once all cp.async copies issued so far by this thread have landed
+__device__ __forceinline__ void mbar_arrive_on_cp_async(unsigned long long *bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        " .reg .pred p;\n"
+        "WAIT_%=:\n"
+        " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra DONE_%=;\n"
+        " bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)),
+        "r"(parity)
+        : "memory");
+}
+
 __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -108,7 +140,7 @@ struct TileLoader {
     }
 };
 
-template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES>
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES, bool MBAR>
 __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_kernel(const __grid_constant__ GemmParams p)
 {
     constexpr int LD_K = BK + 4;
@@ -167,17 +199,36 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
     constexpr int B_KK = B_KF ? 4 : 4 * LD_FB;
 
 #pragma unroll
+    // MBAR: every stage has a "full" barrier (all threads' copies of the tile have landed) and an
+    // "empty" barrier (all threads are done reading it), so a warp only waits for data and for the
+    // slot it refills -- never for the slowest warp of the current tile, as with the CTA-wide barrier.
+    __shared__ unsigned long long full_bar[STAGES], empty_bar[STAGES];
+    if (MBAR) {
+        if (t == 0) {
+#pragma unroll
+            for (int s = 0; s < STAGES; ++s) {
+                mbar_init(&full_bar[s], NT);
+                mbar_init(&empty_bar[s], NT);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
     for (int s = 0; s < STAGES - 1; ++s) {
         if (s < nkt) {
             la.load(As + s * A_STAGE, p.ak, k_begin + s * BK, k_end);
             lb.load(Bs + s * B_STAGE, p.bk, k_begin + s * BK, k_end);
+            if (MBAR) mbar_arrive_on_cp_async(&full_bar[s]);
         }
         cp_async_commit();
     }
     for (int it = 0; it < nkt; ++it) {
-        cp_async_wait<STAGES - 2>();
-        __syncthreads();
-        {
+        const int slot = it % STAGES;
+        if (MBAR) {
+            mbar_wait(&full_bar[slot], (unsigned)(it / STAGES) & 1u);
+        } else {
+            cp_async_wait<STAGES - 2>();
+            __syncthreads();
             const int nx = it + STAGES - 1;
             if (nx < nkt) {
                 la.load(As + (nx % STAGES) * A_STAGE, p.ak, k_begin + nx * BK, k_end);
@@ -185,8 +236,8 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
             }
             cp_async_commit();
         }
-        const double *as = As + (it % STAGES) * A_STAGE + a_off;
-        const double *bs = Bs + (it % STAGES) * B_STAGE + b_off;
+        const double *as = As + slot * A_STAGE + a_off;
+        const double *bs = Bs + slot * B_STAGE + b_off;
 #pragma unroll
         for (int kk = 0; kk < BK / 4; ++kk) {
             double a[FM], b[FN];
@@ -198,6 +249,17 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
             for (int i = 0; i < FM; ++i)
 #pragma unroll
                 for (int j = 0; j < FN; ++j) dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+        if (MBAR) {
+            mbar_arrive(&empty_bar[slot]);             // this thread is done with the tile
+            const int nx = it + STAGES - 1;            // refill the slot of tile it - 1
+            if (nx < nkt) {
+                const int ns = nx % STAGES;
+                if (it >= 1) mbar_wait(&empty_bar[ns], (unsigned)((it - 1) / STAGES) & 1u);
+                la.load(As + ns * A_STAGE, p.ak, k_begin + nx * BK, k_end);
+                lb.load(Bs + ns * B_STAGE, p.bk, k_begin + nx * BK, k_end);
+                mbar_arrive_on_cp_async(&full_bar[ns]);
+            }
         }
     }
     cp_async_wait<0>();
@@ -251,7 +313,7 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
     }
 }
 
-template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES>
+template <bool A_KF, bool B_KF, bool VEC, int BN, int WN, int BK, int STAGES, bool MBAR>
 void launch_big(const GemmParams &p_in)
 {
     constexpr int NT = 128 * BN / WN;
@@ -260,7 +322,7 @@ void launch_big(const GemmParams &p_in)
     constexpr int B_STAGE = B_KF ? BN * LD_K : BK * (BN + 4);
     constexpr size_t smem = (size_t)STAGES * (A_STAGE + B_STAGE) * sizeof(double);
     static bool attr_done = false;
-    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN, WN, BK, STAGES>;
+    auto kern = tgemm_big_kernel<A_KF, B_KF, VEC, BN, WN, BK, STAGES, MBAR>;
     if (!attr_done) {
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
@@ -291,7 +353,7 @@ bool vec_ok(const double *base, const Map4 &fast, const Map4 &slow, const Map4 &
            all_even(batch);
 }
 
-template <int BN, int WN, int BK, int STAGES>
+template <int BN, int WN, int BK, int STAGES, bool MBAR>
 void dispatch_big(const GemmParams &p)
 {
     const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;
@@ -300,14 +362,14 @@ void dispatch_big(const GemmParams &p)
     const bool vec = va && vb;
     if (akf) {
         if (bkf)
-            vec ? launch_big<true, true, true, BN, WN, BK, STAGES>(p) : launch_big<true, true, false, BN, WN, BK, STAGES>(p);
+            vec ? launch_big<true, true, true, BN, WN, BK, STAGES, MBAR>(p) : launch_big<true, true, false, BN, WN, BK, STAGES, MBAR>(p);
         else
-            vec ? launch_big<true, false, true, BN, WN, BK, STAGES>(p) : launch_big<true, false, false, BN, WN, BK, STAGES>(p);
+            vec ? launch_big<true, false, true, BN, WN, BK, STAGES, MBAR>(p) : launch_big<true, false, false, BN, WN, BK, STAGES, MBAR>(p);
     } else {
         if (bkf)
-            vec ? launch_big<false, true, true, BN, WN, BK, STAGES>(p) : launch_big<false, true, false, BN, WN, BK, STAGES>(p);
+            vec ? launch_big<false, true, true, BN, WN, BK, STAGES, MBAR>(p) : launch_big<false, true, false, BN, WN, BK, STAGES, MBAR>(p);
         else
-            vec ? launch_big<false, false, true, BN, WN, BK, STAGES>(p) : launch_big<false, false, false, BN, WN, BK, STAGES>(p);
+            vec ? launch_big<false, false, true, BN, WN, BK, STAGES, MBAR>(p) : launch_big<false, false, false, BN, WN, BK, STAGES, MBAR>(p);
     }
 }
 
@@ -320,14 +382,19 @@ void tensor_gemm_big(const GemmParams &p, int bn)
     // TATRG_GEMM_WN64 selects the 8-warp variant for comparison
     static const bool wn64 = getenv("TATRG_GEMM_WN64") != nullptr;
     static const bool bk16 = getenv("TATRG_GEMM_BK16") != nullptr;   // comparison: BK = 16, 4 stages
+    // decoupled mbarrier pipeline (default; +9 % over the CTA-wide barrier on the c3 shapes);
+    // TATRG_GEMM_SYNC selects the __syncthreads pipeline for comparison
+    static const bool sync = getenv("TATRG_GEMM_SYNC") != nullptr;
     if (bn == 64)
-        dispatch_big<64, 64, 16, 4>(p);
+        dispatch_big<64, 64, 16, 4, false>(p);
     else if (wn64)
-        dispatch_big<128, 64, 16, 4>(p);
+        dispatch_big<128, 64, 16, 4, false>(p);
     else if (bk16)
-        dispatch_big<128, 32, 16, 4>(p);
+        dispatch_big<128, 32, 16, 4, false>(p);
+    else if (sync)
+        dispatch_big<128, 32, 32, 3, false>(p);
     else
-        dispatch_big<128, 32, 32, 3>(p);
+        dispatch_big<128, 32, 32, 3, true>(p);
 }
 
 }  // namespace tatrg
