@@ -131,7 +131,6 @@ void scale_rows(double *x, long long rows, long long cols, const double *v, int 
 void scale_leg(double *x, long long total, long long inner, long long n, const double *v, int mode);
 void symmetrize(double *x, int n);                                            // x = (x + x^T)/2
 void fill_identity(double *x, int n);
-void mirror_lower(double *x, int n);                                          // x[i][j] = x[j][i] for j > i
 void fill_zero(double *x, long long n);
 void transpose_small(const double *in, double *out, int rows, int cols);      // out[c,r] = in[r,c]
 void max_dev_identity(const double *G, int n, double *out);                   // out[0] = max |G - I| over the lower triangle

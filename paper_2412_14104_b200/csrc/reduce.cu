@@ -240,23 +240,6 @@ void symmetrize(double *x, int n)
     count_launch();
 }
 
-// x[i][j] = x[j][i] for j > i: completes a symmetric matrix whose lower triangle was computed
-__global__ void mirror_lower_kernel(double *__restrict__ x, int n)
-{
-    const long long total = (long long)n * n;
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-        const int r = (int)(i / n), c = (int)(i - (long long)r * n);
-        if (c > r) x[i] = x[(long long)c * n + r];
-    }
-}
-
-void mirror_lower(double *x, int n)
-{
-    mirror_lower_kernel<<<grid_for((long long)n * n), RED_THREADS, 0, stream()>>>(x, n);
-    TATRG_LAUNCH_CHECK();
-    count_launch();
-}
-
 void fill_identity(double *x, int n)
 {
     identity_kernel<<<grid_for((long long)n * n), RED_THREADS, 0, stream()>>>(x, n);

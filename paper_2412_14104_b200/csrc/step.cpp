@@ -950,23 +950,16 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             const Ten &Kt = (i == 0) ? A : (i == 1) ? Xs : (i == 2) ? Ys : D;
             const bool mid = (i == 0 || i == 3);
             const Ten &Rm = (i == 0) ? RX : RY;
-            // S is formed once (n12 x n12, its lower tiles by one machine-filling GEMM, then mirrored): the
-            // q + 2 applications are then small GEMMs instead of two passes over the chi^5-sized tensor each
-            Ten Sm = ws_tensor("pqPQ", {n1, n2, n1, n2});
-            {
-                size_t mk = ws_mark();
-                if (mid) {
-                    Ten KR = ws_tensor("xpqtb", {Kt.legs[0].n, n1, n2, Kt.legs[3].n, Kt.legs[4].n});
-                    contract(Kt.as("xpqta"), Rm, KR);
-                    contract(Kt.as("xpqtb"), KR.as("xPQtb"), Sm, 1.0, false, true);
-                } else {
-                    contract(Kt.as("xpqta"), Kt.as("xPQta"), Sm, 1.0, false, true);
-                }
-                mirror_lower(Sm.p, (int)n12);
-                ws_release(mk);
-            }
+            const long long e0 = Kt.legs[0].n, e3 = Kt.legs[3].n, e4 = Kt.legs[4].n;
+            Ten t1 = ws_tensor("xtaz", {e0, e3, e4, kk}), t2 = ws_tensor("xtbz", {e0, e3, e4, kk});
             auto S_op = [&](const double *w, double *out) {
-                contract(Sm, Ten::make(const_cast<double *>(w), "PQz", {n1, n2, kk}), Ten::make(out, "pqz", {n1, n2, kk}));
+                contract(Kt.as("xpqta"), Ten::make(const_cast<double *>(w), "pqz", {n1, n2, kk}), t1);
+                if (mid) {
+                    contract(t1, Rm, t2);
+                    contract(Kt.as("xpqtb"), t2, Ten::make(out, "pqz", {n1, n2, kk}));
+                } else {
+                    contract(Kt.as("xpqta"), t1, Ten::make(out, "pqz", {n1, n2, kk}));
+                }
             };
             int *flag = nullptr;
             double *ratio = nullptr;

@@ -171,18 +171,29 @@ __global__ void __launch_bounds__(TS_NT) ts_dot_kernel(const __grid_constant__ G
     }
 }
 
-// C = alpha * sum_b partial[b] (+ C), through the output maps; one thread per output
-__global__ void ts_dot_reduce_kernel(const __grid_constant__ GemmParams p, const double *__restrict__ partial, int nparts)
+// C = alpha * sum_b partial[b] (+ C), through the output maps.  A CTA of 32 x 32 threads owns 32 outputs;
+// thread (o, g) adds the partials b = g (mod 32) of output o, then the 32 groups are added in a fixed order.
+__global__ void __launch_bounds__(1024) ts_dot_reduce_kernel(const __grid_constant__ GemmParams p, const double *__restrict__ partial,
+                                                             int nparts)
 {
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= p.M * p.N) return;
+    __shared__ double red[32][33];
+    const int o = threadIdx.x & 31, g = threadIdx.x >> 5;
+    const int idx = blockIdx.x * 32 + o, total = p.M * p.N;
     double s = 0.0;
-    for (int b = 0; b < nparts; ++b) s += partial[(long long)b * p.M * p.N + idx];
-    const int i = idx / p.N, j = idx - i * p.N;
-    double *c = p.C + map_off(p.cm, i) + map_off(p.cn, j);
-    double v = p.alpha * s;
-    if (p.accumulate) v += *c;
-    *c = v;
+    if (idx < total)
+        for (int b = g; b < nparts; b += 32) s += partial[(long long)b * total + idx];
+    red[g][o] = s;
+    __syncthreads();
+    if (g == 0 && idx < total) {
+        double v = 0.0;
+#pragma unroll
+        for (int k = 0; k < 32; ++k) v += red[k][o];
+        const int i = idx / p.N, j = idx - i * p.N;
+        double *c = p.C + map_off(p.cm, i) + map_off(p.cn, j);
+        v *= p.alpha;
+        if (p.accumulate) v += *c;
+        *c = v;
+    }
 }
 
 bool single_unit(const Map4 &m) { return m.n0 == TATRG_RADIX_INF && m.s0 == 1; }
@@ -233,7 +244,7 @@ void launch_dot(const GemmParams &p)
     double *partial = ws_doubles((long long)grid * p.M * p.N);
     ts_dot_kernel<F><<<grid, TS_NT, smem, stream()>>>(p, partial);
     TATRG_LAUNCH_CHECK();
-    ts_dot_reduce_kernel<<<(p.M * p.N + 255) / 256, 256, 0, stream()>>>(p, partial, grid);
+    ts_dot_reduce_kernel<<<(p.M * p.N + 31) / 32, 1024, 0, stream()>>>(p, partial, grid);
     TATRG_LAUNCH_CHECK();
     count_launch(2);
     ws_release(mark);
