@@ -188,3 +188,40 @@ def test_order_parameter_matches_oracle(tt):
         for leg in range(4):
             xo, xg = orc.order_parameter_X(st, leg), tt.order_parameter(leg + 1)
             assert abs(xg / xo - 1) < 1e-9, (m, leg, xg, xo)
+
+
+def test_errors_leave_the_state_intact(tt):
+    """include/tatrg.h: errors never abort; a failed coarse_grain leaves the previous state in place."""
+    import paper_2412_14104_b200 as t
+    tt.init_ising_tensor(1 / 6.0, 0.0)
+    tt.coarse_grain(1, 6, 2, 2, 1)
+    tt.coarse_grain(2, 6, 2, 2, 1)
+    before, dims = tt.log_Z_per_site(), tt.get_dims()
+    for args in ((0, 6, 2, 2, 1), (5, 6, 2, 2, 1), (1, 0, 2, 2, 1), (1, 6, 0, 2, 1), (1, 6, 2, -1, 1), (1, 65, 2, 2, 1),
+                 (1, 64, 3, 2, 1)):
+        with pytest.raises(t.TatrgError):
+            tt.coarse_grain(*args)
+    with pytest.raises(t.TatrgError):
+        tt.init_ising_tensor(-1.0, 0.0)
+    assert tt.log_Z_per_site() == before and tt.get_dims() == dims
+    # a workspace that cannot hold some step: that step fails with a TatrgError and the state of the
+    # step before is still there
+    import torch
+    small = torch.empty(1 << 17, dtype=torch.float64, device="cuda")     # 1 MB
+    t._check(t.lib().tatrg_set_workspace(small.data_ptr(), small.numel() * 8))
+    try:
+        tt.init_ising_tensor(1 / 6.0, 0.0)
+        failed_at = None
+        for m in range(8):
+            before, dims = tt.log_Z_per_site(), tt.get_dims()
+            try:
+                tt.coarse_grain(m % 4 + 1, 16, 2, 2, 1)
+            except t.TatrgError as e:
+                failed_at = m
+                assert "workspace" in str(e)
+                break
+        assert failed_at is not None and failed_at >= 1
+        assert tt.log_Z_per_site() == before and tt.get_dims() == dims
+    finally:
+        tt.set_workspace(nbytes=8 << 30)
+        tt.init_ising_tensor(1 / 6.0, 0.0)
