@@ -468,6 +468,7 @@ def run_ours(args, cfg, name):
 
 # ------------------------------------------------------------------------------ kernel micro-benchmark
 GEMM_SHAPES = {   # the c3 (chi=32, r=2) contraction shapes of SURVEY.md 8(a), plain row-major operands
+    "a6_i_EM=E.M4": (65536, 1024, 32),
     "a6_ii_P=EM.F": (65536, 2048, 1024),
     "a6_iv_Phi=P.Q": (32768, 1024, 4096),
     "a2_G1_Z=D.w": (1024, 2048, 32768),

@@ -325,18 +325,21 @@ void tensor_gemm(GemmParams p)
     p.ktiles_per_split = ktiles;
     p.partial = nullptr;
     size_t mark = ws_mark();
-    // split-K: the number of splits that fills whole waves of resident CTAs best (fewer on ties)
+    // split-K: the number of splits that minimises a simple cost model, in units of one k tile of 16:
+    // waves of resident CTAs x (k tiles per CTA + a fixed per-CTA cost for the pipeline fill and the
+    // epilogue) + the second pass over the partial sums
     const long long slots = (long long)g_num_sms * (big ? 1 : mid ? 2 : 3);
-    if (tiles < 4 * slots && max_split > 1) {
-        auto eff = [&](int ks) {
-            const double x = (double)tiles * ks / (double)slots;
-            return (x < 1.0 ? x : x / ceil(x)) - 0.0005 * ks;   // machine fill, then whole waves
+    if (max_split > 1) {
+        const double fixed = 4.0, reduce_per_split = (double)p.M * p.N * p.batch / 2.0e6;
+        auto cost = [&](int ks) {
+            const double waves = ceil((double)tiles * ks / (double)slots);
+            return waves * (ceil((double)ktiles / ks) + fixed) + (ks > 1 ? ks * reduce_per_split + 2.0 : 0.0);
         };
         int ks = 1;
-        double best = eff(1);
+        double best = cost(1);
         for (int c = 2; c <= max_split; ++c) {
-            const double e = eff(c);
-            if (e > best * 1.08) {
+            const double e = cost(c);
+            if (e < best * 0.97) {
                 best = e;
                 ks = c;
             }
