@@ -528,6 +528,7 @@ void tatrg_destroy(void)
     if (c.side_ok) {
         for (auto &st : c.side) cudaStreamDestroy(st);
         for (auto &e : c.join_ev) cudaEventDestroy(e);
+        for (auto &e : c.dep_ev) cudaEventDestroy(e);
         cudaEventDestroy(c.fork_ev);
     }
     if (c.copy_stream) {

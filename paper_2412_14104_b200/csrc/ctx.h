@@ -34,9 +34,9 @@ struct Ctx {
     // independent chains of small kernels (the three squeezers, the four isometries) run on side
     // streams forked from / joined to `stream` with events; each chain bump-allocates from its own
     // slice of the free workspace (step.cpp: Fork)
-    static constexpr int MAX_CHAINS = 4;
+    static constexpr int MAX_CHAINS = 8;
     cudaStream_t side[MAX_CHAINS] = {};
-    cudaEvent_t fork_ev = nullptr, join_ev[MAX_CHAINS] = {};
+    cudaEvent_t fork_ev = nullptr, join_ev[MAX_CHAINS] = {}, dep_ev[MAX_CHAINS] = {};
     bool side_ok = false;
     char *pinned = nullptr;                 // page-locked host scratch for asynchronous read-backs
     static constexpr size_t PINNED_BYTES = 1 << 16;

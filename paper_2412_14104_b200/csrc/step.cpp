@@ -94,27 +94,46 @@ Ten gauge_rotation(const Ten &P, const std::vector<double> &s, int k)
 // outlive the join are allocated on the main stream before the Fork is constructed.
 class Fork {
 public:
-    explicit Fork(int n) : c_(ctx()), n_(n), main_(c_.stream), lo0_(c_.lo), hi0_(c_.hi)
+    // main_slice: the main stream keeps a slice of the workspace too and goes on enqueuing while forked
+    // (ordering with the chains through side_after_main / main_after_side)
+    explicit Fork(int n, bool main_slice = false) : c_(ctx()), n_(n), main_(c_.stream), lo0_(c_.lo), hi0_(c_.hi)
     {
         if (n < 1 || n > Ctx::MAX_CHAINS) fail(-22, "Fork: %d chains", n);
         if (!c_.side_ok) {
             for (auto &st : c_.side) TATRG_CUDA_CHECK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
             for (auto &e : c_.join_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            for (auto &e : c_.dep_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
             TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&c_.fork_ev, cudaEventDisableTiming));
             c_.side_ok = true;
         }
         if (!c_.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c_.pinned, Ctx::PINNED_BYTES));
         TATRG_CUDA_CHECK(cudaEventRecord(c_.fork_ev, main_));
-        const size_t slice = ((hi0_ - lo0_) / n) & ~(size_t)255;
+        const size_t slice = ((hi0_ - lo0_) / (n + (main_slice ? 1 : 0))) & ~(size_t)255;
         for (int i = 0; i < n; ++i) {
             TATRG_CUDA_CHECK(cudaStreamWaitEvent(c_.side[i], c_.fork_ev, 0));
-            lo_[i] = lo0_ + i * slice;
+            lo_[i] = lo0_ + (i + (main_slice ? 1 : 0)) * slice;
             hi_[i] = lo_[i] + slice;
         }
-        c_.lo = c_.hi = hi0_;   // nothing is allocated on the main stream while forked
+        main_lo_ = main_slice ? lo0_ : hi0_;   // without a slice nothing is allocated on the main stream while forked
+        main_hi_ = main_slice ? lo0_ + slice : hi0_;
+        c_.lo = main_lo_;
+        c_.hi = main_hi_;
+    }
+    // chain i continues only after everything enqueued on the main stream so far
+    void side_after_main(int i)
+    {
+        TATRG_CUDA_CHECK(cudaEventRecord(c_.dep_ev[i], main_));
+        TATRG_CUDA_CHECK(cudaStreamWaitEvent(c_.side[i], c_.dep_ev[i], 0));
+    }
+    // the main stream continues only after everything enqueued on chain i so far
+    void main_after_side(int i)
+    {
+        TATRG_CUDA_CHECK(cudaEventRecord(c_.join_ev[i], c_.side[i]));
+        TATRG_CUDA_CHECK(cudaStreamWaitEvent(main_, c_.join_ev[i], 0));
     }
     void enter(int i)
     {
+        if (cur_ < 0) main_lo_ = c_.lo;
         cur_ = i;
         c_.stream = c_.side[i];
         c_.lo = lo_[i];
@@ -127,7 +146,8 @@ public:
         c_.peak = std::max(c_.peak, c_.lo + (c_.ws_bytes - hi0_));
         cur_ = -1;
         c_.stream = main_;
-        c_.lo = c_.hi = hi0_;
+        c_.lo = main_lo_;
+        c_.hi = main_hi_;
     }
     void sync(int i) { TATRG_CUDA_CHECK(cudaStreamSynchronize(c_.side[i])); }
     // page-locked host scratch of chain i (PINNED_BYTES / MAX_CHAINS bytes)
@@ -157,6 +177,7 @@ private:
     cudaStream_t main_;
     size_t lo0_, hi0_;
     size_t lo_[Ctx::MAX_CHAINS], hi_[Ctx::MAX_CHAINS];
+    size_t main_lo_ = 0, main_hi_ = 0;
     int cur_ = -1;
     bool joined_ = false;
 };
@@ -404,18 +425,25 @@ struct SqChain {
         // a failed factorisation / Jacobi, or a block too ill conditioned for two Cholesky-QR passes
         return back->flag == 0 && back->ratio[0] > 1e-5 * back->ratio[1] && back->ratio[2] > 1e-5 * back->ratio[3];
     }
-    void phaseA(char *pinned)
+    // on the main stream, before any fork: the buffers of the two Cholesky factors
+    void prep()
     {
-        back = reinterpret_cast<Back *>(pinned);
         LL = ws_tensor("ki", {N2, N2});
         LR = ws_tensor("kj", {N2, N2});
         d2d(LL.p, GLm.p, (long long)N2 * N2);
         d2d(LR.p, GRm.p, (long long)N2 * N2);
         flag = (int *)ws_alloc(sizeof(int));
         TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    }
+    // the two factorisations G^L + delta = L_L L_L^T, G^R + delta = L_R L_R^T: independent chains
+    void factor(int which)
+    {
         const double shift = 3e-14;
-        cholesky_lower_async(LL.p, N2, shift, nullptr, flag);
-        cholesky_lower_async(LR.p, N2, shift, nullptr, flag);
+        cholesky_lower_async(which == 0 ? LL.p : LR.p, N2, shift, nullptr, flag);
+    }
+    void phaseA(char *pinned)
+    {
+        back = reinterpret_cast<Back *>(pinned);
         F = ws_tensor("ij", {N2, N2});
         contract(LL, LR, F);                               // F = L_L^T L_R
         ratio = ws_doubles(4);
@@ -497,13 +525,15 @@ struct RedBasis {
     Ten L2inv;   // [k,l] lower triangular: Q = Q1 L2inv^T
 };
 
-// Two phases: phase 1 enqueues everything up to |G2 - I| and its read-back, phase 2 (after the host has
-// looked at it) the second factor and R.
+// One tensor's factorisation in three pieces, so that the two Cholesky factorisations (latency-bound,
+// a few CTAs) run on side streams under the machine-filling GEMMs of the main stream.
 struct OrthoChain {
     Ten T;
     RedBasis o;
     long long nk = 0;
-    Ten G1, G2;
+    Ten G1, G2, L1inv;
+    int *flag = nullptr;
+    double *dev = nullptr;
     struct Back {
         int flag;
         int pad;
@@ -511,34 +541,33 @@ struct OrthoChain {
     } *back = nullptr;
     double err = INFINITY;
 
-    void alloc(const Ten &T_)   // on the main stream: what outlives the fork
+    void alloc(const Ten &T_, char *pinned)   // on the main stream, before the fork
     {
         T = T_;
+        back = reinterpret_cast<Back *>(pinned);
         const long long n0 = T.legs[0].n, n1 = T.legs[1].n, n2 = T.legs[2].n, n3 = T.legs[3].n, a = T.legs[4].n;
         nk = n0 * a;
         o.Q1 = ws_tensor("pqtk", {n1, n2, n3, nk});
         o.R = ws_tensor("kcb", {nk, n0, a});
         o.L2inv = ws_tensor("kl", {nk, nk});
-    }
-    void phase1(char *pinned)
-    {
-        back = reinterpret_cast<Back *>(pinned);
-        const long long n0 = T.legs[0].n, a = T.legs[4].n;
-        int *flag = (int *)ws_alloc(sizeof(int));
-        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
         G1 = ws_tensor("cbde", {n0, a, n0, a});
-        Ten L1inv = ws_tensor("kcb", {nk, n0, a});
-        contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true);
-        cholesky_lower_async(G1.p, (int)nk, 0.0, L1inv.p, flag);
-        contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
         G2 = ws_tensor("kl", {nk, nk});
+        L1inv = ws_tensor("kcb", {nk, n0, a});
+        flag = (int *)ws_alloc(sizeof(int));
+        dev = ws_doubles(1);
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+    }
+    void gram1() { contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true); }              // main
+    void factor1() { cholesky_lower_async(G1.p, (int)nk, 0.0, L1inv.p, flag); }                 // side
+    void basis()                                                                                 // main
+    {
+        contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
         contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
-        double *dev = ws_doubles(1);
         max_dev_identity(G2.p, (int)nk, dev);
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->err, dev, sizeof(double), cudaMemcpyDeviceToHost, stream()));
     }
-    bool usable()   // after the chain's stream has been synchronised
+    bool usable()   // after the main stream has been synchronised
     {
         err = back->err;
         return back->flag == 0 && err < 0.05;
@@ -556,25 +585,34 @@ struct OrthoChain {
 };
 
 // Both bases of the reduced bond swap; false when either matricisation is rank deficient or too
-// ill conditioned for two Cholesky-QR passes (|G2 - I| > 0.05).  One after the other on the caller's
-// stream: the work is dominated by machine-filling GEMMs, which gain nothing from overlapping (and
-// whose per-launch timing would be blurred by it).
+// ill conditioned for two Cholesky-QR passes (|G2 - I| > 0.05).
+// Main stream: G1_A, G1_D, Q1_A, G2_A, Q1_D, G2_D; side streams: chol(G1_A) under G1_D, chol(G1_D) under Q1_A.
 bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
 {
     Ctx &c = ctx();
     if (!c.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c.pinned, Ctx::PINNED_BYTES));
     OrthoChain ch[2];
-    ch[0].alloc(A);
-    ch[1].alloc(D);
+    ch[0].alloc(A, c.pinned);
+    ch[1].alloc(D, c.pinned + 64);
     if (ch[0].nk > 0x7fffffff) return false;
-    bool ok = true;
-    for (int i = 0; i < 2 && ok; ++i) {
-        size_t mk = ws_mark();
-        ch[i].phase1(c.pinned);
-        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
-        ok = ch[i].usable() && ch[i].phase2();
-        ws_release(mk);
+    {
+        Fork fk(2, true);
+        for (int i = 0; i < 2; ++i) {
+            ch[i].gram1();
+            fk.side_after_main(i);
+            fk.enter(i);
+            ch[i].factor1();
+            fk.leave();
+        }
+        for (int i = 0; i < 2; ++i) {
+            fk.main_after_side(i);
+            ch[i].basis();
+        }
+        fk.join();
     }
+    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    bool ok = ch[0].usable() && ch[1].usable();
+    for (int i = 0; i < 2 && ok; ++i) ok = ch[i].phase2();
     bA = ch[0].o;
     bD = ch[1].o;
     return ok;
@@ -1171,6 +1209,18 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             nact += ch[mu].active;
         }
         if (nact > 0) {
+            for (int mu = 0; mu < 3; ++mu)
+                if (ch[mu].active) ch[mu].prep();
+            {   // six Cholesky factorisations side by side
+                Fork fk6(6);
+                for (int mu = 0; mu < 3; ++mu)
+                    for (int w = 0; w < 2 && ch[mu].active; ++w) {
+                        fk6.enter(2 * mu + w);
+                        ch[mu].factor(w);
+                        fk6.leave();
+                    }
+                fk6.join();
+            }
             Fork fk(3);
             for (int mu = 0; mu < 3; ++mu)
                 if (ch[mu].active) {
