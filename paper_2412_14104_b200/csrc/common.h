@@ -115,7 +115,8 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
 // jacobi_small.cu : one-CTA versions for m, n <= 64 (same output conventions)
 void svd_small(double *G, int m, int n, double *V, double *s);
 // without host synchronisation: no convergence within the sweep limit raises *flag_dev (sticky, device)
-void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev);
+// tol_override > 0: convergence threshold on the column cosines (default: a few eps), for estimates
+void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev, double tol_override = 0.0);
 void eig_small_async(const double *S, int n, double *V, double *lam, int *flag_dev);
 void eig_small(const double *S, int n, double *V, double *lam);   // symmetric S; V column j = eigenvector j
 // reduce.cu

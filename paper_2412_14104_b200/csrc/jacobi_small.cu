@@ -278,12 +278,12 @@ void set_attr()
 
 }  // namespace
 
-void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev)
+void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_dev, double tol_override)
 {
     if (m > SJ_MAX || n > SJ_MAX || m < 1 || n < 1) fail(-22, "svd_small: size %d x %d not supported", m, n);
     set_attr();
     const int mn = m > n ? m : n;
-    const double tol = 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
+    const double tol = tol_override > 0.0 ? tol_override : 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
     const size_t smem = (size_t)n * (m + n) * sizeof(double);
     svd_small_kernel<<<1, SJ_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag_dev);
     TATRG_LAUNCH_CHECK();

@@ -406,12 +406,13 @@ struct SqChain {
     }
     // Ritz step on the current Q (two Cholesky-QR passes have just been applied to it):
     // B^T = F^T Q = Q_B R_B, R_B^T V = U diag(s); read-back of flag, condition estimates, s
-    void enqueue_ritz()
+    // estimate: only the singular values are wanted, to two or three digits (iteration count)
+    void enqueue_ritz(bool estimate = false)
     {
         mulFt(Q, Qt);
         cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
         if (b <= 64)
-            svd_small_async(Rb, b, b, V, sv, flag);
+            svd_small_async(Rb, b, b, V, sv, flag, estimate ? 1e-4 : 0.0);
         else
             jacobi_svd(Rb, b, b, V, sv, 1, 0, 0, 0);       // multi-launch Jacobi (synchronises this chain)
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
@@ -463,7 +464,7 @@ struct SqChain {
             mulF(Qt, Q);
             cholqr_async(Q, N2, b, it == 1 ? 2 : 1, it == 1 ? 0.0 : it_shift, flag, it == 1 ? ratio : nullptr, nullptr);
         }
-        enqueue_ritz();
+        enqueue_ritz(true);
     }
     // iteration count from the measured decay rho = s_b / s_chi: rho^(2p+1) < 1e-13
     bool plan()
