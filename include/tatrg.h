@@ -134,6 +134,12 @@ double tatrg_probe_fp64_peak(int mode, int iters);
 int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N, int K, int batch,
                       const int64_t *maps, double alpha, int accumulate);
 
+/* out (device, n doubles) <- the seeded N(0,1) stream (seed, step, which) of the input recipe
+ * (the device implementation of the generator of seeded_inputs/, which the
+ * library uses for every input the caller did not supply with tatrg_set_sketch).  Equal to the host
+ * generator's values up to the last-bit differences of log / sincos. */
+int tatrg_fill_gauss(double *out, uint64_t n, uint64_t seed, uint64_t step, uint64_t which);
+
 /* Thin QR with R_ii >= 0 of the row-major m x n matrix Y (device; m >= n, n <= 64): Q overwrites
  * Y, R (n x n row-major upper triangular) goes to R (device).  The "QR decomposition in the RSVD"
  * of PAPER.md:106 / the canonical form of PAPER.md:37 (Householder TSQR, robust to rank deficiency). */

@@ -24,7 +24,7 @@ EXPORTS = [
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
-    "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
+    "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
     "tatrg_last_error", "tatrg_destroy",
 ]
 
@@ -74,6 +74,7 @@ def lib():
             "tatrg_gemm_flops": (c_d, [c_i]),
             "tatrg_probe_fp64_peak": (c_d, [c_i, c_i]),
             "tatrg_tensor_gemm": (c_i, [c_vp, c_vp, c_vp, c_i, c_i, c_i, c_i, c_vp, c_d, c_i]),
+            "tatrg_fill_gauss": (c_i, [c_vp, c_u64, c_u64, c_u64, c_u64]),
             "tatrg_qr_pos": (c_i, [c_vp, c_i64, c_i, c_vp]),
             "tatrg_cholesky": (c_i, [c_vp, c_i, c_d, c_vp]),
             "tatrg_cholqr": (c_i, [c_vp, c_i64, c_i, c_i, c_d, c_vp]),
@@ -277,6 +278,12 @@ def tensor_gemm(A, B, C, M, N, K, maps, batch=1, alpha=1.0, accumulate=False):
     arr = np.asarray(flat, dtype=np.int64)
     _check(lib().tatrg_tensor_gemm(A.data_ptr(), B.data_ptr(), C.data_ptr(), int(M), int(N), int(K),
                                    int(batch), arr.ctypes.data, float(alpha), int(accumulate)))
+
+
+def fill_gauss(out, seed: int, step: int, which: int):
+    """out (CUDA float64 tensor) <- the seeded N(0,1) stream (seed, step, which), generated on the device."""
+    _require_cuda()
+    _check(lib().tatrg_fill_gauss(out.data_ptr(), out.numel(), int(seed), int(step), int(which)))
 
 
 def qr_pos(Y, R):

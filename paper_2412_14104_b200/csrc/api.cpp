@@ -452,6 +452,16 @@ int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N,
     });
 }
 
+extern "C" uint64_t si_subseed(uint64_t seed, uint64_t step, uint64_t which);
+
+int tatrg_fill_gauss(double *out, uint64_t n, uint64_t seed, uint64_t step, uint64_t which)
+{
+    return guarded([&] {
+        if (!out && n) fail(TATRG_EINVAL, "tatrg_fill_gauss: null pointer");
+        device_fill_gauss(out, n, si_subseed(seed, step, which));
+    });
+}
+
 int tatrg_qr_pos(double *Y, int64_t m, int n, double *R)
 {
     return guarded([&] {
@@ -536,8 +546,6 @@ void tatrg_destroy(void)
         for (auto &e : c.pre_ev) cudaEventDestroy(e);
     }
     if (c.pinned) cudaFreeHost(c.pinned);
-    for (auto &b : c.start_blk)
-        if (b) cudaFreeHost(b);
     c = Ctx();
 }
 

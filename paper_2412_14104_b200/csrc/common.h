@@ -144,6 +144,8 @@ void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full,
 void near_identity_chol(double *G, int n, double *Linv);
 void diag_minmax(const double *L, int n, double *out);   // out[0..1] = min, max of diag(L), L n x n row-major
 void chol_block(double *A, long long lda, int n, double *Linv, int *flag, double *dminmax, double shift_rel = 0.0);
+// rng.cu : out[0..n) = the seeded N(0,1) stream `subseed` (the recipe of seeded_inputs/), generated on the device
+void device_fill_gauss(double *out, unsigned long long n, unsigned long long subseed);
 // gauge.cu
 void cluster_qr(const double *P, int ldp, double *W, int n, const int *bounds_dev, int nclusters);
 

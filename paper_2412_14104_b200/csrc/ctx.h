@@ -40,8 +40,6 @@ struct Ctx {
     bool side_ok = false;
     char *pinned = nullptr;                 // page-locked host scratch for asynchronous read-backs
     static constexpr size_t PINNED_BYTES = 1 << 16;
-    double *start_blk[4] = {};              // page-locked start blocks of the iterative solvers
-    long long start_blk_n[4] = {};
 
     // host-resident inputs of a step are uploaded by a copy stream from the start of the step on
     // (step.cpp: prefetch_inputs), overlapping the canonical form; get_input waits for the event

@@ -233,12 +233,9 @@ Ten get_input(int which, long long rows, long long cols, const StepCfg &cfg, con
         }
         return t;
     }
-    std::vector<double> host((size_t)n);
-    uint64_t st = (which >= 5) ? 0 : (uint64_t)cfg.step;   // gauge references are step independent
-    si_fill_gauss(host.data(), (uint64_t)n, si_subseed(cfg.seed, st, (uint64_t)which), 0);
+    const uint64_t st = (which >= 5) ? 0 : (uint64_t)cfg.step;   // gauge references are step independent
     t = ws_tensor(names2, {rows, cols});
-    h2d(t.p, host.data(), n);
-    TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    device_fill_gauss(t.p, (unsigned long long)n, si_subseed(cfg.seed, st, (uint64_t)which));
     return t;
 }
 
@@ -349,19 +346,8 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
 // convergence, so the result does not depend on it beyond rounding).
 Ten solver_start_block(long long rows, long long cols, int tag, const char *names2)
 {
-    Ctx &c = ctx();
-    if (tag < 0 || tag >= 4) fail(-22, "solver_start_block: tag %d", tag);
-    const long long n = rows * cols;
-    if (c.start_blk_n[tag] != n) {   // page-locked host cache: the upload below is then truly asynchronous
-        if (c.start_blk[tag]) cudaFreeHost(c.start_blk[tag]);
-        c.start_blk[tag] = nullptr;
-        c.start_blk_n[tag] = 0;
-        TATRG_CUDA_CHECK(cudaMallocHost((void **)&c.start_blk[tag], sizeof(double) * n));
-        si_fill_gauss(c.start_blk[tag], (uint64_t)n, si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag), 0);
-        c.start_blk_n[tag] = n;
-    }
     Ten t = ws_tensor(names2, {rows, cols});
-    h2d(t.p, c.start_blk[tag], n);
+    device_fill_gauss(t.p, (unsigned long long)(rows * cols), si_subseed(0x7a7e6ULL, 0, 100 + (uint64_t)tag));
     return t;
 }
 

@@ -249,3 +249,18 @@ def test_tensor_gemm_tall_skinny_streaming(tt, M, N, K):
         tt.tensor_gemm(dAt, dB, dC2, M, N, K, maps2, alpha=0.5, accumulate=True)
         torch.cuda.synchronize()
         np.testing.assert_allclose(dC2.cpu().numpy(), 1.0 + 0.5 * (A @ B), rtol=0, atol=1e-11 * np.sqrt(K))
+
+
+@pytest.mark.parametrize("n", [1, 2, 7, 100001])
+def test_device_generator_equals_host_generator(tt, n):
+    """The library's device implementation of the seeded Gaussian recipe against the shared host module
+    (what the oracle draws from): same values up to last-bit differences of log / sincos."""
+    import torch
+    import seeded_inputs as si
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    tt.fill_gauss(out, 20241216, 11, 3)
+    ref = si.gauss(si.subseed(20241216, 11, 3), n)
+    got = out.cpu().numpy()
+    assert np.abs(got - ref).max() <= 4e-15
+    if n > 1000:
+        assert abs(got.mean()) < 0.02 and abs(got.std() - 1.0) < 0.02

