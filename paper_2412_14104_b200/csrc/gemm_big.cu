@@ -7,8 +7,8 @@
 //
 // 128x128: 16 warps, warp tile 32 x 32 (32 FP64 accumulators per thread), BK = 32, 3-stage cp.async
 // pipeline synchronised by per-stage mbarriers ("full": the copies of all threads have landed, "empty":
-// all threads are done reading) instead of a CTA-wide barrier per k tile.  128x64: 4 warps, warp tile
-// 32 x 64, BK = 16, 4 stages, __syncthreads.
+// all threads are done reading) instead of a CTA-wide barrier per k tile.  128x64: 8 warps, warp tile
+// 32 x 32, BK = 16, 3 stages, the same mbarrier pipeline, two CTAs per SM.
 // The shared-memory layout of an operand tile follows the operand's contiguous index in global
 // memory, so that 16-byte cp.async copies land on 16 consecutive bytes of shared memory:
 //   contiguous index = the free index (m or n):  tile stored [k][m], leading dimension 128 + 4
@@ -386,7 +386,7 @@ void tensor_gemm_big(const GemmParams &p, int bn)
     // TATRG_GEMM_SYNC selects the __syncthreads pipeline for comparison
     static const bool sync = getenv("TATRG_GEMM_SYNC") != nullptr;
     if (bn == 64)
-        dispatch_big<64, 64, 16, 4, false>(p);
+        dispatch_big<64, 32, 16, 3, true>(p);
     else if (wn64)
         dispatch_big<128, 64, 16, 4, false>(p);
     else if (bk16)
