@@ -310,9 +310,12 @@ void tensor_gemm(GemmParams p)
     const int max_split = ktiles / 8 < 512 ? ktiles / 8 : 512;
     bool big = p.M >= 96 && p.N >= 96 &&
                (big_tiles * 5 >= 4LL * g_num_sms || big_tiles * (long long)(max_split > 1 ? max_split : 1) >= 2LL * g_num_sms);
-    const bool mid = !big && p.N <= 64 && p.N >= 17 && p.M >= 96;
+    // a short summed index (one or two k tiles) never fills the pipeline: two co-resident 128x64 CTAs per
+    // SM hide each other's load and store phases (measured 0.37 -> 0.30 ms on the K = 32 product E M^(4))
+    if (big && p.K <= 64) big = false;
+    const bool mid = !big && p.N >= 17 && p.M >= 96 && (p.N <= 64 || p.K <= 64);
     long long tiles = big ? big_tiles
-                          : mid ? (long long)((p.M + 127) / 128) * p.batch
+                          : mid ? (long long)((p.M + 127) / 128) * ((p.N + 63) / 64) * p.batch
                                 : (long long)((p.M + 63) / 64) * ((p.N + 63) / 64) * p.batch;
     if (p.lower_only) {   // only the tiles that touch the lower triangle do work
         const int bm = (big || mid) ? 128 : 64, bn = big ? 128 : 64;
