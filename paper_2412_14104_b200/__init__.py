@@ -215,6 +215,27 @@ def order_parameter(leg: int = 4) -> float:
     return float(lib().tatrg_order_parameter(int(leg)))
 
 
+def critical_temperature(chi: int, r: int, q: int, seed: int, T_lo: float, T_hi: float, n_steps: int = 12,
+                         iters: int = 12, h: float = 0.0, leg: int = 4) -> float:
+    """T_c by bisection on the order parameter X^(m) (Fig. 7): X -> 2 in the ordered
+    phase (two degenerate ground states), X -> 1 in the disordered one; the bracket [T_lo, T_hi] is halved
+    `iters` times on X(T) >< 1.5 after n_steps coarse-graining steps (directions cycling 1..4).  Host loop
+    over the three calls of the path; every temperature is an independent run (replicas across GPUs).
+    At h = 0 nothing protects the Z2 symmetry numerically: after ~16-20 steps rounding selects one of the two
+    ordered states and X drops to 1 on the ordered side too, so X is read on its plateau (n_steps = 12-16)."""
+    lo, hi = float(T_lo), float(T_hi)
+    for _ in range(iters):
+        T = 0.5 * (lo + hi)
+        init_ising_tensor(1.0 / T, h)
+        for m in range(n_steps):
+            coarse_grain(m % 4 + 1, chi, r, q, seed)
+        if order_parameter(leg) > 1.5:
+            lo = T          # still ordered: T_c is above
+        else:
+            hi = T
+    return 0.5 * (lo + hi)
+
+
 def stage_ms() -> dict:
     out = np.zeros(16)
     n = lib().tatrg_get_stage_ms(out.ctypes.data, out.size)

@@ -231,3 +231,10 @@ def test_errors_leave_the_state_intact(tt):
     finally:
         tt.set_workspace(nbytes=8 << 30)
         tt.init_ising_tensor(1 / 6.0, 0.0)
+
+
+def test_critical_temperature_bisection(tt):
+    """SURVEY 8(f) NEXT-1 / PAPER.md Fig. 7: bisection on X^(m).  At chi = 8 the estimate is crude (the paper
+    needs chi ~ 50 for 0.1 %); it must land in the neighbourhood of the Monte Carlo value T_c = 6.68."""
+    Tc = tt.critical_temperature(chi=8, r=2, q=2, seed=5, T_lo=5.0, T_hi=8.5, n_steps=12, iters=8)
+    assert 6.4 < Tc < 7.2, Tc
