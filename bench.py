@@ -595,6 +595,7 @@ def main():
                     help="time every tensor-GEMM launch (default: only the dominant 128x128-tile kernel)")
     ap.add_argument("--gemm", default=None, help="kernel micro-benchmark: 'all' or one of " + ", ".join(GEMM_SHAPES))
     ap.add_argument("--small", action="store_true", help="micro-benchmark of the small latency-bound solvers")
+    ap.add_argument("--chi", type=int, default=None, help="override the bond dimension of the chosen config (scaling study)")
     args = ap.parse_args()
     if args.small:
         run_small_micro(args)
@@ -602,7 +603,9 @@ def main():
     if args.gemm:
         run_gemm_micro(args)
         return
-    cfg = CONFIGS[args.config]
+    cfg = dict(CONFIGS[args.config])
+    if args.chi:
+        cfg["chi"] = args.chi
     if args.impl == "reference":
         run_reference(args, cfg, args.config)
         return
