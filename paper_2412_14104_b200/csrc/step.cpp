@@ -10,6 +10,7 @@
 //   t / T  lone leg upper / lower   a,b  canonical bonds alpha, beta   g,d  swap bond gamma
 //   k,l  oversampled internal lines (r chi)   m,n,w  renormalised legs   z  sketch columns
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -557,6 +558,7 @@ struct OrthoChain {
     bool usable()   // after the main stream has been synchronised
     {
         err = back->err;
+        if (getenv("TATRG_TRACE")) fprintf(stderr, "tatrg-trace ortho: nk %lld |G2 - I| = %.3e flag %d\n", nk, err, back->flag);
         return back->flag == 0 && err < 0.05;
     }
     bool phase2()
