@@ -10,11 +10,17 @@
  * the output is the free energy.
  *
  * Conventions
- *   - One process-global context; not thread safe.  All device work is enqueued on the
- *     stream given by tatrg_set_stream (default: the legacy default stream).
+ *   - One process-global context; not thread safe.  The step is enqueued on the stream given
+ *     by tatrg_set_stream (default: the legacy default stream); inside coarse_grain the library
+ *     forks independent chains of small kernels (squeezers, isometries, factorisations) and the
+ *     upload of host-resident inputs onto non-blocking streams of its own and joins them back
+ *     with events, so everything a call enqueues is ordered before whatever the caller enqueues
+ *     on its stream afterwards.
  *   - The library allocates no device memory: every device buffer lives in the workspace
  *     the caller passes to tatrg_set_workspace (e.g. a torch tensor).  The caller keeps it
- *     alive and unchanged until tatrg_destroy or the next tatrg_set_workspace.
+ *     alive and unchanged until tatrg_destroy or the next tatrg_set_workspace.  What the library
+ *     owns (released by tatrg_destroy): its side streams and events, 64 KB of page-locked host
+ *     memory for asynchronous read-backs.
  *   - Status: 0 = OK, negative = error, message via tatrg_last_error().  Errors never abort
  *     the process.  A failed coarse_grain leaves the renormalised tensor (Phi, Psi), the
  *     step count and the ln Z accumulator of the previous step intact.

@@ -1392,6 +1392,9 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     std::vector<double> nv = d2h(ss, 2);
     stage_mark(8);
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    // an uploaded input that no stage consumed (wrong shape for this step) may still be in flight:
+    // the caller's host buffers are read during the call only
+    if (c.copy_stream) TATRG_CUDA_CHECK(cudaStreamSynchronize(c.copy_stream));
     if (!(nv[0] > 0) || !(nv[1] > 0) || !std::isfinite(nv[0]) || !std::isfinite(nv[1]))
         fail(-34, "coarse_grain: non-finite or zero norm of the renormalised tensor");
     // ---- commit
