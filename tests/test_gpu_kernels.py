@@ -264,3 +264,41 @@ def test_device_generator_equals_host_generator(tt, n):
     assert np.abs(got - ref).max() <= 4e-15
     if n > 1000:
         assert abs(got.mean()) < 0.02 and abs(got.std() - 1.0) < 0.02
+
+
+def test_tensor_gemm_randomised_shapes_and_layouts(tt):
+    """Seeded sweep over shapes (ragged tails, all three CTA tiles, split-K, short and long summed index) and
+    operand layouts (either index of A, B contiguous; odd leading dimensions defeat the 16-byte copies)."""
+    import torch
+    rng = np.random.default_rng(20241104)
+    sizes_mn = [1, 5, 17, 33, 64, 65, 96, 130, 257, 520, 1030]
+    sizes_k = [1, 3, 16, 31, 33, 64, 100, 257, 1025, 4100]
+    for case in range(60):
+        M, N, K = int(rng.choice(sizes_mn)), int(rng.choice(sizes_mn)), int(rng.choice(sizes_k))
+        if case % 10 == 0:
+            M, N, K = int(rng.choice([2048, 3000])), int(rng.choice([40, 64, 200])), int(rng.choice([32, 64, 700]))
+        a_kfast, b_kfast = bool(rng.integers(2)), bool(rng.integers(2))
+        pad_a, pad_b = int(rng.integers(3)), int(rng.integers(3))
+        A, B = rng.standard_normal((M, K)), rng.standard_normal((K, N))
+        if a_kfast:                      # A stored [m][k] with leading dimension K + pad
+            bufA = np.zeros((M, K + pad_a)); bufA[:, :K] = A
+            am, ak = [(M, K + pad_a)], [(K, 1)]
+        else:                            # A stored [k][m]
+            bufA = np.zeros((K, M + pad_a)); bufA[:, :M] = A.T
+            am, ak = [(M, 1)], [(K, M + pad_a)]
+        if b_kfast:                      # B stored [n][k]
+            bufB = np.zeros((N, K + pad_b)); bufB[:, :K] = B.T
+            bk, bn = [(K, 1)], [(N, K + pad_b)]
+        else:                            # B stored [k][n]
+            bufB = np.zeros((K, N + pad_b)); bufB[:, :N] = B
+            bk, bn = [(K, N + pad_b)], [(N, 1)]
+        C0 = rng.standard_normal((M, N))
+        acc = bool(rng.integers(2))
+        alpha = float(rng.choice([1.0, -0.5]))
+        dA, dB, dC = _dev(bufA), _dev(bufB), _dev(C0)
+        maps = dict(am=am, ak=ak, bk=bk, bn=bn, cm=[(M, N)], cn=[(N, 1)])
+        tt.tensor_gemm(dA, dB, dC, M, N, K, maps, alpha=alpha, accumulate=acc)
+        torch.cuda.synchronize()
+        ref = alpha * (A @ B) + (C0 if acc else 0.0)
+        err = np.abs(dC.cpu().numpy() - ref).max()
+        assert err <= 1e-11 * np.sqrt(K) * 4, (case, M, N, K, a_kfast, b_kfast, pad_a, pad_b, acc, err)
