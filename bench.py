@@ -440,6 +440,8 @@ def run_ours(args, cfg, name):
                 "traffic": NCU_TRAFFIC["dram_bytes"],
                 "traffic_of": NCU_TRAFFIC,
                 "peak_source": "%s bf16_tflops_sustained x nominal FP64/bf16 ratio 45/2250" % how,
+                "peak_note": ("the bf16 figure is power-throttled (1.3 GHz), FP64 runs at 1965 MHz and ~450 W, so frac can "
+                              "exceed 1; the stricter denominator is the live register-resident DMMA probe: frac_of_probe"),
                 "peak_probe_dmma_tflops": probe, "peak_probe_dfma_tflops": probe_dfma,
                 "frac_of_probe": achieved / probe if probe > 0 else None,
                 "flops_per_launch": g_fl / g_n if g_n else 0.0, "avg_launch_ms": g_ms / g_n if g_n else 0.0,
