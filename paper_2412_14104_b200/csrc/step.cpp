@@ -996,10 +996,15 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 ratio = ws_doubles(16);
             }
             int nqr = 0;
-            auto orth = [&](double *Y) {
+            // last: the block that enters the Ritz step (two passes); before it only the span is carried on
+            auto orth = [&](double *Y, bool last) {
                 if (fast) {
-                    cholqr_async(Y, n12, kk, 2, 0.0, flag, ratio + 2 * nqr, nullptr);
-                    ++nqr;
+                    if (last) {
+                        cholqr_async(Y, n12, kk, 2, 0.0, flag, ratio + 2 * nqr, nullptr);
+                        ++nqr;
+                    } else {
+                        cholqr_async(Y, n12, kk, 1, 1e-13, flag, nullptr, nullptr);
+                    }
                 } else {
                     double *Rtmp = ws_doubles((long long)kk * kk);
                     tsqr(Y, n12, kk, Rtmp);
@@ -1008,11 +1013,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             Ten om = get_input(1 + i, n12, kk, cfg, "rz");
             Ten Qi = ws_tensor("rz", {n12, kk}), SQ = ws_tensor("ry", {n12, kk});
             S_op(om.p, Qi.p);
-            orth(Qi.p);
+            orth(Qi.p, q == 0);
             for (int it = 0; it < q; ++it) {
                 S_op(Qi.p, SQ.p);
                 d2d(Qi.p, SQ.p, n12 * kk);
-                orth(Qi.p);
+                orth(Qi.p, it == q - 1);
             }
             S_op(Qi.p, SQ.p);
             Ten Hm = ws_tensor("zy", {kk, kk});
