@@ -198,7 +198,6 @@ __global__ void __launch_bounds__(128 * BN / WN, BN == 128 ? 1 : 2) tgemm_big_ke
     constexpr int A_KK = A_KF ? 4 : 4 * LD_F;       // step between k groups of 4
     constexpr int B_KK = B_KF ? 4 : 4 * LD_FB;
 
-#pragma unroll
     // MBAR: every stage has a "full" barrier (all threads' copies of the tile have landed) and an
     // "empty" barrier (all threads are done reading it), so a warp only waits for data and for the
     // slot it refills -- never for the slowest warp of the current tile, as with the CTA-wide barrier.

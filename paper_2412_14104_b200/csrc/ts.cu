@@ -22,7 +22,7 @@ constexpr int TS_ROWS = 128;   // rows per tile of ts_apply
 constexpr int TD_ROWS = 64;    // rows per tile of ts_dot
 
 // ---------------------------------------------------------------------------------------
-template <int NH>   // outputs per thread: two threads share a row, each owns NH <= 32 of the N columns
+template <int NH>   // the N <= 2 NH columns are split over four threads; each thread owns two rows
 __global__ void __launch_bounds__(TS_NT) ts_apply_kernel(const __grid_constant__ GemmParams p)
 {
     extern __shared__ double sm[];
@@ -37,7 +37,6 @@ __global__ void __launch_bounds__(TS_NT) ts_apply_kernel(const __grid_constant__
         Ws[i] = (j < N) ? p.B[map_off(p.bk, c) + map_off(p.bn, j)] : 0.0;
     }
     const int tiles = (p.M + TS_ROWS - 1) / TS_ROWS;
-    const int r_loc = t & (TS_ROWS - 1), half = t / TS_ROWS;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
         const int r0 = tile * TS_ROWS;
         __syncthreads();
@@ -61,27 +60,35 @@ __global__ void __launch_bounds__(TS_NT) ts_apply_kernel(const __grid_constant__
                 if (lane < K) Xs[(warp + (TS_NT / 32) * i) * ldx + lane] = v[i];
         }
         __syncthreads();
-        double acc[NH];
+        // thread = (row pair rp, rp + 64; quarter of the columns): every small-operand read feeds two rows
+        constexpr int NQ = NH / 2;
+        const int rp = t & 63, quarter = t >> 6;
+        double acc0[NQ], acc1[NQ];
 #pragma unroll
-        for (int j = 0; j < NH; ++j) acc[j] = 0.0;
-        const double *xr = Xs + r_loc * ldx;
-        const double *wh = Ws + half * NH;
+        for (int j = 0; j < NQ; ++j) acc0[j] = acc1[j] = 0.0;
+        const double *x0r = Xs + rp * ldx, *x1r = Xs + (rp + 64) * ldx;
+        const double *wq = Ws + quarter * NQ;
         for (int c = 0; c < K; ++c) {
-            const double x = xr[c];
-            const double2 *w2 = reinterpret_cast<const double2 *>(wh + c * 2 * NH);
+            const double x0 = x0r[c], x1 = x1r[c];
+            const double2 *w2 = reinterpret_cast<const double2 *>(wq + c * 2 * NH);
 #pragma unroll
-            for (int j = 0; j < NH / 2; ++j) {
+            for (int j = 0; j < NQ / 2; ++j) {
                 const double2 w = w2[j];
-                acc[2 * j] = fma(x, w.x, acc[2 * j]);
-                acc[2 * j + 1] = fma(x, w.y, acc[2 * j + 1]);
+                acc0[2 * j] = fma(x0, w.x, acc0[2 * j]);
+                acc0[2 * j + 1] = fma(x0, w.y, acc0[2 * j + 1]);
+                acc1[2 * j] = fma(x1, w.x, acc1[2 * j]);
+                acc1[2 * j + 1] = fma(x1, w.y, acc1[2 * j + 1]);
             }
         }
         // results through shared memory (the X tile is dead), then whole rows per warp: coalesced stores
         __syncthreads();
-        double *Ys = Xs;                     // [TS_ROWS][ldy], ldy <= ldx only if N <= K: use its own stride
+        double *Ys = Xs;                     // [TS_ROWS][ldy]
         const int ldy = (2 * NH) | 1;
 #pragma unroll
-        for (int j = 0; j < NH; ++j) Ys[r_loc * ldy + half * NH + j] = acc[j];
+        for (int j = 0; j < NQ; ++j) {
+            Ys[rp * ldy + quarter * NQ + j] = acc0[j];
+            Ys[(rp + 64) * ldy + quarter * NQ + j] = acc1[j];
+        }
         __syncthreads();
         for (int rr = warp; rr < TS_ROWS; rr += TS_NT / 32) {
             if (offC[rr] >= 0) {
