@@ -425,16 +425,36 @@ def contract_triad(E, F, G, H, U, Ms, Ns):
 def contract_atrg(A, X, sig, Y, D, Ms, Ns):
     """Plain ATRG contraction without triads, O(chi^9) (Table 1 :113):
     Phi = sum A (X sigma) M1 M2 M3, Psi = sum Y D N1 N2 N3; sigma stays on the Phi side as in
-    the triad form (it sits in F, Eq. 5)."""
-    n1, n2, n3 = A.shape[1], A.shape[2], A.shape[3]
+    the triad form (it sits in F, Eq. 5).
+
+    The two five-operand sums
+        Phi[x,m,n,w,g] = sum A[x,p,q,t,a] (X sigma)[a,r,s,u,g] M1[p,r,m] M2[q,s,n] M3[t,u,w]
+        Psi[x,m,n,w,g] = sum Y[b,p,q,t,g] D[x,r,s,u,b] N1[m,p,r] N2[n,q,s] N3[w,t,u]
+    are evaluated pairwise in the order of Table 1's cost count (squeezer of the first pair leg,
+    then the O(chi^9) product with the second site over (bond, pair leg), then the other two
+    squeezers), one value of the pass-through leg x at a time: x is a free index of both sums, and
+    the chi^7-sized intermediate of the whole tensor would not fit host memory at chi = 24
+    (BASELINE.json config 4).  Pinned by the 14-leg brute force of test_P7."""
+    n0, n1, n2, n3 = A.shape[0], A.shape[1], A.shape[2], A.shape[3]
     M1 = Ms[1].reshape(n1, n1, -1)
     M2 = Ms[2].reshape(n2, n2, -1)
     M3 = Ms[3].reshape(n3, n3, -1)
     N1 = Ns[1].reshape(-1, n1, n1)
     N2 = Ns[2].reshape(-1, n2, n2)
     N3 = Ns[3].reshape(-1, n3, n3)
-    phi = np.einsum("xpqta,arsug,prm,qsn,tuw->xmnwg", A, X * sig, M1, M2, M3, optimize=True)
-    psi = np.einsum("bpqtg,xrsub,mpr,nqs,wtu->xmnwg", Y, D, N1, N2, N3, optimize=True)
+    Xs = X * sig
+    g = len(sig)
+    phi = np.empty((n0, M1.shape[2], M2.shape[2], M3.shape[2], g))
+    psi = np.empty((n0, N1.shape[0], N2.shape[0], N3.shape[0], g))
+    for x in range(n0):
+        t = np.einsum("pqta,prm->qtarm", A[x], M1, optimize=True)
+        t = np.einsum("qtarm,arsug->qtmsug", t, Xs, optimize=True)       # the O(chi^9) product
+        t = np.einsum("qtmsug,qsn->tmnug", t, M2, optimize=True)
+        phi[x] = np.einsum("tmnug,tuw->mnwg", t, M3, optimize=True)
+        t = np.einsum("rsub,mpr->subpm", D[x], N1, optimize=True)
+        t = np.einsum("subpm,bpqtg->sumqtg", t, Y, optimize=True)        # the O(chi^9) product
+        t = np.einsum("sumqtg,nqs->umntg", t, N2, optimize=True)
+        psi[x] = np.einsum("umntg,wtu->mnwg", t, N3, optimize=True)
     return phi, psi
 
 
