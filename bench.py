@@ -260,6 +260,25 @@ def job_value(world, steps, ms):
     return world * steps / (ms * 1e-3)
 
 
+SCHEDULE_STEPS = 40   # BASELINE.json: every config is a 40-step schedule (8 for c1), directions cycling 1..4
+
+
+def timed_segments(ramp, W, K, sched=SCHEDULE_STEPS):
+    """The timed steps stay inside the config's schedule (BASELINE.json c3: 'steps 9...40'): after `ramp`
+    untimed ramp-up steps and W warm-up steps at most sched - ramp - W steps are timed in one go; a larger
+    K is split into segments, each from a fresh init + ramp-up + warm-up.  Returns lists of 0-based step
+    indices."""
+    room = sched - ramp - W
+    if room < 1:
+        raise ValueError("warm-up of %d steps leaves no timed step inside the %d-step schedule" % (W, sched))
+    segs, left = [], K
+    while left > 0:
+        n = min(left, room)
+        segs.append(list(range(ramp + W, ramp + W + n)))
+        left -= n
+    return segs
+
+
 def run_ours(args, cfg, name):
     import torch
     import paper_2412_14104_b200 as tt
@@ -281,21 +300,22 @@ def run_ours(args, cfg, name):
         torch.cuda.synchronize()
 
     chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
-    K, W = args.steps, max(args.warmup, 0)
+    K, W, ramp = args.steps, max(args.warmup, 0), cfg["ramp"]
+    segs = timed_segments(ramp, W, K, 8 if name == "c1" else SCHEDULE_STEPS)
     tt.set_workspace(chi=chi, r=r, device="cuda:%d" % local, atrg=bool(cfg.get("atrg")))
     step_fn = tt.coarse_grain_atrg if cfg.get("atrg") else tt.coarse_grain
     stream = torch.cuda.Stream()
     tt.set_stream(stream)
-    tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
-    m = 0
-    for _ in range(cfg["ramp"]):                       # untimed ramp-up to the steady state
-        for which, t in gauge_refs(tt, cfg, m % 4 + 1).items():
-            tt.set_sketch(which, t)
-        step_fn(m % 4 + 1, chi, r, q, seed)
-        m += 1
-    dims = tt.get_dims()
-    steady = all(d == chi for d in dims[:5])
 
+    def start():
+        """init + untimed ramp-up to the steady state (inputs generated by the library from the seed)."""
+        tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
+        for m in range(ramp):
+            step_fn(m % 4 + 1, chi, r, q, seed)
+        return tt.get_dims()
+
+    dims = start()
+    steady = all(d == chi for d in dims[:5])
     refs = {d: gauge_refs(tt, cfg, d) for d in (1, 2, 3, 4)}
 
     def set_inputs(sk, d):
@@ -304,115 +324,128 @@ def run_ours(args, cfg, name):
         for which, t in refs[d].items():
             tt.set_sketch(which, t)
 
-    # ---- pass 1: sketches resident in HBM before the timed region.  Small configs: all W + K steps
-    # sketches are uploaded first and one event pair brackets the K steps.  Large configs (chi = 64: 17 GB
-    # of sketch per step): one device buffer set, refilled between steps outside the per-step event
-    # pairs, whose times are summed.
+    # Host-generated (north star) seeded sketches of every step the two passes run, page-locked.  Large
+    # configs (chi = 64: 17 GB of sketch per step): one buffer set, refilled between steps outside the
+    # per-step event pairs.
     per_step_bytes = sum(a * b * 8 for a, b in (tt.sketch_shape(w, 1, chi, r) for w in range(5)))
-    streamed = per_step_bytes * (W + K) > (20 << 30)
+    span = W + max(len(sg) for sg in segs)
+    streamed = per_step_bytes * span > (20 << 30)
+    hosts = {}
     if streamed:
-        host = pinned_sketches(tt, cfg, m, m % 4 + 1)
-        dev1 = {w: torch.empty_like(t, device="cuda") for w, t in host.items()}
+        host1 = pinned_sketches(tt, cfg, ramp, ramp % 4 + 1)
+    else:
+        for mm in range(ramp, ramp + span):
+            hosts[mm] = pinned_sketches(tt, cfg, mm, mm % 4 + 1)
 
-        def inputs_for(i):
-            pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1, reuse=host)
-            for w, t in host.items():
+    # ---- pass 1: the step's sketches resident in HBM before the timed region
+    if streamed:
+        dev1 = {w: torch.empty_like(t, device="cuda") for w, t in host1.items()}
+
+        def resident(mm):
+            pinned_sketches(tt, cfg, mm, mm % 4 + 1, reuse=host1)
+            for w, t in host1.items():
                 dev1[w].copy_(t)
             torch.cuda.synchronize()
             return dev1
     else:
-        hosts = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(W + K)]
-        dev = [{w: t.cuda() for w, t in sk.items()} for sk in hosts]
+        dev = {mm: {w: t.cuda() for w, t in sk.items()} for mm, sk in hosts.items()}
         torch.cuda.synchronize()
 
-        def inputs_for(i):
-            return dev[i]
-    for i in range(W):
-        set_inputs(inputs_for(i), (m + i) % 4 + 1)
-        step_fn((m + i) % 4 + 1, chi, r, q, seed)
-    tt.set_profile(2 if args.profile_all else 1)
-    tt.launch_count(reset=True)
-    tt.gemm_flops(reset=True)
+        def resident(mm):
+            return dev[mm]
     vis = os.environ.get("CUDA_VISIBLE_DEVICES", "").split(",")
     sampler = ClockSampler(vis[local] if local < len(vis) and vis[local].strip().isdigit() else local)
     stages = {}
     gprof = {}
     pairs = []
-    barrier()
-    sampler.start()
-    if not streamed:
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        pairs.append((e0, e1))
-    for i in range(W, W + K):
-        d = (m + i) % 4 + 1
-        sk = inputs_for(i)
-        if streamed:
+    launches = 0
+    flops = 0.0
+    first = True
+    for sg in segs:
+        if not first:
+            start()
+        for mm in range(ramp, ramp + W):
+            set_inputs(resident(mm), mm % 4 + 1)
+            step_fn(mm % 4 + 1, chi, r, q, seed)
+        tt.set_profile(2 if args.profile_all else 1)
+        tt.launch_count(reset=True)
+        tt.gemm_flops(reset=True)
+        barrier()
+        if first:
+            sampler.start()
+        if not streamed:
             pairs.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
             pairs[-1][0].record(stream)
-        set_inputs(sk, d)
-        step_fn(d, chi, r, q, seed)
-        if streamed:
+        for mm in sg:
+            d = mm % 4 + 1
+            sk = resident(mm)
+            if streamed:
+                pairs.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
+                pairs[-1][0].record(stream)
+            set_inputs(sk, d)
+            step_fn(d, chi, r, q, seed)
+            if streamed:
+                pairs[-1][1].record(stream)
+            for k, v in tt.stage_ms().items():
+                stages[k] = stages.get(k, 0.0) + v / K
+            for k, v in tt.gemm_profile().items():
+                g = gprof.setdefault(k, {"ms": [0.0, 0.0], "flops": [0.0, 0.0], "launches": [0, 0]})
+                for j in range(2):
+                    g["ms"][j] += v["ms"][j]
+                    g["flops"][j] += v["flops"][j]
+                    g["launches"][j] += v["launches"][j]
+        if not streamed:
             pairs[-1][1].record(stream)
-        for k, v in tt.stage_ms().items():
-            stages[k] = stages.get(k, 0.0) + v / K
-        for k, v in tt.gemm_profile().items():
-            g = gprof.setdefault(k, {"ms": [0.0, 0.0], "flops": [0.0, 0.0], "launches": [0, 0]})
-            for j in range(2):
-                g["ms"][j] += v["ms"][j]
-                g["flops"][j] += v["flops"][j]
-                g["launches"][j] += v["launches"][j]
-    if not streamed:
-        pairs[0][1].record(stream)
-    barrier()
+        barrier()
+        launches += tt.launch_count(reset=True)
+        flops += tt.gemm_flops(reset=True)
+        tt.set_profile(False)
+        first = False
     clocks = sampler.stop()
     ms = sum(a.elapsed_time(b) for a, b in pairs)
-    launches = tt.launch_count(reset=True)
-    flops = tt.gemm_flops(reset=True)
-    tt.set_profile(False)
-    m += W + K
     lnz = tt.log_Z_per_site()
     if streamed:
         del dev1
     else:
         del dev
-        hosts = None
     torch.cuda.empty_cache()
 
-    # ---- pass 2: end to end through the C-ABI with host sketch buffers + ln Z read-back
-    Ke = K
+    # ---- pass 2: the SAME steps end to end through the C-ABI: host (page-locked) sketch buffers, copied
+    # host -> device inside coarse_grain on the library's copy stream, + the ln Z/V read-back every step
     h2d = 0
+    h2d_ms = 0.0
     pairs2 = []
-    if streamed:
+    for sg in segs:
+        start()
+        for mm in range(ramp, ramp + W):
+            sk = pinned_sketches(tt, cfg, mm, mm % 4 + 1, reuse=host1) if streamed else hosts[mm]
+            set_inputs(sk, mm % 4 + 1)
+            step_fn(mm % 4 + 1, chi, r, q, seed)
         barrier()
-        for i in range(Ke):
-            d = (m + i) % 4 + 1
-            pinned_sketches(tt, cfg, m + i, d, reuse=host)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            set_inputs(host, d)                          # host pointers: copied inside coarse_grain
+        if not streamed:
+            pairs2.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
+            pairs2[-1][0].record(stream)
+        for mm in sg:
+            d = mm % 4 + 1
+            if streamed:
+                sk = pinned_sketches(tt, cfg, mm, d, reuse=host1)
+                pairs2.append((torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)))
+                pairs2[-1][0].record(stream)
+            else:
+                sk = hosts[mm]
+            set_inputs(sk, d)                             # host pointers: copied inside coarse_grain
             step_fn(d, chi, r, q, seed)
-            lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
-            b.record(stream)
-            pairs2.append((a, b))
-            h2d += sum(t.numel() * 8 for t in host.values())
+            lnz2 = tt.log_Z_per_site()                    # device dot product + scalar D2H
+            if streamed:
+                pairs2[-1][1].record(stream)
+            t_ms, t_b = tt.h2d()
+            h2d += t_b
+            h2d_ms += t_ms
+        if not streamed:
+            pairs2[-1][1].record(stream)
         barrier()
-    else:
-        e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        host2 = [pinned_sketches(tt, cfg, m + i, (m + i) % 4 + 1) for i in range(Ke)]
-        barrier()
-        e2.record(stream)
-        for i in range(Ke):
-            d = (m + i) % 4 + 1
-            set_inputs(host2[i], d)                      # host pointers: copied inside coarse_grain
-            step_fn(d, chi, r, q, seed)
-            lnz = tt.log_Z_per_site()                     # device dot product + scalar D2H
-            h2d += sum(t.numel() * 8 for t in host2[i].values())
-        e3.record(stream)
-        barrier()
-        pairs2.append((e2, e3))
     ms_e2e = sum(a.elapsed_time(b) for a, b in pairs2)
-    m += Ke
+    lnz_match = abs(lnz2 - lnz) <= 1e-12 * abs(lnz)       # both passes ran the same steps on the same inputs
 
     # ---- max over ranks
     (ms, ms_e2e), (launches,) = reduce_over_ranks([ms, ms_e2e], [launches], dist, "cuda")
@@ -425,7 +458,7 @@ def run_ours(args, cfg, name):
     g_n = sum(v["launches"][1] for v in gprof.values())
     s_ms = sum(v["ms"][0] for v in gprof.values())
     s_fl = sum(v["flops"][0] for v in gprof.values())
-    peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * FP64_OVER_BF16_NOMINAL
+    peak_bf16_ratio = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) * FP64_OVER_BF16_NOMINAL
     achieved = g_fl / (g_ms * 1e-3) / 1e12 if g_ms > 0 else 0.0
     probe = tt.probe_fp64_peak(0, 1 << 14)
     probe_dfma = tt.probe_fp64_peak(1, 1 << 14)
@@ -436,14 +469,17 @@ def run_ours(args, cfg, name):
                  for k, v in gprof.items()}
     roofline = {"bound": "tensor",
                 "kernel": "tgemm_big_kernel<..,BN=128,WN=32,BK=32,STAGES=3,MBAR> (128x128 CTA tile, FP64 DMMA.8x8x4)",
-                "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak if peak else None,
+                "achieved": achieved, "peak": probe, "unit": "TFLOP/s", "frac": achieved / probe if probe > 0 else None,
                 "traffic": NCU_TRAFFIC["dram_bytes"],
                 "traffic_of": NCU_TRAFFIC,
-                "peak_source": "%s bf16_tflops_sustained x nominal FP64/bf16 ratio 45/2250" % how,
-                "peak_note": ("the bf16 figure is power-throttled (1.3 GHz), FP64 runs at 1965 MHz and ~450 W, so frac can "
-                              "exceed 1; the stricter denominator is the live register-resident DMMA probe: frac_of_probe"),
-                "peak_probe_dmma_tflops": probe, "peak_probe_dfma_tflops": probe_dfma,
-                "frac_of_probe": achieved / probe if probe > 0 else None,
+                "peak_source": ("FP64 tensor-pipe peak measured live on this GPU: register-resident DMMA.8x8x4 loop "
+                                "(tatrg_probe_fp64_peak); MEASURED_PEAKS.json has no FP64 figure; nominal 148 SM x 64 FMA/clk x "
+                                "2 x 1.965 GHz = 37.2"),
+                "peak_from_bf16_ratio": peak_bf16_ratio,
+                "peak_from_bf16_ratio_note": ("%s bf16_tflops_sustained x nominal FP64/bf16 ratio 45/2250: the bf16 figure is "
+                                              "power-throttled (~1.3 GHz) while FP64 runs at 1965 MHz, so this denominator is "
+                                              "below what the FP64 pipe delivers; not used for frac" % how),
+                "peak_probe_dfma_tflops": probe_dfma,
                 "flops_per_launch": g_fl / g_n if g_n else 0.0, "avg_launch_ms": g_ms / g_n if g_n else 0.0,
                 "launches": g_n, "share_of_step_time": g_ms / ms if ms > 0 else None,
                 "small_tile_kernel": {"tflops": s_fl / (s_ms * 1e-3) / 1e12 if s_ms > 0 else 0.0,
@@ -452,17 +488,24 @@ def run_ours(args, cfg, name):
 
     line = None
     if rank == 0:
+        timed = ", ".join("%d..%d" % (sg[0] + 1, sg[-1] + 1) for sg in segs)
         line = {"metric": METRIC, "value": job_value(world, K, ms), "unit": UNIT, "n_gpus": world, "steps": K,
                 "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": workload_name(name, cfg), "chi": chi, "r": r, "q": q,
                            "steady_state": steady, "dims": list(dims[:5]),
+                           "timed_steps": "steps %s of the config's schedule (1-based), after %d ramp-up + %d warm-up "
+                                          "steps; both passes time the same steps" % (timed, ramp, W),
                            "l2": "inputs larger than L2 (Phi, Psi, A, D, X, Y are %.0f MB each)" % (8e-6 * chi ** 5),
                            "timed_region": ("per-step event pairs summed, sketch refilled between steps"
-                                            if streamed else "one event pair around the K steps"),
+                                            if streamed else "one event pair around the timed steps of a segment"),
                            "parallelism": "replicas only" if world > 1 else "1 GPU"},
-                "e2e": {"value": job_value(world, Ke, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke,
-                        "d2h_bytes_per_step": 8, "steps": Ke},
+                "e2e": {"value": job_value(world, K, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": h2d // K,
+                        "d2h_bytes_per_step": 8, "steps": K, "ms_per_step": ms_e2e / K,
+                        "h2d_ms_per_step": h2d_ms / K,
+                        "h2d_note": "copy-stream time of the step's uploads; they run beside the canonical form and the "
+                                    "basis factorisations of the bond swap",
+                        "ln_Z_equal_to_resident_pass": bool(lnz_match)},
                 "gpu_launches": launches, "clocks": clocks, "roofline": roofline,
                 "stages_ms_per_step": stages, "stages_gemm": per_stage, "ln_Z_per_site": lnz}
     return line

@@ -110,6 +110,11 @@ double tatrg_order_parameter(int leg);
  * named by tatrg_stage_name(i).  Returns the number of stages. */
 int tatrg_get_stage_ms(double *host_out, int cap);
 const char *tatrg_stage_name(int i);
+/* Host->device upload of the last step's host-resident inputs (tatrg_set_sketch with on_device == 0;
+ * the seeded sketches of SURVEY.md 8(d)): *ms_out (host) = device milliseconds between the first and the
+ * last copy on the library's copy stream (it runs beside the canonical form and the basis factorisations
+ * of the bond swap), *bytes_out (host) = bytes copied.  Either pointer may be NULL. */
+int tatrg_get_h2d(double *ms_out, size_t *bytes_out);
 /* Per-launch device timing of the tensor-GEMM kernel (CUDA event pairs on the library's stream
  * around the launches inside coarse_grain; a few microseconds of overhead per timed launch).
  * on = 1: only the 128x128-tile launches (the dominant kernel) are timed; on = 2: every tensor-GEMM

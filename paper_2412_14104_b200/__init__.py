@@ -21,7 +21,7 @@ EXPORTS = [
     "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_bytes_atrg",
     "tatrg_workspace_peak",
     "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
-    "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name",
+    "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name", "tatrg_get_h2d",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
     "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
@@ -68,6 +68,7 @@ def lib():
             "tatrg_order_parameter": (c_d, [c_i]),
             "tatrg_get_stage_ms": (c_i, [c_vp, c_i]),
             "tatrg_stage_name": (ctypes.c_char_p, [c_i]),
+            "tatrg_get_h2d": (c_i, [c_vp, c_vp]),
             "tatrg_set_profile": (c_i, [c_i]),
             "tatrg_get_gemm_profile": (c_i, [c_vp, c_i]),
             "tatrg_launch_count": (ctypes.c_longlong, [c_i]),
@@ -240,6 +241,13 @@ def stage_ms() -> dict:
     out = np.zeros(16)
     n = lib().tatrg_get_stage_ms(out.ctypes.data, out.size)
     return {lib().tatrg_stage_name(i).decode(): float(out[i]) for i in range(n)}
+
+
+def h2d():
+    """(milliseconds on the copy stream, bytes) of the last step's host -> device input upload."""
+    ms, nb = ctypes.c_double(0.0), ctypes.c_size_t(0)
+    _check(lib().tatrg_get_h2d(ctypes.byref(ms), ctypes.byref(nb)))
+    return ms.value, nb.value
 
 
 def set_profile(on):

@@ -393,6 +393,13 @@ int tatrg_get_gemm_profile(double *host_out, int cap)
     return k;
 }
 
+int tatrg_get_h2d(double *ms_out, size_t *bytes_out)
+{
+    if (ms_out) *ms_out = ctx().h2d_ms;
+    if (bytes_out) *bytes_out = ctx().h2d_bytes;
+    return TATRG_OK;
+}
+
 const char *tatrg_stage_name(int i) { return (i >= 0 && i < ST_COUNT) ? kStageNames[i] : ""; }
 
 long long tatrg_launch_count(int reset)
@@ -544,6 +551,8 @@ void tatrg_destroy(void)
     if (c.copy_stream) {
         cudaStreamDestroy(c.copy_stream);
         for (auto &e : c.pre_ev) cudaEventDestroy(e);
+        cudaEventDestroy(c.pre_t0);
+        cudaEventDestroy(c.pre_t1);
     }
     if (c.pinned) cudaFreeHost(c.pinned);
     c = Ctx();

@@ -45,6 +45,10 @@ struct Ctx {
     // (step.cpp: prefetch_inputs), overlapping the canonical form; get_input waits for the event
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t pre_ev[9] = {};
+    cudaEvent_t pre_t0 = nullptr, pre_t1 = nullptr;   // timing events around the step's uploads
+    bool pre_timed = false;
+    double h2d_ms = 0;                                // copy-stream time of the last step's uploads
+    size_t h2d_bytes = 0;
     double *pre[9] = {};
     size_t pre_n[9] = {};
 

@@ -196,15 +196,21 @@ void prefetch_inputs()
 {
     Ctx &c = ctx();
     for (int w = 0; w < 9; ++w) c.pre[w] = nullptr;
+    c.pre_timed = false;
+    c.h2d_ms = 0;
+    c.h2d_bytes = 0;
     bool any = false;
     for (int w = 0; w < 9; ++w) any = any || (c.in[w].ptr && !c.in[w].on_device && c.in[w].n > 0);
     if (!any) return;
     if (!c.copy_stream) {
         TATRG_CUDA_CHECK(cudaStreamCreateWithFlags(&c.copy_stream, cudaStreamNonBlocking));
         for (auto &e : c.pre_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        TATRG_CUDA_CHECK(cudaEventCreate(&c.pre_t0));
+        TATRG_CUDA_CHECK(cudaEventCreate(&c.pre_t1));
     }
     TATRG_CUDA_CHECK(cudaEventRecord(c.pre_ev[0], c.stream));
     TATRG_CUDA_CHECK(cudaStreamWaitEvent(c.copy_stream, c.pre_ev[0], 0));
+    TATRG_CUDA_CHECK(cudaEventRecord(c.pre_t0, c.copy_stream));
     for (int w = 0; w < 9; ++w) {
         const Input &in = c.in[w];
         if (!in.ptr || in.on_device || in.n == 0) continue;
@@ -212,7 +218,10 @@ void prefetch_inputs()
         c.pre_n[w] = in.n;
         TATRG_CUDA_CHECK(cudaMemcpyAsync(c.pre[w], in.ptr, sizeof(double) * in.n, cudaMemcpyHostToDevice, c.copy_stream));
         TATRG_CUDA_CHECK(cudaEventRecord(c.pre_ev[w], c.copy_stream));
+        c.h2d_bytes += sizeof(double) * in.n;
     }
+    TATRG_CUDA_CHECK(cudaEventRecord(c.pre_t1, c.copy_stream));
+    c.pre_timed = true;
 }
 
 Ten get_input(int which, long long rows, long long cols, const StepCfg &cfg, const char *names2)
@@ -221,7 +230,10 @@ Ten get_input(int which, long long rows, long long cols, const StepCfg &cfg, con
     long long n = rows * cols;
     Ten t;
     Input &in = c.in[which];
-    if (in.ptr && in.n == (size_t)n) {
+    if (in.ptr && in.n != (size_t)n)
+        fail(-22, "input %d set with tatrg_set_sketch has %zu doubles, this step needs %lld x %lld = %lld (tatrg_sketch_shape)",
+             which, in.n, rows, cols, n);
+    if (in.ptr) {
         if (!in.on_device && c.pre[which] && c.pre_n[which] == (size_t)n) {
             TATRG_CUDA_CHECK(cudaStreamWaitEvent(stream(), c.pre_ev[which], 0));
             return Ten::make(c.pre[which], names2, {rows, cols});
@@ -460,7 +472,8 @@ struct SqChain {
         if (!(sh[chi - 1] > 1e-6 * sh[0])) return false;
         const double rho = sh[b - 1] / sh[chi - 1];
         const int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
-        more = std::max(1, std::min(need + 1, 80) - 2);    // two iterations are done
+        if (need + 1 > 80) return false;                   // decay too slow for this block width: dense route
+        more = std::max(1, need + 1 - 2);                  // two iterations are done
         return true;
     }
     void phaseB()
@@ -1400,6 +1413,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     // an uploaded input that no stage consumed (wrong shape for this step) may still be in flight:
     // the caller's host buffers are read during the call only
     if (c.copy_stream) TATRG_CUDA_CHECK(cudaStreamSynchronize(c.copy_stream));
+    if (c.pre_timed) {
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, c.pre_t0, c.pre_t1) == cudaSuccess) c.h2d_ms = ms;
+    }
     if (!(nv[0] > 0) || !(nv[1] > 0) || !std::isfinite(nv[0]) || !std::isfinite(nv[1]))
         fail(-34, "coarse_grain: non-finite or zero norm of the renormalised tensor");
     // ---- commit
