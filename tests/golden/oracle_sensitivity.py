@@ -5,12 +5,14 @@ value.  Two correct FP64 implementations of the same step differ by rounding, an
 steps near criticality amplify that; this script measures the amplification on the oracle alone, so that
 the tolerances of the parity tests rest on the method's conditioning, not on what the CUDA path happens
 to reach.  It runs a config twice with the same seeds: once as it stands, once with every Gaussian
-sketch element (bond swap and the four isometries) multiplied by (1 + 2^-52), i.e. moved by one ulp, and
-records, per step and per spectrum, max_i |s_i - s_i'| / s_1 and the relative change of ln Z/V.
+sketch element (bond swap and the four isometries) multiplied by (1 + u 2^-52), i.e. moved by u ulps
+(u = 1 by default; u = 64 stands for the backward error of a different but backward-stable factorisation of
+a 10^3..10^5-row block, which is tens of ulps), and records, per step and per spectrum,
+max_i |s_i - s_i'| / s_1 and the relative change of ln Z/V.
 
 Imports ONLY oracle/ and seeded_inputs/.  Writes tests/golden/oracle_sensitivity_<name>.json.
 
-    python tests/golden/oracle_sensitivity.py c2
+    python tests/golden/oracle_sensitivity.py c2 [ulps]
 """
 from __future__ import annotations
 
@@ -33,14 +35,14 @@ SPECTRA = ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3")
 ULP = 2.0 ** -52
 
 
-def main(name):
+def main(name, ulps=1):
     from oracle import driver
     from oracle import tatrg_oracle as orc
     cfg = RUNS[name]
     beta = 1.0 / cfg["T"]
     a = orc.init_ising_tensor(beta, cfg["h"])
     b = orc.init_ising_tensor(beta, cfg["h"])
-    out = {"name": name, "config": cfg, "perturbation": "every element of the five Gaussian sketches x (1 + 2^-52)",
+    out = {"name": name, "config": cfg, "perturbation": "every element of the five Gaussian sketches x (1 + %d * 2^-52)" % ulps,
            "steps": []}
     worst = {}
     for m in range(cfg["steps"]):
@@ -49,7 +51,7 @@ def main(name):
 
         def moved(which, rows, cols, base=base):
             g = base(which, rows, cols)
-            return g if which.startswith("ref") else g * (1.0 + ULP)
+            return g if which.startswith("ref") else g * (1.0 + ulps * ULP)
         ra = orc.coarse_grain(a, d, cfg["chi"], cfg["r"], cfg["q"], base)
         rb = orc.coarse_grain(b, d, cfg["chi"], cfg["r"], cfg["q"], moved)
         la, lb = orc.log_Z_per_site(a), orc.log_Z_per_site(b)
@@ -64,7 +66,7 @@ def main(name):
         out["steps"].append(rec)
         print(" ".join("%s %.1e" % (k, v) if k != "step" else "step %d" % (v + 1) for k, v in rec.items()), flush=True)
     out["worst"] = worst
-    path = os.path.join(HERE, "oracle_sensitivity_%s.json" % name)
+    path = os.path.join(HERE, "oracle_sensitivity_%s%s.json" % (name, "" if ulps == 1 else "_%dulp" % ulps))
     with open(path, "w") as f:
         json.dump(out, f, indent=1)
         f.write("\n")
@@ -73,4 +75,4 @@ def main(name):
 
 
 if __name__ == "__main__":
-    main(sys.argv[1] if len(sys.argv) > 1 else "c2")
+    main(sys.argv[1] if len(sys.argv) > 1 else "c2", int(sys.argv[2]) if len(sys.argv) > 2 else 1)
