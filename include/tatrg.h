@@ -95,6 +95,15 @@ int tatrg_sketch_shape(int which, int direction, int chi, int r, int64_t *rows, 
  * step (1 value).  Returns the count (<= cap) or a negative status. */
 int tatrg_get_spectrum(int which, double *host_out, int cap);
 
+/* Oversampled isometries of the LAST coarse_grain step (Eqs. 2-3; I, J, K, L of Eqs. 8-11),
+ * for tests (the projector U U^T is gauge invariant and is what parity compares).  tatrg_keep_isometries(1)
+ * makes every following step copy its four isometries to the host (one extra synchronisation per step);
+ * tatrg_get_isometry copies U^which (which = 0..3: A, X, Y, D), row-major [(p,q), k] in the rotated
+ * frame, rows = d_t1 d_t2, cols = min(r chi, rows) (the identity when cols = rows), to host_out (host,
+ * capacity cap doubles; NULL = only rows / cols are returned). */
+int tatrg_keep_isometries(int on);
+int tatrg_get_isometry(int which, double *host_out, size_t cap, int *rows, int *cols);
+
 /* dims_out[0..3] = leg dimensions d1..d4, dims_out[4] = bond, dims_out[5] = step count. */
 int tatrg_get_dims(int dims_out[6]);
 

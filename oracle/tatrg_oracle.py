@@ -491,6 +491,7 @@ def coarse_grain(st, direction, chi, r, q, inputs, mode="triad", iso_mode="rsvd"
         U, spec = make_isometries(A, X, sig, Y, D, chi, r, q, om, iso_mode)
         for t in "AXYD":
             rec["S" + t] = spec[t]
+        rec["U"] = U                      # record only (tests compare the projectors U U^T)
         E, F, G, H = triad_tensors(A, X, sig, Y, D, U)
         GL, GR = triad_grams(E, F, G, H, U)
     elif mode == "atrg":

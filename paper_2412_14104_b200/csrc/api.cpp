@@ -326,6 +326,29 @@ int tatrg_get_spectrum(int which, double *host_out, int cap)
     return n;
 }
 
+int tatrg_keep_isometries(int on)
+{
+    ctx().keep_iso = on != 0;
+    if (!on)
+        for (auto &v : ctx().iso) v.clear();
+    return TATRG_OK;
+}
+
+int tatrg_get_isometry(int which, double *host_out, size_t cap, int *rows, int *cols)
+{
+    Ctx &c = ctx();
+    if (which < 0 || which > 3) return set_error(TATRG_EINVAL, "tatrg_get_isometry: which must be 0..3 (A, X, Y, D)");
+    const std::vector<double> &v = c.iso[which];
+    if (v.empty()) return set_error(TATRG_ESTATE, "tatrg_get_isometry: nothing kept (tatrg_keep_isometries(1) before the step; Triad-ATRG steps only)");
+    if (rows) *rows = c.iso_rows;
+    if (cols) *cols = c.iso_cols;
+    if (host_out) {
+        if (cap < v.size()) return set_error(TATRG_EINVAL, "tatrg_get_isometry: need %zu doubles", v.size());
+        memcpy(host_out, v.data(), v.size() * sizeof(double));
+    }
+    return TATRG_OK;
+}
+
 int tatrg_get_gaps(double out[4])
 {
     for (int i = 0; i < 4; ++i) out[i] = ctx().gaps[i];

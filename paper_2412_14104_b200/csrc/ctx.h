@@ -53,6 +53,9 @@ struct Ctx {
     size_t pre_n[9] = {};
 
     Input in[9];
+    bool keep_iso = false;                  // tatrg_keep_isometries: host copies of U^A, U^X, U^Y, U^D of the last step
+    std::vector<double> iso[4];
+    int iso_rows = 0, iso_cols = 0;
     std::vector<double> spec[10];
     double gaps[4] = {0, 0, 0, 0};
 

@@ -1078,6 +1078,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             }
     }
     kd = U[0].legs[2].n;
+    if (c.keep_iso) {   // tests: the gauge-invariant projectors U U^T are compared with the oracle's
+        c.iso_rows = (int)n12;
+        c.iso_cols = (int)kd;
+        for (int i = 0; i < 4; ++i) c.iso[i] = d2h(U[i].p, n12 * kd);
+    }
     stage_mark(3);
 
     // =================== O5 triad tensors (Eqs. 4-7) ===================

@@ -13,6 +13,20 @@ pytestmark = pytest.mark.gpu
 
 LNZ_RTOL = 1e-10
 SPEC_TOL = 1e-9
+# S^A..S^D are Ritz values after q unconverged subspace iterations, not truncated spectra.  The oracle's own
+# conditioning (tests/golden/oracle_sensitivity_c2*.json: the oracle against itself with its sketches moved by
+# 1 and by 64 ulps) moves them 10-27 times further than sigma^T / sigma_swap / s^(mu) along config 2's 40
+# steps; the CUDA path shows the same ratio (sigma^T 1.3e-10, S^D 3.3e-9 at worst, whether it is fed the
+# oracle's bytes or its own generator's).  They are held to 1e-9 like the rest wherever that is reached
+# (config 1, config 3's 12 stored steps, config 4, the wide routes, config 2 up to step 21) and to
+# RITZ_TOL_LATE on config 2's late steps only.
+RITZ_TOL_LATE = 1e-8
+# The isometries themselves, gauge invariant (reading G18): max |U S U^T - U_o S_o U_o^T| / S_1, the Ritz
+# vectors weighted by their Ritz values (the plain projector U U^T is not unique when K K^T has fewer than
+# r chi non-zero eigenvalues, as in the early steps: the trailing Ritz vectors then span an arbitrary part
+# of the null space and carry zero weight in Gamma)
+PROJ_TOL = 1e-9        # measured: <= 7e-13 on configs 1, 3; 9.6e-9 at worst on config 2's late steps
+PROJ_TOL_LATE = 3e-8
 
 
 @pytest.fixture(scope="module")
@@ -32,34 +46,52 @@ def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None, mode="triad
     recs = []
     st = orc.init_ising_tensor(beta, h)
     tt.init_ising_tensor(beta, h)
+    tt.keep_isometries(mode == "triad")
     assert abs(tt.log_Z_per_site() / orc.log_Z_per_site(st) - 1) < 1e-13
     for m in range(n_steps):
         d = directions[m % len(directions)] if directions else (m % 4) + 1
         rec = orc.coarse_grain(st, d, chi, r, q, driver.seeded_inputs_for(seed, m), mode=mode)
         (tt.coarse_grain if mode == "triad" else tt.coarse_grain_atrg)(d, chi, r, q, seed)
         out = {"step": m, "lnz_o": orc.log_Z_per_site(st), "lnz_g": tt.log_Z_per_site(),
-               "dims_o": st.dims, "dims_g": tt.get_dims()[:5], "spec": {}}
+               "dims_o": st.dims, "dims_g": tt.get_dims()[:5], "spec": {}, "proj": {}}
         for name in ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3"):
             so, sg = np.asarray(rec[name]) if name in rec else np.zeros(0), tt.get_spectrum(name)
             out["spec"][name] = (so, sg)
+        if mode == "triad":
+            for t in "AXYD":
+                uo = rec["U"][t].reshape(-1, rec["U"][t].shape[-1])
+                ug = tt.get_isometry(t)
+                assert uo.shape == ug.shape, (m, t, uo.shape, ug.shape)
+                so, sg = np.asarray(rec["S" + t]), tt.get_spectrum("S" + t)
+                if len(so):
+                    out["proj"][t] = float(np.abs((uo * so) @ uo.T - (ug * sg) @ ug.T).max() / so[0])
         recs.append(out)
+    tt.keep_isometries(False)
     return recs
 
 
-def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL):
+def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL, ritz_late=None):
+    """ritz_late = (first 0-based step, tolerance): S^A..S^D from that step on are held to that tolerance."""
+    worst = {}
     for o in recs:
         assert tuple(o["dims_o"]) == tuple(o["dims_g"]), o
         for name, (so, sg) in o["spec"].items():
             assert len(so) == len(sg), (o["step"], name, len(so), len(sg))
             if len(so):
-                tol = np.full(len(so), spec_tol)
-                if name in ("SA", "SX", "SY", "SD"):
-                    # Ritz values of q unconverged subspace iterations (reading G13): they are
-                    # not truncated spectra and amplify the rounding-level differences of the two sides'
-                    # tensors; compared at 1e-8 (measured worst case over config 2's 40 steps: 1.3e-9)
-                    tol[:] = 10 * spec_tol
-                assert np.all(np.abs(so - sg) <= tol * so[0]), (o["step"], name, np.abs(so - sg).max() / so[0])
-        assert abs(o["lnz_g"] / o["lnz_o"] - 1) <= lnz_rtol, (o["step"], o["lnz_g"], o["lnz_o"])
+                tol = spec_tol
+                if ritz_late and name in ("SA", "SX", "SY", "SD") and o["step"] >= ritz_late[0]:
+                    tol = ritz_late[1]
+                dev = np.abs(so - sg).max() / so[0]
+                worst[name] = max(worst.get(name, 0.0), dev)
+                assert dev <= tol, (o["step"], name, dev)
+        for t, dev in o["proj"].items():
+            worst["P" + t] = max(worst.get("P" + t, 0.0), dev)
+            ptol = PROJ_TOL_LATE if (ritz_late and o["step"] >= ritz_late[0]) else PROJ_TOL
+            assert dev <= ptol, (o["step"], "projector U^" + t, dev)
+        dz = abs(o["lnz_g"] / o["lnz_o"] - 1)
+        worst["lnz"] = max(worst.get("lnz", 0.0), dz)
+        assert dz <= lnz_rtol, (o["step"], o["lnz_g"], o["lnz_o"])
+    print("worst deviations:", {k: "%.2e" % v for k, v in worst.items()})
 
 
 def test_config1_chi6_8steps(tt):
@@ -84,7 +116,7 @@ def test_direction_orders_with_field(tt, dirs):
 def test_config2_chi16_all_40_steps(tt):
     """BASELINE.json configs[1] (T=6.65, chi=16, r=2, q=2) in full: 40 steps, L = 2^10 per direction.
     (Measured: ln Z/V agrees to 3e-15 at every step, the spectra to 5e-10.)"""
-    check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 40, 20241215))
+    check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 40, 20241215), ritz_late=(21, RITZ_TOL_LATE))
 
 
 def test_config3_chi32_first_steps_incl_one_full_size_step(tt):
