@@ -172,17 +172,27 @@ struct TileCoord {
     int m0, n0, bz, split;
 };
 
+// per_z: live tiles of one (split, batch) slice.  lower_only (symmetric output, M = N): only the tiles on
+// or below the diagonal are enumerated, row by row: index l -> (tm, tn <= tm), l = tm (tm + 1) / 2 + tn
 __device__ __forceinline__ TileCoord decode_tile(const GemmParams &p, int tile, int tiles_m, int per_z)
 {
     TileCoord c;
     const int z = tile / per_z;
     const int r = tile - z * per_z;
-    const int band = r / (RASTER_W * p.tiles_n);
-    const int in_band = r - band * (RASTER_W * p.tiles_n);
-    const int w = min(RASTER_W, tiles_m - band * RASTER_W);
-    const int tn = in_band / w;
-    c.n0 = tn * BN;
-    c.m0 = (band * RASTER_W + (in_band - tn * w)) * BM;
+    if (p.lower_only) {
+        int tm = (int)((sqrtf(8.0f * (float)r + 1.0f) - 1.0f) * 0.5f);
+        while ((tm + 1) * (tm + 2) / 2 <= r) ++tm;
+        while (tm * (tm + 1) / 2 > r) --tm;
+        c.m0 = tm * BM;
+        c.n0 = (r - tm * (tm + 1) / 2) * BN;
+    } else {
+        const int band = r / (RASTER_W * p.tiles_n);
+        const int in_band = r - band * (RASTER_W * p.tiles_n);
+        const int w = min(RASTER_W, tiles_m - band * RASTER_W);
+        const int tn = in_band / w;
+        c.n0 = tn * BN;
+        c.m0 = (band * RASTER_W + (in_band - tn * w)) * BM;
+    }
     c.split = z / p.batch;
     c.bz = z - c.split * p.batch;
     return c;
@@ -200,7 +210,7 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const int tiles_m = (p.M + BM - 1) / BM;
-    const int per_z = tiles_m * p.tiles_n;
+    const int per_z = p.lower_only ? tiles_m * (tiles_m + 1) / 2 : tiles_m * p.tiles_n;
     if (t == 0) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
@@ -249,15 +259,6 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
     lb.init_thread(t);
     int p_tile = blockIdx.x, p_kt = 0, p_nkt = 0, p_kbeg = 0, p_kend = 0;
     unsigned p_it = 0;
-    auto next_live = [&](int tile) {   // skips the tiles strictly above the diagonal of a symmetric output
-        if (p.lower_only)
-            while (tile < total_tiles) {
-                const TileCoord c = decode_tile(p, tile, tiles_m, per_z);
-                if (c.n0 < c.m0 + BM) break;
-                tile += gridDim.x;
-            }
-        return tile;
-    };
     auto k_range = [&](int split, int &kb, int &ke) {
         kb = 0;
         ke = p.K;
@@ -267,7 +268,6 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
         }
     };
     auto prod_setup = [&]() {
-        p_tile = next_live(p_tile);
         if (p_tile >= total_tiles) return;
         const TileCoord c = decode_tile(p, p_tile, tiles_m, per_z);
         k_range(c.split, p_kbeg, p_kend);
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
 
     // ---- consumer
     unsigned it = 0;
-    for (int c_tile = next_live(blockIdx.x); c_tile < total_tiles; c_tile = next_live(c_tile + gridDim.x)) {
+    for (int c_tile = blockIdx.x; c_tile < total_tiles; c_tile += gridDim.x) {
         const TileCoord tc = decode_tile(p, c_tile, tiles_m, per_z);
         int kb, ke;
         k_range(tc.split, kb, ke);
@@ -461,7 +461,9 @@ void launch_p(const GemmParams &p_in, int num_sms)
     }
     GemmParams p = p_in;
     p.tiles_n = (p.N + BN - 1) / BN;
-    const long long tiles = (long long)((p.M + BM - 1) / BM) * p.tiles_n * p.batch * (p.ksplit > 1 ? p.ksplit : 1);
+    const long long tm = (p.M + BM - 1) / BM;
+    if (p.lower_only && tm != p.tiles_n) fail(-22, "tensor_gemm: a symmetric (lower_only) output needs M = N");
+    const long long tiles = (p.lower_only ? tm * (tm + 1) / 2 : tm * p.tiles_n) * p.batch * (p.ksplit > 1 ? p.ksplit : 1);
     if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
     const unsigned grid = (unsigned)std::min<long long>(tiles, num_sms);
     // 16-byte stores of column pairs: bit 0 for C through its maps, bit 1 for the split-K partial sums

@@ -302,3 +302,37 @@ def test_tensor_gemm_randomised_shapes_and_layouts(tt):
         ref = alpha * (A @ B) + (C0 if acc else 0.0)
         err = np.abs(dC.cpu().numpy() - ref).max()
         assert err <= 1e-11 * np.sqrt(K) * 4, (case, M, N, K, a_kfast, b_kfast, pad_a, pad_b, acc, err)
+
+
+@pytest.mark.parametrize("a_kfast", [False, True])
+@pytest.mark.parametrize("b_kfast", [False, True])
+@pytest.mark.parametrize("pad", [0, 1])
+def test_tensor_gemm_persistent_tile_all_layouts(tt, a_kfast, b_kfast, pad):
+    """The persistent 128x128 tile (gemm_p.cu): every operand layout (either index contiguous: the four
+    swizzled shared-memory tile formats), 16-byte and 8-byte copies (an odd leading dimension defeats the
+    16-byte path), ragged M / N / K tails, more tiles than SMs (several tiles per CTA: the pipeline runs
+    across tile boundaries), alpha and accumulation, 16-byte and scalar epilogue stores."""
+    import torch
+    rng = np.random.default_rng(7 + 2 * a_kfast + 4 * b_kfast + 8 * pad)
+    for (M, N, K, batch) in ((1500, 1301 + pad, 100, 1), (2100, 2048, 77, 1), (520, 524, 70, 6), (1024, 1024, 4100, 1)):
+        A, B = rng.standard_normal((batch, M, K)), rng.standard_normal((batch, K, N))
+        if a_kfast:
+            bufA = np.zeros((batch, M, K + pad)); bufA[:, :, :K] = A
+            am, ak, ab = [(M, K + pad)], [(K, 1)], [(batch, M * (K + pad))]
+        else:
+            bufA = np.zeros((batch, K, M + pad)); bufA[:, :, :M] = A.transpose(0, 2, 1)
+            am, ak, ab = [(M, 1)], [(K, M + pad)], [(batch, K * (M + pad))]
+        if b_kfast:
+            bufB = np.zeros((batch, N, K + pad)); bufB[:, :, :K] = B.transpose(0, 2, 1)
+            bk, bn, bb = [(K, 1)], [(N, K + pad)], [(batch, N * (K + pad))]
+        else:
+            bufB = np.zeros((batch, K, N + pad)); bufB[:, :, :N] = B
+            bk, bn, bb = [(K, N + pad)], [(N, 1)], [(batch, K * (N + pad))]
+        C0 = rng.standard_normal((batch, M, N))
+        dA, dB, dC = _dev(bufA), _dev(bufB), _dev(C0)
+        maps = dict(am=am, ak=ak, bk=bk, bn=bn, cm=[(M, N)], cn=[(N, 1)], ab=ab, bb=bb, cb=[(batch, M * N)])
+        tt.tensor_gemm(dA, dB, dC, M, N, K, maps, batch=batch, alpha=-0.5, accumulate=True)
+        torch.cuda.synchronize()
+        ref = -0.5 * np.einsum("bmk,bkn->bmn", A, B) + C0
+        err = np.abs(dC.cpu().numpy() - ref).max()
+        assert err <= 4e-11 * np.sqrt(K), (M, N, K, batch, err)
