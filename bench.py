@@ -44,11 +44,11 @@ CONFIGS = {
     "c5": dict(T=6.5, h=0.01, chi=64, r=2, q=3, seed=20241218, ramp=8),
 }
 # DRAM traffic of one launch of the dominant kernel, from the committed `ncu --set full` capture
-# (profiles/r1_gemm_a6ii_mbar_full.md: dram__bytes_read.sum + dram__bytes_write.sum), next to the
+# (profiles/r2_gemm_persistent_full.md: dram__bytes_read.sum + dram__bytes_write.sum), next to the
 # algorithmic bytes of that launch (each operand read once, the output written once)
-NCU_TRAFFIC = {"launch": "a6(ii) P = EM.F at c3: M=65536 N=2048 K=1024", "dram_bytes": 1.70e9,
+NCU_TRAFFIC = {"launch": "a6(ii) P = EM.F at c3: M=65536 N=2048 K=1024", "dram_bytes": 0.724769792e9 + 1.035347e9,
                "algorithmic_bytes": 8.0 * (65536 * 1024 + 1024 * 2048 + 65536 * 2048),
-               "source": "profiles/r1_gemm_a6ii_mbar_full.md"}
+               "source": "profiles/r2_gemm_persistent_full.md"}
 # nominal dense peaks of /opt/skills/guides (B200): FP64 tensor 45 TFLOP/s, bf16 2250 TFLOP/s
 FP64_OVER_BF16_NOMINAL = 45.0 / 2250.0
 
@@ -468,7 +468,7 @@ def run_ours(args, cfg, name):
                      "gemm_launches_per_step": (v["launches"][0] + v["launches"][1]) / K}
                  for k, v in gprof.items()}
     roofline = {"bound": "tensor",
-                "kernel": "tgemm_big_kernel<..,BN=128,WN=32,BK=32,STAGES=3,MBAR> (128x128 CTA tile, FP64 DMMA.8x8x4)",
+                "kernel": "tgemm_p_kernel<A_KF,B_KF,VEC> (persistent 128x128 CTA tile, FP64 DMMA.8x8x4, gemm_p.cu)",
                 "achieved": achieved, "peak": probe, "unit": "TFLOP/s", "frac": achieved / probe if probe > 0 else None,
                 "traffic": NCU_TRAFFIC["dram_bytes"],
                 "traffic_of": NCU_TRAFFIC,

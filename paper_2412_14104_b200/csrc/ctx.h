@@ -62,6 +62,7 @@ struct Ctx {
     cudaEvent_t ev[ST_COUNT + 1] = {};
     bool ev_ok = false;
     double stage_ms[ST_COUNT] = {};
+    double host_t[ST_COUNT + 1] = {};       // host clock at the stage marks (trace)
 
     long long launches = 0;
     double flops = 0;

@@ -14,6 +14,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <chrono>
 
 #include "ctx.h"
 
@@ -261,6 +262,7 @@ void stage_mark(int i)
     }
     TATRG_CUDA_CHECK(cudaEventRecord(c.ev[i], c.stream));
     c.cur_stage = i < ST_COUNT ? i : ST_COUNT - 1;
+    c.host_t[i] = std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
 }
 
 // Symmetric PSD eigenproblem of the n x n matrix S (overwritten): on exit the rows of Vt
@@ -1441,6 +1443,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         float ms = 0;
         cudaEventElapsedTime(&ms, c.ev[i], c.ev[i + 1]);
         c.stage_ms[i] = ms;
+    }
+    if (getenv("TATRG_TRACE")) {
+        fprintf(stderr, "tatrg-trace stages (gpu ms / host enqueue ms):");
+        for (int i = 0; i < ST_COUNT; ++i) fprintf(stderr, " %d: %.2f / %.2f", i, c.stage_ms[i], 1e3 * (c.host_t[i + 1] - c.host_t[i]));
+        fprintf(stderr, "\n");
     }
     if (c.prof) prof_collect();
 }

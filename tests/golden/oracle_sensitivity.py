@@ -30,6 +30,9 @@ if ROOT not in sys.path:
 RUNS = {
     "c1": dict(T=6.0, h=0.0, chi=6, r=2, q=2, seed=20241214, steps=8),
     "c2": dict(T=6.65, h=0.0, chi=16, r=2, q=2, seed=20241215, steps=40),
+    # the first steps of the wide-route golden (tests/golden/oracle_w80.json): legs 2 -> 4 -> 16 -> 40, where the
+    # pair operator K K_w^T still has exact rank deficiencies (no truncation has happened on those legs yet)
+    "w80": dict(T=6.5, h=0.01, chi=40, r=2, q=3, seed=20241218, steps=4),
 }
 SPECTRA = ("sigmaT", "sigma_swap", "SA", "SX", "SY", "SD", "s1", "s2", "s3")
 ULP = 2.0 ** -52
