@@ -534,7 +534,7 @@ struct OrthoChain {
     Ten T;
     RedBasis o;
     long long nk = 0;
-    Ten G1, G2, L1inv;
+    Ten G1, G1copy, G2, L1inv;
     int *flag = nullptr;
     double *dev = nullptr;
     struct Back {
@@ -543,6 +543,7 @@ struct OrthoChain {
         double err;
     } *back = nullptr;
     double err = INFINITY;
+    bool transposed_r = false;
 
     void alloc(const Ten &T_, char *pinned)   // on the main stream, before the fork
     {
@@ -554,14 +555,34 @@ struct OrthoChain {
         o.R = ws_tensor("kcb", {nk, n0, a});
         o.L2inv = ws_tensor("kl", {nk, nk});
         G1 = ws_tensor("cbde", {n0, a, n0, a});
+        G1copy = ws_tensor("cbde", {n0, a, n0, a});
         G2 = ws_tensor("kl", {nk, nk});
         L1inv = ws_tensor("kcb", {nk, n0, a});
         flag = (int *)ws_alloc(sizeof(int));
         dev = ws_doubles(1);
         TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
     }
-    void gram1() { contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true); }              // main
+    void gram1()                                                                                 // main
+    {
+        contract(T.as("cpqtb"), T.as("dpqte"), G1, 1.0, false, true);
+        d2d(G1copy.p, G1.p, nk * nk);
+    }
     void factor1() { cholesky_lower_async(G1.p, (int)nk, 0.0, L1inv.p, flag); }                 // side
+    // When T2 is numerically rank deficient (the ordered fixed point: cond(T2) beyond ~3e7) the plain
+    // factorisation breaks down: it is redone with a shift of 1e-13 max diag (above the rounding noise of
+    // G1).  T2 = Q1 L1^T holds by construction whatever the shift, which only decides how far Q1 is from
+    // orthonormal -- the extra pass takes care of that.
+    bool redo_shifted()
+    {
+        d2d(G1.p, G1copy.p, nk * nk);
+        if (!cholesky_lower(G1.p, (int)nk, 1e-13, L1inv.p)) return false;
+        contract(T.as("cpqtb"), L1inv, o.Q1);
+        contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
+        max_dev_identity(G2.p, (int)nk, dev);
+        err = d2h(dev, 1)[0];
+        if (getenv("TATRG_TRACE")) fprintf(stderr, "tatrg-trace ortho: shifted first pass, |G2 - I| = %.3e\n", err);
+        return std::isfinite(err);
+    }
     void basis()                                                                                 // main
     {
         contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
@@ -574,7 +595,33 @@ struct OrthoChain {
     {
         err = back->err;
         if (getenv("TATRG_TRACE")) fprintf(stderr, "tatrg-trace ortho: nk %lld |G2 - I| = %.3e flag %d\n", nk, err, back->flag);
-        return back->flag == 0 && err < 0.05;
+        return back->flag == 0 && std::isfinite(err);
+    }
+    bool failed_factor() const { return back->flag != 0 || !std::isfinite(back->err); }
+    // One more explicit pass when Q1 is too far from orthonormal for the implicit last pass (|G2 - I| >= 0.05:
+    // T2 ill conditioned, the shifted first pass left cond(Q1) up to ~1e6): G2 = L2 L2^T, Q2 = Q1 L2^-T
+    // written over Q1, G3 = Q2^T Q2; then the implicit pass on G3.  R = L3^T L2^T L1^T.
+    bool extra_pass()
+    {
+        Ten L2inv = ws_tensor("kl", {nk, nk});
+        if (!cholesky_lower(G2.p, (int)nk, 0.0, L2inv.p)) return false;
+        // L21[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]  (= (L1 L2)^T: the triangular factor so far)
+        Ten L21 = ws_tensor("ij", {nk, nk});
+        contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), L21);
+        d2d(G1.p, L21.p, nk * nk);                      // G1 now holds (L1 L2)^T row-major, used as "L1^T" below
+        {
+            size_t mk = ws_mark();
+            Ten Q2 = ws_tensor("pqtl", {o.Q1.legs[0].n, o.Q1.legs[1].n, o.Q1.legs[2].n, nk});
+            contract(o.Q1.as("pqtk"), L2inv.as("lk"), Q2);
+            d2d(o.Q1.p, Q2.p, Q2.size());
+            ws_release(mk);
+        }
+        contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
+        max_dev_identity(G2.p, (int)nk, dev);
+        err = d2h(dev, 1)[0];
+        if (getenv("TATRG_TRACE")) fprintf(stderr, "tatrg-trace ortho: extra pass, |G3 - I| = %.3e\n", err);
+        transposed_r = true;
+        return std::isfinite(err) && err < 0.05;
     }
     bool phase2()
     {
@@ -582,8 +629,10 @@ struct OrthoChain {
             near_identity_chol(G2.p, (int)nk, o.L2inv.p);
         else if (!cholesky_lower(G2.p, (int)nk, 0.0, o.L2inv.p))
             return false;
-        // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
-        contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
+        if (transposed_r)   // after an extra pass G1 holds the accumulated factor transposed: R[i][j] = sum_k L3[k][i] G1[k][j]
+            contract(G2.as("ki"), Ten::make(G1.p, "kj", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
+        else                // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
+            contract(G2.as("ki"), Ten::make(G1.p, "jk", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
         return true;
     }
 };
@@ -615,7 +664,10 @@ bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
         fk.join();
     }
     TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
-    bool ok = ch[0].usable() && ch[1].usable();
+    bool ok = true;
+    for (int i = 0; i < 2 && ok; ++i) ok = ch[i].usable() || (ch[i].failed_factor() && ch[i].redo_shifted());
+    for (int i = 0; i < 2 && ok; ++i)
+        if (ch[i].err >= 0.05) ok = ch[i].extra_pass();
     for (int i = 0; i < 2 && ok; ++i) ok = ch[i].phase2();
     bA = ch[0].o;
     bD = ch[1].o;
