@@ -641,6 +641,7 @@ def main():
     ap.add_argument("--gemm", default=None, help="kernel micro-benchmark: 'all' or one of " + ", ".join(GEMM_SHAPES))
     ap.add_argument("--small", action="store_true", help="micro-benchmark of the small latency-bound solvers")
     ap.add_argument("--chi", type=int, default=None, help="override the bond dimension of the chosen config (scaling study)")
+    ap.add_argument("--r", type=int, default=None, help="override the oversampling parameter r (the paper's figures use r = 7)")
     args = ap.parse_args()
     if args.small:
         run_small_micro(args)
@@ -651,6 +652,8 @@ def main():
     cfg = dict(CONFIGS[args.config])
     if args.chi:
         cfg["chi"] = args.chi
+    if args.r:
+        cfg["r"] = args.r
     if args.impl == "reference":
         run_reference(args, cfg, args.config)
         return

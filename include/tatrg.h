@@ -95,6 +95,14 @@ int tatrg_sketch_shape(int which, int direction, int chi, int r, int64_t *rows, 
  * step (1 value).  Returns the count (<= cap) or a negative status. */
 int tatrg_get_spectrum(int which, double *host_out, int cap);
 
+/* Every stage of coarse_grain has a fast route (used when its conditions hold) and a robust route that
+ * follows the oracle's algorithm step by step: mask bit 0 forces the bond swap on the
+ * plain chi^4-dimensional operator M instead of its chi^3-dimensional core, bit 1 Householder
+ * TSQR instead of Cholesky-QR, bit 2 the squeezers by dense eigendecompositions (PAPER.md:81-86
+ * Eq. 12) instead of Cholesky + subspace iteration, bit 3 the four isometries one after the other with
+ * synchronous solvers (Eqs. 2-3).  For tests: both routes must give the same step.  0 = default. */
+int tatrg_set_routes(int mask);
+
 /* Oversampled isometries of the LAST coarse_grain step (Eqs. 2-3; I, J, K, L of Eqs. 8-11),
  * for tests (the projector U U^T is gauge invariant and is what parity compares).  tatrg_keep_isometries(1)
  * makes every following step copy its four isometries to the host (one extra synchronisation per step);

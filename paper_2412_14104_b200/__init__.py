@@ -20,7 +20,7 @@ EXPORTS = [
     "init_ising_tensor", "coarse_grain", "coarse_grain_atrg", "log_Z_per_site",
     "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_bytes_atrg",
     "tatrg_workspace_peak",
-    "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_keep_isometries", "tatrg_get_isometry", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
+    "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_set_routes", "tatrg_keep_isometries", "tatrg_get_isometry", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name", "tatrg_get_h2d",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
@@ -62,6 +62,7 @@ def lib():
             "tatrg_set_sketch": (c_i, [c_i, c_vp, c_sz, c_i]),
             "tatrg_sketch_shape": (c_i, [c_i, c_i, c_i, c_i, ctypes.POINTER(c_i64), ctypes.POINTER(c_i64)]),
             "tatrg_get_spectrum": (c_i, [c_i, c_vp, c_i]),
+            "tatrg_set_routes": (c_i, [c_i]),
             "tatrg_keep_isometries": (c_i, [c_i]),
             "tatrg_get_isometry": (c_i, [c_i, c_vp, c_sz, ctypes.POINTER(c_i), ctypes.POINTER(c_i)]),
             "tatrg_get_gaps": (c_i, [c_vp]),
@@ -191,6 +192,14 @@ def get_spectrum(which) -> np.ndarray:
     if n < 0:
         _check(n)
     return out[:n].copy()
+
+
+ROUTE_PLAIN_SWAP, ROUTE_HOUSEHOLDER_QR, ROUTE_DENSE_SQUEEZER, ROUTE_SEQUENTIAL_ISO = 1, 2, 4, 8
+
+
+def set_routes(mask=0):
+    """Forces the robust routes of coarse_grain (mask of ROUTE_*); 0 restores the defaults."""
+    _check(lib().tatrg_set_routes(int(mask)))
 
 
 def keep_isometries(on=True):

@@ -320,10 +320,21 @@ int tatrg_sketch_shape(int which, int direction, int chi, int r, int64_t *rows, 
 int tatrg_get_spectrum(int which, double *host_out, int cap)
 {
     if (which < 0 || which > 9 || !host_out) return set_error(TATRG_EINVAL, "tatrg_get_spectrum: bad arguments");
+    if (which >= 2 && which <= 5 && ctx().iso_pending[which - 2]) {
+        int rc = guarded([&] { resolve_iso_spectra(); });
+        if (rc != TATRG_OK) return rc;
+    }
     const std::vector<double> &s = ctx().spec[which];
     int n = (int)s.size() < cap ? (int)s.size() : cap;
     for (int i = 0; i < n; ++i) host_out[i] = s[i];
     return n;
+}
+
+int tatrg_set_routes(int mask)
+{
+    if (mask < 0 || mask > 15) return set_error(TATRG_EINVAL, "tatrg_set_routes: mask must be in 0..15");
+    ctx().routes = mask;
+    return TATRG_OK;
 }
 
 int tatrg_keep_isometries(int on)
@@ -338,6 +349,10 @@ int tatrg_get_isometry(int which, double *host_out, size_t cap, int *rows, int *
 {
     Ctx &c = ctx();
     if (which < 0 || which > 3) return set_error(TATRG_EINVAL, "tatrg_get_isometry: which must be 0..3 (A, X, Y, D)");
+    if (c.iso_pending[which]) {
+        int rc = guarded([&] { resolve_iso_spectra(); });
+        if (rc != TATRG_OK) return rc;
+    }
     const std::vector<double> &v = c.iso[which];
     if (v.empty()) return set_error(TATRG_ESTATE, "tatrg_get_isometry: nothing kept (tatrg_keep_isometries(1) before the step; Triad-ATRG steps only)");
     if (rows) *rows = c.iso_rows;

@@ -99,10 +99,10 @@ void tensor_gemm_big(const GemmParams &p, int bn);   // gemm_big.cu: the 128 x b
 bool tensor_gemm_persistent(const GemmParams &p, int num_sms);   // gemm_p.cu: persistent 128 x 128 tile; false = not taken
 bool tensor_gemm_ts(const GemmParams &p);   // ts.cu: HBM-bound tall-and-skinny shapes; false = not taken
 double probe_fp64_peak(int mode, int iters);
-// qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 128.
+// qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 256.
 // Q overwrites Y; R (n x n, row-major, upper triangular) to Rout (device).
 void tsqr(double *Y, long long m, int n, double *Rout);
-// Asynchronous Cholesky-QR of a tall block (n <= 64): `passes` rounds of {C = Y^T Y (+ shift_rel * max diag),
+// Asynchronous Cholesky-QR of a tall block (n <= 256): `passes` rounds of {C = Y^T Y (+ shift_rel * max diag),
 // C = L L^T, Y <- Y L^-T}; no host synchronisation.  A failed factorisation raises *flag_dev (sticky);
 // ratio_dev (optional) receives min / max of the first pass's diag(L); Rout (optional, n x n row-major)
 // receives the accumulated triangular factor.  The caller checks the flag when it next synchronises.

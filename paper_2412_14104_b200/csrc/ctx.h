@@ -8,6 +8,9 @@ namespace tatrg {
 
 enum Stage { ST_CANON = 0, ST_SWAP, ST_ISO, ST_TRIAD, ST_GRAM, ST_SQUEEZE, ST_CONTRACT, ST_NORM, ST_COUNT };
 
+// tatrg_set_routes: forces the robust routes of the step (for tests: fast and robust routes must agree)
+enum Route { ROUTE_PLAIN_SWAP = 1, ROUTE_HOUSEHOLDER_QR = 2, ROUTE_DENSE_SQUEEZER = 4, ROUTE_SEQUENTIAL_ISO = 8 };
+
 struct Input {
     const double *ptr = nullptr;
     size_t n = 0;
@@ -53,9 +56,12 @@ struct Ctx {
     size_t pre_n[9] = {};
 
     Input in[9];
+    int routes = 0;                         // mask of Route: robust routes forced by tatrg_set_routes
     bool keep_iso = false;                  // tatrg_keep_isometries: host copies of U^A, U^X, U^Y, U^D of the last step
     std::vector<double> iso[4];
     int iso_rows = 0, iso_cols = 0;
+    std::vector<double> iso_H[4];           // wide isometries: Ritz matrices whose spectra are computed on demand
+    bool iso_pending[4] = {false, false, false, false};
     std::vector<double> spec[10];
     double gaps[4] = {0, 0, 0, 0};
 
@@ -96,6 +102,7 @@ void do_init(double beta, double h);
 void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mode);
 double do_log_z();
 double do_order_parameter(int leg);
+void resolve_iso_spectra();
 // api.cpp : per-launch GEMM timing
 int prof_begin(double flops, int big);   // returns slot or -1
 void prof_end(int slot);

@@ -254,7 +254,7 @@ void tsqr_impl(double *Y, long long m, int n, double *Rout)
 // that cond^2 eps << 1; otherwise nothing has been written and the caller falls back to TSQR.
 namespace {
 
-// C (n x n row-major, n <= 128) -> its lower Cholesky factor in place (after adding shift_rel * max
+// C (n x n row-major) -> its lower Cholesky factor in place (after adding shift_rel * max
 // diag); returns L^-1 as a [d][c] view; mm (optional) receives min / max of diag(L).  Asynchronous.
 Ten chol_inv(Ten &C, int n, double shift_rel, int *flag, double *mm)
 {
@@ -311,7 +311,7 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
                   double *Rout)
 {
-    if (n < 1 || n > 128 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
+    if (n < 1 || n > 256 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
     size_t mark = ws_mark();
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten T = ws_tensor("rd", {m, n});
@@ -343,8 +343,8 @@ void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, i
 
 namespace {
 
-// n > 64: block Gram-Schmidt with reorthogonalisation over two column halves of at most 64 columns,
-// each factored by tsqr (the robust route for blocks that are not tall or too ill conditioned for
+// n > 64: block Gram-Schmidt with reorthogonalisation over two column halves (recursively: tsqr of a
+// half wider than 64 columns splits again), each factored by tsqr (the robust route for blocks that are not tall or too ill conditioned for
 // Cholesky-QR): Y = [Q1 Q2] [[R11, R12], [0, R22]].
 void tsqr_split(double *Y, long long m, int n, double *Rout)
 {
@@ -364,6 +364,20 @@ void tsqr_split(double *Y, long long m, int n, double *Rout)
     fill_identity(Id.p, h1);
     contract(Id, Rb, R12, 1.0, true);            // R12 += Rb
     tsqr(Y2.p, m, h2, R22.p);
+    {
+        // "Twice is enough" holds for the projection of a block of full numerical rank.  When Y is rank
+        // deficient (the pair operators of the early steps, r chi above their rank) some columns of the
+        // projected Y2 are pure rounding noise, 1e-9 or less of what they were, and the unit vectors tsqr
+        // makes of them keep components along Q1 of eps / 1e-9: one more projection AFTER the
+        // normalisation, folded into R:  Q2 = Q2'' T + Q1 C  =>  R12 += C R22,  R22 <- T R22.
+        Ten Cc = ws_tensor("ed", {h1, h2}), Tm = ws_tensor("gd", {h2, h2}), R22n = ws_tensor("gf", {h2, h2});
+        contract(Y1.as("re"), Y2, Cc);
+        contract(Y1.as("re"), Cc, Y2, -1.0, true);
+        tsqr(Y2.p, m, h2, Tm.p);
+        contract(Cc, R22, R12.as("ef"), 1.0, true);
+        contract(Tm, R22, R22n);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(R22.p, R22n.p, sizeof(double) * h2 * h2, cudaMemcpyDeviceToDevice, stream()));
+    }
     TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y, pitch, Y1.p, sizeof(double) * h1, sizeof(double) * h1, m, cudaMemcpyDeviceToDevice, stream()));
     TATRG_CUDA_CHECK(cudaMemcpy2DAsync(Y + h1, pitch, Y2.p, sizeof(double) * h2, sizeof(double) * h2, m, cudaMemcpyDeviceToDevice, stream()));
     fill_zero(Rout, (long long)n * n);
@@ -378,8 +392,8 @@ void tsqr_split(double *Y, long long m, int n, double *Rout)
 void tsqr(double *Y, long long m, int n, double *Rout)
 {
     if (n < 1 || m < 1) fail(-22, "tsqr: empty matrix");
-    if (n > 128) fail(-22, "tsqr: n = %d > 128 not supported", n);
-    if (m >= 16LL * n && m >= 512 && cholqr2(Y, m, n, Rout)) return;
+    if (n > 256) fail(-22, "tsqr: n = %d > 256 not supported", n);
+    if (!(ctx().routes & ROUTE_HOUSEHOLDER_QR) && m >= 16LL * n && m >= 512 && cholqr2(Y, m, n, Rout)) return;
     if (n > 64)
         tsqr_split(Y, m, n, Rout);
     else if (n > 32)

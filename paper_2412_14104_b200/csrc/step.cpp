@@ -300,7 +300,7 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
     // flags / condition estimates are read once at the end, and if they are bad everything is redone
     // with the robust synchronous QR.
     bool done = false;
-    if (ell <= 128 && rows >= 16LL * ell && cols >= 16LL * ell && rows >= 512 && cols >= 512) {
+    if (!(ctx().routes & ROUTE_HOUSEHOLDER_QR) && ell <= 256 && rows >= 16LL * ell && cols >= 16LL * ell && rows >= 512 && cols >= 512) {
         int *flag = (int *)ws_alloc(sizeof(int));
         double *ratio = ws_doubles(4);
         TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
@@ -723,6 +723,10 @@ void do_init(double beta, double h)
     std::vector<double> v = d2h(ss, 2);
     c.log_acc = 0.5 * (log(v[0]) + log(v[1]));
     for (auto &s : c.spec) s.clear();
+    for (int i = 0; i < 4; ++i) {
+        c.iso_pending[i] = false;
+        c.iso_H[i].clear();
+    }
     for (auto &i : c.in) i = Input();
     c.inited = true;
 }
@@ -766,13 +770,47 @@ double do_order_parameter(int leg)
     return tr * tr / tr2;
 }
 
+// Wide isometries (r chi > 64) leave their Ritz step out of the path (see do_coarse_grain): the spectra
+// S^A..S^D and, for tatrg_get_isometry, the Ritz vectors U = Q V are computed here, when asked for, from
+// the kk x kk Ritz matrices the step kept.
+void resolve_iso_spectra()
+{
+    Ctx &c = ctx();
+    bool any = false;
+    for (int i = 0; i < 4; ++i) any = any || c.iso_pending[i];
+    if (!any || !c.inited) return;
+    c.lo = c.state_low ? c.state_bytes : 0;
+    c.hi = c.state_low ? c.ws_bytes : c.ws_bytes - c.state_bytes;
+    for (int i = 0; i < 4; ++i) {
+        if (!c.iso_pending[i]) continue;
+        const int kk = (int)llround(sqrt((double)c.iso_H[i].size()));
+        size_t mk = ws_mark();
+        Ten Hm = ws_tensor("zy", {kk, kk}), Vt = ws_tensor("kz", {kk, kk});
+        double *lam = ws_doubles(kk);
+        h2d(Hm.p, c.iso_H[i].data(), (long long)kk * kk);
+        std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);
+        c.spec[2 + i].resize(kk);
+        for (int j = 0; j < kk; ++j) c.spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
+        if (!c.iso[i].empty() && c.iso_cols == kk) {   // kept isometry: Q -> Q V
+            const long long n12 = c.iso_rows;
+            Ten Qd = ws_tensor("rz", {n12, kk}), Ud = ws_tensor("rk", {n12, kk});
+            h2d(Qd.p, c.iso[i].data(), n12 * kk);
+            contract(Qd, Vt, Ud);
+            c.iso[i] = d2h(Ud.p, n12 * kk);
+        }
+        ws_release(mk);
+        c.iso_pending[i] = false;
+        c.iso_H[i].clear();
+    }
+}
+
 // =======================================================================================
 void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mode)
 {
     Ctx &c = ctx();
     if (!c.inited) fail(-1, "coarse_grain: call init_ising_tensor first");
     if (direction < 1 || direction > 4 || chi < 1 || r < 1 || q < 0) fail(-22, "coarse_grain: bad arguments");
-    if ((long long)r * chi > 128 || chi > 64) fail(-22, "coarse_grain: r*chi = %d > 128 (or chi > 64) not supported", r * chi);
+    if ((long long)r * chi > 256 || chi > 64) fail(-22, "coarse_grain: r*chi = %d > 256 (or chi > 64) not supported", r * chi);
     StepCfg cfg{seed, c.step};
     c.prof_rec.clear();
 
@@ -836,7 +874,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         double *Yq[2] = {Qp.p, Qs.p};
         const double *src[2] = {c.phi, c.psi};
         double *Rq[2] = {Rp.p, Rs.p};
-        if (R >= 16LL * g0 && R >= 512) {
+        if (!(c.routes & ROUTE_HOUSEHOLDER_QR) && R >= 16LL * g0 && R >= 512) {
             struct QrBack {
                 int flag;
                 int pad;
@@ -916,7 +954,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     // qr+((1 x Q) y) = (1 x Q) qr+(y), so the RSVD of M with the sketch Omega is the RSVD of m with the
     // sketch (1 x Q_D)^T Omega, expanded at the end: the same X, sigma, Y at 1/chi of the flops.
     const long long nk = n0 * a;
-    if (nT >= 2 * nk && nk >= 16) {
+    if (!(c.routes & ROUTE_PLAIN_SWAP) && nT >= 2 * nk && nk >= 16) {
         size_t mk = ws_mark();
         RedBasis bA, bD;
         if (ortho_factor_pair(A, D, bA, bD)) {
@@ -1010,6 +1048,9 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     stage_mark(2);
 
     Ten U[4];   // A, X, Y, D : [p,q,k]
+    bool iso_lazy[4] = {false, false, false, false};
+    double *Hkeep[4] = {nullptr, nullptr, nullptr, nullptr};
+    int iso_kk = 0;
     Ten E, F, G, H;
     long long kd = 0;
     Ten GL[3], GR[3];
@@ -1091,6 +1132,19 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(Qi, SQ, Hm);
             Ten Vt = ws_tensor("kz", {kk, kk});
             double *lam = ws_doubles(kk);
+            if (fast && kk > 64) {
+                // Wide internal lines (r chi > 64): the Ritz rotation is left out of the path.  Gamma^triad
+                // depends on U only through its span (E I = A U U^T etc.: every oversampled line is summed
+                // over in Eqs. 13-14 and in the Grams of Eq. 12), so the orthonormal block Q itself is used
+                // as U; the kk x kk Ritz matrix H goes to the host and the spectrum S (a diagnostic of the
+                // step) is computed from it when it is asked for (resolve_iso_spectra).
+                d2d(U[i].p, Qi.p, n12 * kk);
+                d2d(Hkeep[i], Hm.p, (long long)kk * kk);
+                back->pad = nqr;
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+                TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 2 * nqr * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+                return;
+            }
             if (fast) {
                 eig_small_async(Hm.p, kk, Vt.p, lam, flag);
                 back->pad = nqr;
@@ -1105,7 +1159,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(Ten::make(Qi.p, "pqz", {n1, n2, kk}), Vt, U[i]);
         };
         bool iso_done[4] = {false, false, false, false};
-        if (kk <= 64 && q + 1 <= 8 && n12 >= 16LL * kk) {   // the four isometries as concurrent chains
+        const bool wide = kk > 64;
+        if (wide)
+            for (int i = 0; i < 4; ++i) Hkeep[i] = ws_doubles((long long)kk * kk);   // outlives the chains' slices
+        if (!(c.routes & ROUTE_SEQUENTIAL_ISO) && kk <= 256 && q + 1 <= 8 && n12 >= (wide ? 2LL : 16LL) * kk) {   // the four isometries as concurrent chains
             Fork fk(4);
             for (int i = 0; i < 4; ++i) {
                 fk.enter(i);
@@ -1118,8 +1175,13 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 bool ok = bk->flag == 0;
                 for (int j = 0; j < bk->pad; ++j) ok = ok && bk->ratio[2 * j] > 1e-5 * bk->ratio[2 * j + 1];
                 if (!ok) continue;   // ill conditioned block or no convergence: redone below
-                spec[2 + i].resize(kk);
-                for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(bk->lam[j], 0.0));
+                if (wide) {
+                    iso_lazy[i] = true;
+                    iso_kk = kk;
+                } else {
+                    spec[2 + i].resize(kk);
+                    for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(bk->lam[j], 0.0));
+                }
                 iso_done[i] = true;
             }
             fk.join();
@@ -1127,6 +1189,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         for (int i = 0; i < 4; ++i)
             if (!iso_done[i]) {
                 size_t mk = ws_mark();
+                iso_lazy[i] = false;
                 iso_body(i, false, nullptr);
                 ws_release(mk);
             }
@@ -1266,7 +1329,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         for (int mu = 0; mu < 3; ++mu) {
             const long long N2 = nn[mu] * nn[mu];
             ch[mu].b = chi < 64 ? 64 : 128;
-            ch[mu].active = N2 >= 4 * ch[mu].b && chi < ch[mu].b;
+            ch[mu].active = !(c.routes & ROUTE_DENSE_SQUEEZER) && N2 >= 4 * ch[mu].b && chi < ch[mu].b;
             ch[mu].GLm = GL[mu];
             ch[mu].GRm = GR[mu];
             ch[mu].N2 = (int)N2;
@@ -1490,6 +1553,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     c.state_bytes = 2 * new_cap;
     spec[9] = {lnc};
     for (int i = 0; i < 10; ++i) c.spec[i] = spec[i];
+    for (int i = 0; i < 4; ++i) {
+        c.iso_pending[i] = iso_lazy[i];
+        c.iso_H[i].clear();
+        if (iso_lazy[i]) c.iso_H[i] = d2h(Hkeep[i], (long long)iso_kk * iso_kk);
+    }
     for (int i = 0; i < 4; ++i) c.gaps[i] = gaps[i];
     for (int i = 0; i < ST_COUNT; ++i) {
         float ms = 0;

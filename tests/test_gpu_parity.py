@@ -13,20 +13,30 @@ pytestmark = pytest.mark.gpu
 
 LNZ_RTOL = 1e-10
 SPEC_TOL = 1e-9
-# S^A..S^D are Ritz values after q unconverged subspace iterations, not truncated spectra.  The oracle's own
-# conditioning (tests/golden/oracle_sensitivity_c2*.json: the oracle against itself with its sketches moved by
-# 1 and by 64 ulps) moves them 10-27 times further than sigma^T / sigma_swap / s^(mu) along config 2's 40
-# steps; the CUDA path shows the same ratio (sigma^T 1.3e-10, S^D 3.3e-9 at worst, whether it is fed the
-# oracle's bytes or its own generator's).  They are held to 1e-9 like the rest wherever that is reached
-# (config 1, config 3's 12 stored steps, config 4, the wide routes, config 2 up to step 21) and to
-# RITZ_TOL_LATE on config 2's late steps only.
-RITZ_TOL_LATE = 1e-8
-# The isometries themselves, gauge invariant (reading G18): max |U S U^T - U_o S_o U_o^T| / S_1, the Ritz
-# vectors weighted by their Ritz values (the plain projector U U^T is not unique when K K^T has fewer than
-# r chi non-zero eigenvalues, as in the early steps: the trailing Ritz vectors then span an arbitrary part
-# of the null space and carry zero weight in Gamma)
-PROJ_TOL = 1e-9        # measured: <= 7e-13 on configs 1, 3; 9.6e-9 at worst on config 2's late steps
-PROJ_TOL_LATE = 3e-8
+# The isometries themselves, gauge invariant (reading G18): max |U S^2 U^T - U_o S_o^2 U_o^T| / S_1^2, the
+# Ritz approximation Q H Q^T of the pair operator K K_w^T that the Ritz step diagonalises.  (The plain
+# projector U U^T is not unique when K K_w^T has fewer than r chi non-zero eigenvalues, as in the early
+# steps: the trailing Ritz vectors then span an arbitrary part of the null space and carry no weight in
+# Gamma; for the same reason the spectra S^A..S^D are compared through lambda = S^2, see below.)
+PROJ_TOL = 1e-9
+# config 2's steps 22..40: the two sides' tensors have drifted apart by 1e-10 (sigma^T) and the Ritz VECTORS of
+# q = 2 unconverged iterations follow with the amplification the oracle's own Ritz values show against itself
+# (10-27x, oracle_sensitivity_c2*.json); measured 2.6e-9 at worst
+PROJ_TOL_LATE = 1e-8
+def spectrum_deviation(name, so, sg):
+    """Reading G13: max_i |s_i - s_i^ref| / s_1^ref for the truncated spectra (sigma^T, sigma_swap, s^(mu)).
+    S^A..S^D are square roots of the Ritz values lambda of the pair operator K K_w^T, which the Ritz step
+    (oracle: eigh of Q^T S Q) determines to eps lambda_1 in absolute terms: a Ritz value at rounding level
+    (rank-deficient K K_w^T in the early steps, r chi above the rank) has a square root anywhere below
+    ~1e-8 S_1, and the oracle's own S^X moves by 2.8e-10 S_1 under a 1-ulp change of its sketches there
+    (tests/golden/oracle_sensitivity_w80.json) while its sigma's move by 1e-15; along config 2's 40 steps the
+    oracle's S^A..S^D move 10-27 times further than its sigma's (oracle_sensitivity_c2*.json).  They are
+    therefore compared through lambda = S^2, the quantity that is determined:
+    max_i |lambda_i - lambda_i^ref| / lambda_1^ref (for S_i ~ S_1 this is twice as strict as the plain rule;
+    measured on config 2's 40 steps: 3.2e-10 at worst, where the plain rule reads 3.3e-9)."""
+    if name in ("SA", "SX", "SY", "SD"):
+        return float(np.abs(so ** 2 - sg ** 2).max() / so[0] ** 2)
+    return float(np.abs(so - sg).max() / so[0])
 
 
 @pytest.fixture(scope="module")
@@ -64,30 +74,26 @@ def run_both(tt, beta, h, chi, r, q, n_steps, seed, directions=None, mode="triad
                 assert uo.shape == ug.shape, (m, t, uo.shape, ug.shape)
                 so, sg = np.asarray(rec["S" + t]), tt.get_spectrum("S" + t)
                 if len(so):
-                    out["proj"][t] = float(np.abs((uo * so) @ uo.T - (ug * sg) @ ug.T).max() / so[0])
+                    out["proj"][t] = float(np.abs((uo * so ** 2) @ uo.T - (ug * sg ** 2) @ ug.T).max() / so[0] ** 2)
         recs.append(out)
     tt.keep_isometries(False)
     return recs
 
 
-def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL, ritz_late=None):
-    """ritz_late = (first 0-based step, tolerance): S^A..S^D from that step on are held to that tolerance."""
+def check(recs, lnz_rtol=LNZ_RTOL, spec_tol=SPEC_TOL, proj_late=None):
     worst = {}
     for o in recs:
         assert tuple(o["dims_o"]) == tuple(o["dims_g"]), o
         for name, (so, sg) in o["spec"].items():
             assert len(so) == len(sg), (o["step"], name, len(so), len(sg))
             if len(so):
-                tol = spec_tol
-                if ritz_late and name in ("SA", "SX", "SY", "SD") and o["step"] >= ritz_late[0]:
-                    tol = ritz_late[1]
-                dev = np.abs(so - sg).max() / so[0]
+                dev = spectrum_deviation(name, so, sg)
                 worst[name] = max(worst.get(name, 0.0), dev)
-                assert dev <= tol, (o["step"], name, dev)
+                assert dev <= spec_tol, (o["step"], name, dev)
         for t, dev in o["proj"].items():
             worst["P" + t] = max(worst.get("P" + t, 0.0), dev)
-            ptol = PROJ_TOL_LATE if (ritz_late and o["step"] >= ritz_late[0]) else PROJ_TOL
-            assert dev <= ptol, (o["step"], "projector U^" + t, dev)
+            ptol = PROJ_TOL_LATE if (proj_late is not None and o["step"] >= proj_late) else PROJ_TOL
+            assert dev <= ptol, (o["step"], "Ritz operator of U^" + t, dev)
         dz = abs(o["lnz_g"] / o["lnz_o"] - 1)
         worst["lnz"] = max(worst.get("lnz", 0.0), dz)
         assert dz <= lnz_rtol, (o["step"], o["lnz_g"], o["lnz_o"])
@@ -116,7 +122,7 @@ def test_direction_orders_with_field(tt, dirs):
 def test_config2_chi16_all_40_steps(tt):
     """BASELINE.json configs[1] (T=6.65, chi=16, r=2, q=2) in full: 40 steps, L = 2^10 per direction.
     (Measured: ln Z/V agrees to 3e-15 at every step, the spectra to 5e-10.)"""
-    check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 40, 20241215), ritz_late=(21, RITZ_TOL_LATE))
+    check(run_both(tt, 1 / 6.65, 0.0, 16, 2, 2, 40, 20241215), proj_late=21)
 
 
 def test_config3_chi32_first_steps_incl_one_full_size_step(tt):
@@ -125,6 +131,20 @@ def test_config3_chi32_first_steps_incl_one_full_size_step(tt):
     (reduced bond swap, concurrent isometry / squeezer chains, 64-column sketches); the oracle needs
     about a minute for it."""
     check(run_both(tt, 1 / 6.65, 0.0, 32, 2, 2, 5, 20241216))
+
+
+def test_r7_parity_chi10(tt):
+    """The paper's oversampling r = 7 (Table 2 and Figs. 4-6 are at r = 7), 8 steps at
+    chi = 10.  (Not chi = 8: there the second bond swap cuts a four-fold degenerate multiplet of singular
+    values 0.1568 s_1 in the middle -- the oracle logs gap_swap = 5e-17 --, so which vectors are kept is not
+    determined and no two implementations agree beyond the truncation error; reading G12.)"""
+    check(run_both(tt, 1 / 6.65, 0.0, 10, 7, 2, 8, 424242))
+
+
+def test_r7_wide_internal_lines_chi20(tt):
+    """r chi = 140 > 128: sketches, Cholesky-QR panels and Ritz cores between 129 and 256 columns wide
+    (5 steps of chi = 20, r = 7, q = 1; the fifth has 140 of 256 pair states kept by the isometries)."""
+    check(run_both(tt, 1 / 6.65, 0.0, 20, 7, 1, 5, 434343))
 
 
 def test_plain_atrg_parity(tt):
@@ -236,7 +256,7 @@ def test_errors_leave_the_state_intact(tt):
     tt.coarse_grain(2, 6, 2, 2, 1)
     before, dims = tt.log_Z_per_site(), tt.get_dims()
     for args in ((0, 6, 2, 2, 1), (5, 6, 2, 2, 1), (1, 0, 2, 2, 1), (1, 6, 0, 2, 1), (1, 6, 2, -1, 1), (1, 65, 2, 2, 1),
-                 (1, 64, 3, 2, 1)):
+                 (1, 64, 5, 2, 1)):
         with pytest.raises(t.TatrgError):
             tt.coarse_grain(*args)
     with pytest.raises(t.TatrgError):
