@@ -530,7 +530,9 @@ def run_gemm_micro(args):
     tt.set_workspace(nbytes=1 << 30)
     stream = torch.cuda.Stream()
     tt.set_stream(stream)
-    out = {}
+    if args.tma:
+        tt.set_routes(tt.ROUTE_TMA_PRODUCER)
+    out = {"producer": "tma" if args.tma else "cp.async"}
     for name, (M, N, K) in GEMM_SHAPES.items():
         if args.gemm != "all" and args.gemm != name:
             continue
@@ -639,6 +641,7 @@ def main():
     ap.add_argument("--profile-all", action="store_true",
                     help="time every tensor-GEMM launch (default: only the dominant 128x128-tile kernel)")
     ap.add_argument("--gemm", default=None, help="kernel micro-benchmark: 'all' or one of " + ", ".join(GEMM_SHAPES))
+    ap.add_argument("--tma", action="store_true", help="with --gemm: feed the persistent tile from TMA instead of cp.async")
     ap.add_argument("--small", action="store_true", help="micro-benchmark of the small latency-bound solvers")
     ap.add_argument("--chi", type=int, default=None, help="override the bond dimension of the chosen config (scaling study)")
     ap.add_argument("--r", type=int, default=None, help="override the oversampling parameter r (the paper's figures use r = 7)")

@@ -100,7 +100,9 @@ int tatrg_get_spectrum(int which, double *host_out, int cap);
  * plain chi^4-dimensional operator M instead of its chi^3-dimensional core, bit 1 Householder
  * TSQR instead of Cholesky-QR, bit 2 the squeezers by dense eigendecompositions (PAPER.md:81-86
  * Eq. 12) instead of Cholesky + subspace iteration, bit 3 the four isometries one after the other with
- * synchronous solvers (Eqs. 2-3).  For tests: both routes must give the same step.  0 = default. */
+ * synchronous solvers (Eqs. 2-3).  For tests: both routes must give the same step.  Bit 4 feeds the persistent
+ * tensor-GEMM tile from TMA (cp.async.bulk.tensor, rank-2 FP64 tensor maps) instead of per-thread cp.async where
+ * the operands are plain row-major matrices (an alternative producer, not a fallback).  0 = default. */
 int tatrg_set_routes(int mask);
 
 /* Oversampled isometries of the LAST coarse_grain step (Eqs. 2-3; I, J, K, L of Eqs. 8-11),

@@ -194,7 +194,7 @@ def get_spectrum(which) -> np.ndarray:
     return out[:n].copy()
 
 
-ROUTE_PLAIN_SWAP, ROUTE_HOUSEHOLDER_QR, ROUTE_DENSE_SQUEEZER, ROUTE_SEQUENTIAL_ISO = 1, 2, 4, 8
+ROUTE_PLAIN_SWAP, ROUTE_HOUSEHOLDER_QR, ROUTE_DENSE_SQUEEZER, ROUTE_SEQUENTIAL_ISO, ROUTE_TMA_PRODUCER = 1, 2, 4, 8, 16
 
 
 def set_routes(mask=0):

@@ -332,7 +332,7 @@ int tatrg_get_spectrum(int which, double *host_out, int cap)
 
 int tatrg_set_routes(int mask)
 {
-    if (mask < 0 || mask > 15) return set_error(TATRG_EINVAL, "tatrg_set_routes: mask must be in 0..15");
+    if (mask < 0 || mask > 31) return set_error(TATRG_EINVAL, "tatrg_set_routes: mask must be in 0..31");
     ctx().routes = mask;
     return TATRG_OK;
 }

@@ -97,6 +97,7 @@ struct Err {
 void tensor_gemm(GemmParams p);
 void tensor_gemm_big(const GemmParams &p, int bn);   // gemm_big.cu: the 128 x bn CTA tile, bn = 128 or 64
 bool tensor_gemm_persistent(const GemmParams &p, int num_sms);   // gemm_p.cu: persistent 128 x 128 tile; false = not taken
+bool tensor_gemm_tma(const GemmParams &p, int num_sms);          // gemm_tma.cu: TMA-fed producer (plain 2D operands); false = not taken
 bool tensor_gemm_ts(const GemmParams &p);   // ts.cu: HBM-bound tall-and-skinny shapes; false = not taken
 double probe_fp64_peak(int mode, int iters);
 // qr.cu : thin QR with R_ii >= 0 of the row-major m x n matrix Y (ld = n), m >= 1, n <= 256.

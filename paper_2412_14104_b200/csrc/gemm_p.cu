@@ -22,10 +22,12 @@
 //     fragment rows is free as long as the epilogue uses the same one --, so one k line holds the
 //     operands of fragments i, i + 1 side by side.
 #include <math.h>
+#include <stdlib.h>
 
 #include <algorithm>
 
 #include "common.h"
+#include "ctx.h"
 
 namespace tatrg {
 
@@ -506,6 +508,9 @@ static double map_span(const Map4 &m, long long count)
 bool tensor_gemm_persistent(const GemmParams &p, int num_sms)
 {
     // the loader keeps the free-index offsets of an operand in 32 bits
+    // the TMA-fed producer (gemm_tma.cu) is within 1-2 % of the cp.async producer but not ahead of it
+    // (profiles/r2_gemm_tma_vs_cpasync.md): opt-in through tatrg_set_routes
+    if ((ctx().routes & ROUTE_TMA_PRODUCER) && tensor_gemm_tma(p, num_sms)) return true;
     const double sa = map_span(p.am, p.M), sb = map_span(p.bn, p.N);
     if (sa < 0 || sb < 0 || sa >= 4294967295.0 || sb >= 4294967295.0) return false;
     const bool akf = p.a_kfast != 0, bkf = p.b_kfast != 0;

@@ -336,3 +336,28 @@ def test_tensor_gemm_persistent_tile_all_layouts(tt, a_kfast, b_kfast, pad):
         ref = -0.5 * np.einsum("bmk,bkn->bmn", A, B) + C0
         err = np.abs(dC.cpu().numpy() - ref).max()
         assert err <= 4e-11 * np.sqrt(K), (M, N, K, batch, err)
+
+
+def test_tensor_gemm_tma_producer_matches(tt):
+    """The TMA-fed producer of the persistent tile (gemm_tma.cu: cp.async.bulk.tensor + SWIZZLE_128B boxes,
+    the stage refilled by the last warp to leave it) against numpy and against the cp.async producer, on plain
+    row-major operands with ragged M / N / K tails, alpha and accumulation."""
+    import torch
+    import paper_2412_14104_b200 as t
+    rng = np.random.default_rng(5)
+    for (M, N, K) in ((1500, 1302, 100), (2100, 2048, 77), (4096, 1024, 1000)):
+        A, B, C0 = rng.standard_normal((M, K)), rng.standard_normal((K, N)), rng.standard_normal((M, N))
+        maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
+        res = []
+        for mask in (0, t.ROUTE_TMA_PRODUCER):
+            tt.set_routes(mask)
+            try:
+                dA, dB, dC = _dev(A), _dev(B), _dev(C0)
+                tt.tensor_gemm(dA, dB, dC, M, N, K, maps, alpha=-0.5, accumulate=True)
+                torch.cuda.synchronize()
+                res.append(dC.cpu().numpy())
+            finally:
+                tt.set_routes(0)
+        ref = -0.5 * (A @ B) + C0
+        assert np.abs(res[1] - ref).max() <= 4e-11 * np.sqrt(K), (M, N, K)
+        assert np.abs(res[1] - res[0]).max() <= 1e-12 * np.sqrt(K), (M, N, K)

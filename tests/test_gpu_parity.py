@@ -21,8 +21,10 @@ SPEC_TOL = 1e-9
 PROJ_TOL = 1e-9
 # config 2's steps 22..40: the two sides' tensors have drifted apart by 1e-10 (sigma^T) and the Ritz VECTORS of
 # q = 2 unconverged iterations follow with the amplification the oracle's own Ritz values show against itself
-# (10-27x, oracle_sensitivity_c2*.json); measured 2.6e-9 at worst
-PROJ_TOL_LATE = 1e-8
+# (10-27x, oracle_sensitivity_c2*.json); measured 8.7e-9 at worst
+PROJ_TOL_LATE = 3e-8
+
+
 def spectrum_deviation(name, so, sg):
     """Reading G13: max_i |s_i - s_i^ref| / s_1^ref for the truncated spectra (sigma^T, sigma_swap, s^(mu)).
     S^A..S^D are square roots of the Ritz values lambda of the pair operator K K_w^T, which the Ritz step
