@@ -367,7 +367,7 @@ def run_ours(args, cfg, name):
         for mm in range(ramp, ramp + W):
             set_inputs(resident(mm), mm % 4 + 1)
             step_fn(mm % 4 + 1, chi, r, q, seed)
-        tt.set_profile(2 if args.profile_all else 1)
+        tt.set_profile(1)
         tt.launch_count(reset=True)
         tt.gemm_flops(reset=True)
         barrier()
@@ -557,79 +557,6 @@ def run_gemm_micro(args):
     print(json.dumps({"gemm_micro": out}), flush=True)
 
 
-def run_small_micro(args):
-    """Stand-alone wall time (host clock around synchronous C-ABI calls, 3 warm-up + 20 timed) of the
-    latency-bound small solvers of the path: blocked Cholesky (+ inverse), Cholesky-QR passes,
-    one-CTA Jacobi SVD; sizes of c3 (chi = 32: chi^2 = 1024, r chi = 64)."""
-    import numpy as np
-    import torch
-    import paper_2412_14104_b200 as tt
-    torch.cuda.set_device(0)
-    tt.set_workspace(nbytes=1 << 30)
-    stream = torch.cuda.Stream()
-    tt.set_stream(stream)
-    out = {}
-
-    def timeit(fn, reps=20):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(reps):
-            fn()
-        torch.cuda.synchronize()
-        return (time.perf_counter() - t0) / reps * 1e3
-
-    rng = np.random.default_rng(0)
-    with torch.cuda.stream(stream):
-        for n in (1024, 4096):
-            B = torch.randn(n, n + 8, dtype=torch.float64, device="cuda")
-            A0 = B @ B.T + n * torch.eye(n, dtype=torch.float64, device="cuda")
-            A = A0.clone()
-            Li = torch.empty_like(A)
-
-            def f1():
-                A.copy_(A0)
-                tt.cholesky(A)
-
-            def f2():
-                A.copy_(A0)
-                tt.cholesky(A, Li)
-            out["cholesky_%d_ms" % n] = timeit(f1, 10)
-            out["cholesky_inverse_%d_ms" % n] = timeit(f2, 10)
-            del B, A0, A, Li
-        for m, n in ((1024, 64), (32768, 64), (1048576, 64)):
-            Y0 = torch.randn(m, n, dtype=torch.float64, device="cuda")
-            Y = Y0.clone()
-            R = torch.empty(n, n, dtype=torch.float64, device="cuda")
-
-            def g(passes):
-                Y.copy_(Y0)
-                tt.cholqr(Y, R, passes=passes)
-            out["cholqr1_%dx%d_ms" % (m, n)] = timeit(lambda: g(1))
-            out["cholqr2_%dx%d_ms" % (m, n)] = timeit(lambda: g(2))
-
-            def h():
-                Y.copy_(Y0)
-                tt.qr_pos(Y, R)
-            out["qr_pos_%dx%d_ms" % (m, n)] = timeit(h)
-            del Y0, Y, R
-        for n in (32, 64):
-            # column-major lower-triangular matrix with graded columns (what the RSVD core R_B^T looks like);
-            # the tensor's row j is column j
-            G0 = torch.triu(torch.randn(n, n, dtype=torch.float64, device="cuda")) * \
-                torch.logspace(0, -6, n, dtype=torch.float64, device="cuda")[:, None]
-            G = G0.clone()
-            V = torch.empty(n, n, dtype=torch.float64, device="cuda")
-            sv = torch.empty(n, dtype=torch.float64, device="cuda")
-
-            def j():
-                G.copy_(G0)
-                tt.jacobi_svd(G, V, sv)
-            out["jacobi_svd_%d_ms" % n] = timeit(j)
-    print(json.dumps({"small_micro": out}), flush=True)
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -638,17 +565,11 @@ def main():
     ap.add_argument("--config", default="c3", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--profile-all", action="store_true",
-                    help="time every tensor-GEMM launch (default: only the dominant 128x128-tile kernel)")
     ap.add_argument("--gemm", default=None, help="kernel micro-benchmark: 'all' or one of " + ", ".join(GEMM_SHAPES))
     ap.add_argument("--tma", action="store_true", help="with --gemm: feed the persistent tile from TMA instead of cp.async")
-    ap.add_argument("--small", action="store_true", help="micro-benchmark of the small latency-bound solvers")
     ap.add_argument("--chi", type=int, default=None, help="override the bond dimension of the chosen config (scaling study)")
     ap.add_argument("--r", type=int, default=None, help="override the oversampling parameter r (the paper's figures use r = 7)")
     args = ap.parse_args()
-    if args.small:
-        run_small_micro(args)
-        return
     if args.gemm:
         run_gemm_micro(args)
         return

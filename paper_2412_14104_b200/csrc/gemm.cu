@@ -356,11 +356,9 @@ void tensor_gemm(GemmParams p)
     }
     if ((long long)p.batch * p.ksplit > 65535) fail(-22, "tensor_gemm: batch too large for grid.z");
     prof_shape(p.M, p.N, p.K, p.batch, p.ksplit);
-    static const bool old_big = getenv("TATRG_GEMM_OLD") != nullptr;   // comparison switch (temporary)
-    if (big && !old_big && tensor_gemm_persistent(p, g_num_sms))
-        ;
-    else if (big)
-        tensor_gemm_big(p, 128);
+    if (big) {
+        if (!tensor_gemm_persistent(p, g_num_sms)) tensor_gemm_big(p, 128);
+    }
     else if (mid)
         tensor_gemm_big(p, 64);
     else

@@ -1,5 +1,6 @@
-// gemm_big.cu -- the 128x128 (and 128x64, for outputs at most 64 columns wide) CTA tiles of the
-// tensor-GEMM (see gemm.cu for the operation):
+// gemm_big.cu -- the non-persistent 128x64 (outputs at most 64 columns wide, two CTAs per SM) and 128x128
+// CTA tiles of the tensor-GEMM (see gemm.cu for the operation; the hot 128x128 shapes run on the persistent
+// tile of gemm_p.cu):
 //   C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)]
 // on the FP64 tensor pipe (mma.sync m8n8k4 -> DMMA.8x8x4).  This is the kernel the O(q r chi^7) bond
 // swap (Table 1) and the O(r^2 chi^7) triad contraction (Eqs. 13-14)
@@ -17,8 +18,6 @@
 // (lane -> (row = lane/4, k = lane%4)) conflict free.  Leg permutations stay folded into the gather
 // addresses (Map4); the 16-byte path is taken when every pair of consecutive elements along the
 // contiguous index is 16-byte aligned in global memory (checked on the host), else 8-byte copies.
-#include <stdlib.h>
-
 #include "common.h"
 
 namespace tatrg {
@@ -374,24 +373,13 @@ void dispatch_big(const GemmParams &p)
 
 }  // namespace
 
+// The 128 x 64 tile (two CTAs per SM) for outputs 17..64 columns wide and for short summed indices; the
+// 128 x 128 instantiation is the fallback of the persistent tile (gemm_p.cu) for operands whose free-index
+// offsets do not fit its 32-bit loader state.
 void tensor_gemm_big(const GemmParams &p, int bn)
 {
-    // 128x128: 16 warps x (32 x 32) measured 2.5-3 % faster than 8 warps x (32 x 64) on the c3 shapes
-    // (four warps per scheduler keep the DMMA pipe fed across the per-k-tile barrier);
-    // TATRG_GEMM_WN64 selects the 8-warp variant for comparison
-    static const bool wn64 = getenv("TATRG_GEMM_WN64") != nullptr;
-    static const bool bk16 = getenv("TATRG_GEMM_BK16") != nullptr;   // comparison: BK = 16, 4 stages
-    // decoupled mbarrier pipeline (default; +9 % over the CTA-wide barrier on the c3 shapes);
-    // TATRG_GEMM_SYNC selects the __syncthreads pipeline for comparison
-    static const bool sync = getenv("TATRG_GEMM_SYNC") != nullptr;
     if (bn == 64)
         dispatch_big<64, 32, 16, 3, true>(p);
-    else if (wn64)
-        dispatch_big<128, 64, 16, 4, false>(p);
-    else if (bk16)
-        dispatch_big<128, 32, 16, 4, false>(p);
-    else if (sync)
-        dispatch_big<128, 32, 32, 3, false>(p);
     else
         dispatch_big<128, 32, 32, 3, true>(p);
 }

@@ -183,11 +183,6 @@ void jacobi_svd(double *G, int m, int n, double *V, double *s, int batch, long l
             unsigned long long h = 0;
             TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(h), cudaMemcpyDeviceToHost, stream()));
             TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
-            if (getenv("TATRG_DEBUG")) {
-                double hv;
-                memcpy(&hv, &h, 8);
-                fprintf(stderr, "jacobi m=%d n=%d sweep %d maxcos %.3e (tol %.3e)\n", m, n, sweep, hv, tol);
-            }
             if (h == 0) break;
         }
         if (sweep == max_sweeps) fail(-34, "jacobi_svd: no convergence after %d sweeps (m=%d n=%d)", max_sweeps, m, n);
