@@ -56,6 +56,8 @@ struct Ctx {
     size_t pre_n[9] = {};
 
     Input in[9];
+    int sq_hist[4][3] = {};                 // subspace iterations each squeezer needed, per direction (step.cpp: SqChain)
+    int sm_reserve = 0;                     // SMs the persistent GEMM leaves to concurrent chains (step.cpp)
     int routes = 0;                         // mask of Route: robust routes forced by tatrg_set_routes
     bool keep_iso = false;                  // tatrg_keep_isometries: host copies of U^A, U^X, U^Y, U^D of the last step
     std::vector<double> iso[4];

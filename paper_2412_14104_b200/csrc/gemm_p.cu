@@ -467,7 +467,8 @@ void launch_p(const GemmParams &p_in, int num_sms)
     if (p.lower_only && tm != p.tiles_n) fail(-22, "tensor_gemm: a symmetric (lower_only) output needs M = N");
     const long long tiles = (p.lower_only ? tm * (tm + 1) / 2 : tm * p.tiles_n) * p.batch * (p.ksplit > 1 ? p.ksplit : 1);
     if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
-    const unsigned grid = (unsigned)std::min<long long>(tiles, num_sms);
+    // while independent chains of small kernels run beside the step's big products, some SMs are left to them
+    const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, num_sms - ctx().sm_reserve));
     // 16-byte stores of column pairs: bit 0 for C through its maps, bit 1 for the split-K partial sums
     int c_flags = 0;
     if (((uintptr_t)p.C & 15) == 0 && p.cn.s0 == 1 && even_or_inf(p.cn.n0) && upper_even(p.cn) && all_even(p.cm) && all_even(p.cb))

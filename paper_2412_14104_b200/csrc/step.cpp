@@ -15,6 +15,7 @@
 
 #include <algorithm>
 #include <chrono>
+#include <functional>
 
 #include "ctx.h"
 
@@ -98,11 +99,17 @@ class Fork {
 public:
     // main_slice: the main stream keeps a slice of the workspace too and goes on enqueuing while forked
     // (ordering with the chains through side_after_main / main_after_side)
-    explicit Fork(int n, bool main_slice = false) : c_(ctx()), n_(n), main_(c_.stream), lo0_(c_.lo), hi0_(c_.hi)
+    // chain_bytes > 0 (with main_slice): every chain gets a slice of that size from the top of the free workspace
+    // and the main stream keeps the rest
+    explicit Fork(int n, bool main_slice = false, size_t chain_bytes = 0)
+        : c_(ctx()), n_(n), main_(c_.stream), lo0_(c_.lo), hi0_(c_.hi)
     {
         if (n < 1 || n > Ctx::MAX_CHAINS) fail(-22, "Fork: %d chains", n);
         if (!c_.side_ok) {
-            for (auto &st : c_.side) TATRG_CUDA_CHECK(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+            // the chains are latency-bound sequences of small kernels: their CTAs go first whenever an SM frees up
+            int prio_lo = 0, prio_hi = 0;
+            TATRG_CUDA_CHECK(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+            for (auto &st : c_.side) TATRG_CUDA_CHECK(cudaStreamCreateWithPriority(&st, cudaStreamNonBlocking, prio_hi));
             for (auto &e : c_.join_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
             for (auto &e : c_.dep_ev) TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
             TATRG_CUDA_CHECK(cudaEventCreateWithFlags(&c_.fork_ev, cudaEventDisableTiming));
@@ -110,14 +117,21 @@ public:
         }
         if (!c_.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c_.pinned, Ctx::PINNED_BYTES));
         TATRG_CUDA_CHECK(cudaEventRecord(c_.fork_ev, main_));
-        const size_t slice = ((hi0_ - lo0_) / (n + (main_slice ? 1 : 0))) & ~(size_t)255;
+        size_t slice = ((hi0_ - lo0_) / (n + (main_slice ? 1 : 0))) & ~(size_t)255;
+        size_t main_size = slice;
+        if (main_slice && chain_bytes > 0) {
+            chain_bytes = (chain_bytes + 255) & ~(size_t)255;
+            if (chain_bytes * n + (1 << 20) > hi0_ - lo0_) fail(-12, "Fork: workspace too small for %d chains of %zu bytes", n, chain_bytes);
+            slice = chain_bytes;
+            main_size = (hi0_ - lo0_) - chain_bytes * n;
+        }
         for (int i = 0; i < n; ++i) {
             TATRG_CUDA_CHECK(cudaStreamWaitEvent(c_.side[i], c_.fork_ev, 0));
-            lo_[i] = lo0_ + (i + (main_slice ? 1 : 0)) * slice;
+            lo_[i] = lo0_ + (main_slice ? main_size : 0) + i * slice;
             hi_[i] = lo_[i] + slice;
         }
         main_lo_ = main_slice ? lo0_ : hi0_;   // without a slice nothing is allocated on the main stream while forked
-        main_hi_ = main_slice ? lo0_ + slice : hi0_;
+        main_hi_ = main_slice ? lo0_ + main_size : hi0_;
         c_.lo = main_lo_;
         c_.hi = main_hi_;
     }
@@ -132,6 +146,12 @@ public:
     {
         TATRG_CUDA_CHECK(cudaEventRecord(c_.join_ev[i], c_.side[i]));
         TATRG_CUDA_CHECK(cudaStreamWaitEvent(main_, c_.join_ev[i], 0));
+    }
+    // chain i continues only after everything enqueued on chain j so far
+    void side_after_side(int i, int j)
+    {
+        TATRG_CUDA_CHECK(cudaEventRecord(c_.dep_ev[j], c_.side[j]));
+        TATRG_CUDA_CHECK(cudaStreamWaitEvent(c_.side[i], c_.dep_ev[j], 0));
     }
     void enter(int i)
     {
@@ -392,7 +412,7 @@ struct SqChain {
     double *ratio = nullptr, *Q = nullptr, *Qt = nullptr, *Rb = nullptr, *V = nullptr, *sv = nullptr;
     Back *back = nullptr;
     std::vector<double> sh;
-    int more = 0, k = 0;
+    int more = 0, k = 0, hist = 0, iters_done = 0, planned = 0;
     double gap = INFINITY;
     Ten Mr, Nr;
     static constexpr double it_shift = 1e-13;
@@ -443,6 +463,9 @@ struct SqChain {
         const double shift = 3e-14;
         cholesky_lower_async(which == 0 ? LL.p : LR.p, N2, shift, nullptr, flag);
     }
+    // hist > 0: the iteration count the same squeezer needed four steps ago (same direction): that many
+    // iterations are done at once and the Ritz step that follows is the final one if the decay it measures
+    // confirms the count (plan); else two iterations and a rough Ritz step to measure the decay first
     void phaseA(char *pinned)
     {
         back = reinterpret_cast<Back *>(pinned);
@@ -459,13 +482,15 @@ struct SqChain {
         // pass is enough: only the span is carried on; the blocks that enter a Ritz step get two.
         mulF(om.p, Q);
         cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
-        for (int it = 0; it < 2; ++it) {
+        iters_done = hist > 0 ? hist : 2;
+        for (int it = 0; it < iters_done; ++it) {
+            const bool last = it == iters_done - 1;
             mulFt(Q, Qt);
             cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
             mulF(Qt, Q);
-            cholqr_async(Q, N2, b, it == 1 ? 2 : 1, it == 1 ? 0.0 : it_shift, flag, it == 1 ? ratio : nullptr, nullptr);
+            cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
         }
-        enqueue_ritz(true);
+        enqueue_ritz(hist <= 0);
     }
     // iteration count from the measured decay rho = s_b / s_chi: rho^(2p+1) < 1e-13
     bool plan()
@@ -475,7 +500,11 @@ struct SqChain {
         const double rho = sh[b - 1] / sh[chi - 1];
         const int need = (rho > 0.0 && rho < 1.0) ? (int)ceil((13.0 / -log10(rho) - 1.0) / 2.0) : 2;
         if (need + 1 > 80) return false;                   // decay too slow for this block width: dense route
-        more = std::max(1, need + 1 - 2);                  // two iterations are done
+        planned = need + 1;
+        if (hist > 0 && iters_done >= planned)
+            more = 0;                                      // the Ritz step just read back is the final one
+        else
+            more = std::max(1, planned - iters_done);
         return true;
     }
     void phaseB()
@@ -575,6 +604,7 @@ struct OrthoChain {
     bool redo_shifted()
     {
         d2d(G1.p, G1copy.p, nk * nk);
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));   // the failed attempt raised it
         if (!cholesky_lower(G1.p, (int)nk, 1e-13, L1inv.p)) return false;
         contract(T.as("cpqtb"), L1inv, o.Q1);
         contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
@@ -623,12 +653,18 @@ struct OrthoChain {
         transposed_r = true;
         return std::isfinite(err) && err < 0.05;
     }
-    bool phase2()
+    // the last factorisation, G2 (or G3) = L L^T: asynchronous, so that the two tensors' run side by side
+    void phase2_factor()
     {
         if (err < 1e-8)
             near_identity_chol(G2.p, (int)nk, o.L2inv.p);
-        else if (!cholesky_lower(G2.p, (int)nk, 0.0, o.L2inv.p))
-            return false;
+        else
+            cholesky_lower_async(G2.p, (int)nk, 0.0, o.L2inv.p, flag);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+    }
+    bool phase2()   // after the factorisations have been synchronised
+    {
+        if (back->flag != 0) return false;
         if (transposed_r)   // after an extra pass G1 holds the accumulated factor transposed: R[i][j] = sum_k L3[k][i] G1[k][j]
             contract(G2.as("ki"), Ten::make(G1.p, "kj", {nk, nk}), Ten::make(o.R.p, "ij", {nk, nk}));
         else                // R[i][(c,b)] = sum_k L2[k][i] L1[(c,b)][k]
@@ -668,6 +704,16 @@ bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
     for (int i = 0; i < 2 && ok; ++i) ok = ch[i].usable() || (ch[i].failed_factor() && ch[i].redo_shifted());
     for (int i = 0; i < 2 && ok; ++i)
         if (ch[i].err >= 0.05) ok = ch[i].extra_pass();
+    if (ok) {
+        Fork fk(2);
+        for (int i = 0; i < 2; ++i) {
+            fk.enter(i);
+            ch[i].phase2_factor();
+            fk.leave();
+        }
+        for (int i = 0; i < 2; ++i) fk.sync(i);
+        fk.join();
+    }
     for (int i = 0; i < 2 && ok; ++i) ok = ch[i].phase2();
     bA = ch[0].o;
     bD = ch[1].o;
@@ -726,6 +772,7 @@ void do_init(double beta, double h)
     for (int i = 0; i < 4; ++i) {
         c.iso_pending[i] = false;
         c.iso_H[i].clear();
+        for (int mu = 0; mu < 3; ++mu) c.sq_hist[i][mu] = 0;
     }
     for (auto &i : c.in) i = Input();
     c.inited = true;
@@ -1047,6 +1094,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     trace_mark("swap: expansion, scaling");
     stage_mark(2);
 
+    bool overlapped = false;   // the squeezers run beside the Gram chains and steps (i), (ii) of the contraction
+    size_t gram_mark = 0;
     Ten U[4];   // A, X, Y, D : [p,q,k]
     bool iso_lazy[4] = {false, false, false, false};
     double *Hkeep[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -1055,10 +1104,168 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     long long kd = 0;
     Ten GL[3], GR[3];
     const long long nn[3] = {n1, n2, n3};
+    Ten Ms[3], Ns[3];
+    int kq[3] = {0, 0, 0};
     for (int mu = 0; mu < 3; ++mu) {
         GL[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
         GR[mu] = ws_tensor("psrv", {nn[mu], nn[mu], nn[mu], nn[mu]});
+        const long long N2 = nn[mu] * nn[mu];
+        Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
+        Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
     }
+    bool done[3] = {false, false, false};
+    // gauge (reading G12) P = N G_ref, then M W and W^T N into the step's squeezer buffers
+    auto finish = [&](int mu, const Ten &Mr, const Ten &Nr, const std::vector<double> &sh, int k) {
+        const long long N2 = nn[mu] * nn[mu];
+        kq[mu] = k;
+        spec[6 + mu].assign(sh.begin(), sh.begin() + k);
+        Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
+        Ten Pq = ws_tensor("kb", {k, k});
+        contract(Nr, rf, Pq);
+        Ten Wq = gauge_rotation(Pq.as("ab"), sh, k);
+        Ms[mu] = Ten::make(Ms[mu].p, "uok", {nn[mu], nn[mu], k});
+        Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
+        contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
+        contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
+    };
+    // The subspace-iteration squeezers of the directions `mus` as concurrent chains (large legs only; the
+    // others, and chains that give up, are left to squeeze_dense).  main_work (may be empty) is enqueued on
+    // the main stream once the chains' factorisations are under way and runs beside them: the persistent GEMM
+    // leaves SM_RESERVE SMs to the chains meanwhile.
+    constexpr int SM_RESERVE = 8;   // measured at c3: 4 -> 81.7 ms, 8 -> 79.7, 12 -> 80.3, 20 -> 81.2 per step
+    int sq_hist_new[3] = {0, 0, 0};
+    auto squeeze_wave = [&](const std::vector<int> &mus, const std::function<void()> &main_work,
+                            const std::function<void()> &tail_work = nullptr) {
+        SqChain ch[3];
+        std::vector<int> act;
+        long long n2max = 0;
+        for (int mu : mus) {
+            const long long N2 = nn[mu] * nn[mu];
+            ch[mu].b = chi < 64 ? 64 : 128;
+            ch[mu].active = !(c.routes & ROUTE_DENSE_SQUEEZER) && N2 >= 4 * ch[mu].b && chi < ch[mu].b;
+            ch[mu].GLm = GL[mu];
+            ch[mu].GRm = GR[mu];
+            ch[mu].N2 = (int)N2;
+            ch[mu].chi = chi;
+            ch[mu].mu = mu;
+            ch[mu].hist = c.sq_hist[direction - 1][mu];
+            if (ch[mu].active) {
+                act.push_back(mu);
+                n2max = std::max(n2max, N2);
+            }
+        }
+        if (act.empty()) {
+            if (main_work) main_work();
+            if (tail_work) tail_work();
+            return;
+        }
+        for (int mu : act) ch[mu].prep();
+        const int na = (int)act.size();
+        const size_t chain_bytes = main_work ? std::max<size_t>((size_t)64 << 20, (size_t)(6 * n2max * n2max * 8)) : 0;
+        Fork fk(2 * na, (bool)main_work, chain_bytes);
+        for (int i = 0; i < na; ++i)           // the two Cholesky factorisations of a chain side by side
+            for (int w = 0; w < 2; ++w) {
+                fk.enter(2 * i + w);
+                ch[act[i]].factor(w);
+                fk.leave();
+            }
+        for (int i = 0; i < na; ++i) fk.side_after_side(2 * i, 2 * i + 1);
+        fk.enter(0);
+        trace_mark("sq chain 0: cholesky x2");
+        fk.leave();
+        if (main_work) {
+            c.sm_reserve = SM_RESERVE;
+            main_work();
+            c.sm_reserve = 0;
+        }
+        for (int i = 0; i < na; ++i) {
+            fk.enter(2 * i);
+            ch[act[i]].phaseA(fk.pinned(2 * i));
+            fk.leave();
+        }
+        fk.enter(0);
+        trace_mark("sq chain 0: phase A");
+        fk.leave();
+        for (int i = 0; i < na; ++i) {
+            fk.sync(2 * i);
+            ch[act[i]].ok = ch[act[i]].plan();
+            if (getenv("TATRG_TRACE"))
+                fprintf(stderr, "tatrg-trace squeezer mu %d: hist %d done %d planned %d more %d ok %d\n", act[i], ch[act[i]].hist,
+                        ch[act[i]].iters_done, ch[act[i]].planned, ch[act[i]].more, (int)ch[act[i]].ok);
+        }
+        for (int i = 0; i < na; ++i)
+            if (ch[act[i]].ok && ch[act[i]].more > 0) {
+                fk.enter(2 * i);
+                ch[act[i]].phaseB();
+                fk.leave();
+            }
+        for (int i = 0; i < na; ++i)
+            if (ch[act[i]].ok) {
+                const int mu = act[i];
+                if (ch[mu].more > 0) fk.sync(2 * i);
+                fk.enter(2 * i);
+                if (ch[mu].phaseC()) {
+                    gaps[1 + mu] = ch[mu].gap;
+                    finish(mu, ch[mu].Mr, ch[mu].Nr, ch[mu].sh, ch[mu].k);
+                    done[mu] = true;
+                    sq_hist_new[mu] = std::max(3, ch[mu].planned);
+                }
+                fk.leave();
+            }
+        fk.enter(0);
+        trace_mark("sq chain 0: phase B, C, gauge");
+        fk.leave();
+        if (tail_work) {   // the chains are enqueued to their end: what follows on the main stream gets every SM
+            for (int i = 0; i < na; ++i) fk.sync(2 * i);
+            tail_work();
+        }
+        fk.join();
+    };
+    // dense route = the oracle's algorithm: eigendecompositions of both Grams, SVD of R1 R2
+    auto squeeze_dense = [&](int mu) {
+        const int N2 = (int)(nn[mu] * nn[mu]);
+        size_t mk = ws_mark();
+        Ten Mr, Nr;
+        std::vector<double> sh;
+        double *sf;
+        int k;
+        {
+            Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
+            double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
+            std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
+            std::vector<double> lam2 = sym_eig(GR[mu].p, N2, V2.p, l2);
+            const int kl = num_rank(lam1, -1), kr = num_rank(lam2, -1);
+            if (kl < 1 || kr < 1) fail(-34, "squeezer: Gram matrix is numerically zero");
+            // R1 = Lambda^1/2 V^T (rows of V1 scaled), R2^T likewise
+            scale_leg(V1.p, (long long)kl * N2, N2, kl, l1, 2);
+            scale_leg(V2.p, (long long)kr * N2, N2, kr, l2, 2);
+            Ten R1 = V1, R2 = V2;
+            R1.legs[0].n = kl;
+            R2.legs[0].n = kr;
+            Ten Fm = ws_tensor("ji", {kr, kl});        // buffer = column-major F = R1 R2 (kl x kr)
+            contract(R2, R1, Fm);
+            Ten Vf = ws_tensor("kj", {kr, kr});
+            sf = ws_doubles(kr);
+            jacobi_svd(Fm.p, kl, kr, Vf.p, sf, 1, 0, 0, 0);   // F V = U diag(s): Fm rows -> U_k[i] s_k
+            sh = d2h(sf, kr);
+            sh.resize(std::min(kl, kr));
+            k = num_rank(sh, chi);
+            if (k < 1) fail(-34, "squeezer: R1 R2 is numerically zero");
+            gaps[1 + mu] = rel_gap(sh, k);
+            Ten Vk = Vf, Uk = Fm.as("ki");
+            Vk.legs[0].n = k;
+            Uk.legs[0].n = k;
+            Mr = ws_tensor("nk", {N2, k});
+            Nr = ws_tensor("kn", {k, N2});
+            contract(R2, Vk, Mr);                       // M = R2 V s^-1/2
+            contract(Uk, R1, Nr);                       // N = s^-1/2 U^T R1, U = Fm rows / s
+            scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
+            scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
+        }
+        finish(mu, Mr, Nr, sh, k);
+        ws_release(mk);
+        done[mu] = true;
+    };
     if (mode == 0) {
     // =================== O4 oversampled isometries (Eqs. 2-3) ===================
     const int kk = (int)std::min<long long>((long long)r * chi, n12);
@@ -1215,7 +1422,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
 
     // =================== O6 Gram matrices of Gamma^triad (Eq. 12) ===================
     {
-        size_t mk = ws_mark();
+        gram_mark = ws_mark();
         Ten HH0 = ws_tensor("bc", {a, a}), EE0 = ws_tensor("ab", {a, a});
         contract(H.as("xktb"), H.as("xktc"), HH0);
         contract(E.as("xkta"), E.as("xktb"), EE0);
@@ -1240,31 +1447,55 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(GG3, HH3, GR[2].as("tsuv"));
             ws_release(mk2);
         }
-        Ten EEk = ws_tensor("kalb", {kd, a, kd, a}), FFk = ws_tensor("kalb", {kd, a, kd, a});
-        Ten GGk = ws_tensor("kblc", {kd, a, kd, a}), HHk = ws_tensor("kblc", {kd, a, kd, a});
-        contract(E.as("xkta"), E.as("xltb"), EEk);
-        contract(F.as("aktg"), Fs.as("bltg"), FFk);
-        contract(G.as("bktg"), Gs.as("cltg"), GGk);
-        contract(H.as("xktb"), H.as("xltc"), HHk);
-        for (int mu = 0; mu < 2; ++mu) {
-            size_t mk2 = ws_mark();
-            const char *n1s = mu == 0 ? "pqk" : "qpk", *n2s = mu == 0 ? "rql" : "qrl";
-            const long long np = nn[mu];
-            Ten UU = ws_tensor("pkrl", {np, kd, np, kd});
-            Ten Ta = ws_tensor("prab", {np, np, a, a}), Tb = ws_tensor("qsab", {np, np, a, a});
-            contract(U[0].as(n1s), U[0].as(n2s), UU);
-            contract(UU, EEk, Ta);
-            contract(U[1].as(n1s), U[1].as(n2s), UU);
-            contract(UU, FFk, Tb.as("prab"));
-            contract(Ta, Tb, GL[mu].as("pqrs"));
-            contract(U[2].as(n1s), U[2].as(n2s), UU);
-            contract(UU, GGk.as("kalb"), Ta);
-            contract(U[3].as(n1s), U[3].as(n2s), UU);
-            contract(UU, HHk.as("kalb"), Tb.as("prab"));
-            contract(Ta, Tb, GR[mu].as("pqrs"));
-            ws_release(mk2);
+        // grouped legs
+        auto gram_grouped = [&]() {
+            size_t mk1 = ws_mark();
+            Ten EEk = ws_tensor("kalb", {kd, a, kd, a}), FFk = ws_tensor("kalb", {kd, a, kd, a});
+            Ten GGk = ws_tensor("kblc", {kd, a, kd, a}), HHk = ws_tensor("kblc", {kd, a, kd, a});
+            contract(E.as("xkta"), E.as("xltb"), EEk);
+            contract(F.as("aktg"), Fs.as("bltg"), FFk);
+            contract(G.as("bktg"), Gs.as("cltg"), GGk);
+            contract(H.as("xktb"), H.as("xltc"), HHk);
+            for (int mu = 0; mu < 2; ++mu) {
+                size_t mk2 = ws_mark();
+                const char *n1s = mu == 0 ? "pqk" : "qpk", *n2s = mu == 0 ? "rql" : "qrl";
+                const long long np = nn[mu];
+                Ten UU = ws_tensor("pkrl", {np, kd, np, kd});
+                Ten Ta = ws_tensor("prab", {np, np, a, a}), Tb = ws_tensor("qsab", {np, np, a, a});
+                contract(U[0].as(n1s), U[0].as(n2s), UU);
+                contract(UU, EEk, Ta);
+                contract(U[1].as(n1s), U[1].as(n2s), UU);
+                contract(UU, FFk, Tb.as("prab"));
+                contract(Ta, Tb, GL[mu].as("pqrs"));
+                contract(U[2].as(n1s), U[2].as(n2s), UU);
+                contract(UU, GGk.as("kalb"), Ta);
+                contract(U[3].as(n1s), U[3].as(n2s), UU);
+                contract(UU, HHk.as("kalb"), Tb.as("prab"));
+                contract(Ta, Tb, GR[mu].as("pqrs"));
+                ws_release(mk2);
+            }
+            ws_release(mk1);
+        };
+        // Large legs: the lone-leg squeezer (the only one steps (i), (ii) of Eqs. 13-14 need) runs as a chain
+        // of small kernels BESIDE the grouped-leg Gram chains, and the two grouped-leg squeezers later beside
+        // (i), (ii): their latency (Cholesky, ~17 subspace iterations, two 64 x 64 Jacobi each) disappears
+        // behind machine-filling GEMMs.
+        const int sq_b = chi < 64 ? 64 : 128;
+        overlapped = !(c.routes & (ROUTE_DENSE_SQUEEZER | ROUTE_SEQUENTIAL_ISO)) && chi < sq_b;
+        for (int mu = 0; mu < 3; ++mu) overlapped = overlapped && nn[mu] * nn[mu] >= 4 * sq_b;
+        {   // room for the grouped-leg temporaries in the main stream's slice
+            const double need = 8.0 * (4.0 * kd * a * kd * a + 2.0 * (double)n1 * kd * n1 * kd + 4.0 * (double)n1 * n1 * a * a) * 1.5 +
+                                2.0 * std::max<double>(64 << 20, 6.0 * 8.0 * (double)n3 * n3 * n3 * n3);
+            overlapped = overlapped && (double)(c.hi - c.lo) > need + (64 << 20);
         }
-        ws_release(mk);
+        if (overlapped) {
+            stage_mark(5);
+            squeeze_wave({2}, gram_grouped);
+            if (!done[2]) squeeze_dense(2);
+        } else {
+            gram_grouped();
+        }
+        ws_release(gram_mark);
     }
     } else {
         // =================== plain ATRG (Table 1): squeezer Grams of A X sigma and of
@@ -1298,138 +1529,52 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             ws_release(mk);
         }
     }
-    stage_mark(5);
+    if (!overlapped) stage_mark(5);
 
     // =================== O6 squeezers (Eq. 12; reading G10) ===================
-    Ten Ms[3], Ns[3];
-    int kq[3];
-    for (int mu = 0; mu < 3; ++mu) {
-        const long long N2 = nn[mu] * nn[mu];
-        Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
-        Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
-    }
-    // gauge (reading G12) P = N G_ref, then M W and W^T N into the step's squeezer buffers
-    auto finish = [&](int mu, const Ten &Mr, const Ten &Nr, const std::vector<double> &sh, int k) {
-        const long long N2 = nn[mu] * nn[mu];
-        kq[mu] = k;
-        spec[6 + mu].assign(sh.begin(), sh.begin() + k);
-        Ten rf = get_input(6 + mu, N2, k, cfg, "nb");
-        Ten Pq = ws_tensor("kb", {k, k});
-        contract(Nr, rf, Pq);
-        Ten Wq = gauge_rotation(Pq.as("ab"), sh, k);
-        Ms[mu] = Ten::make(Ms[mu].p, "uok", {nn[mu], nn[mu], k});
-        Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
-        contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
-        contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
-    };
-    bool done[3] = {false, false, false};
-    {   // the three subspace-iteration squeezers as concurrent chains (large legs only)
-        SqChain ch[3];
-        int nact = 0;
-        for (int mu = 0; mu < 3; ++mu) {
-            const long long N2 = nn[mu] * nn[mu];
-            ch[mu].b = chi < 64 ? 64 : 128;
-            ch[mu].active = !(c.routes & ROUTE_DENSE_SQUEEZER) && N2 >= 4 * ch[mu].b && chi < ch[mu].b;
-            ch[mu].GLm = GL[mu];
-            ch[mu].GRm = GR[mu];
-            ch[mu].N2 = (int)N2;
-            ch[mu].chi = chi;
-            ch[mu].mu = mu;
-            nact += ch[mu].active;
-        }
-        if (nact > 0) {
-            for (int mu = 0; mu < 3; ++mu)
-                if (ch[mu].active) ch[mu].prep();
-            {   // six Cholesky factorisations side by side
-                Fork fk6(6);
-                for (int mu = 0; mu < 3; ++mu)
-                    for (int w = 0; w < 2 && ch[mu].active; ++w) {
-                        fk6.enter(2 * mu + w);
-                        ch[mu].factor(w);
-                        fk6.leave();
-                    }
-                fk6.join();
-            }
-            Fork fk(3);
-            for (int mu = 0; mu < 3; ++mu)
-                if (ch[mu].active) {
-                    fk.enter(mu);
-                    ch[mu].phaseA(fk.pinned(mu));
-                    fk.leave();
-                }
-            for (int mu = 0; mu < 3; ++mu)
-                if (ch[mu].active) {
-                    fk.sync(mu);
-                    ch[mu].ok = ch[mu].plan();
-                }
-            for (int mu = 0; mu < 3; ++mu)
-                if (ch[mu].ok) {
-                    fk.enter(mu);
-                    ch[mu].phaseB();
-                    fk.leave();
-                }
-            for (int mu = 0; mu < 3; ++mu)
-                if (ch[mu].ok) {
-                    fk.sync(mu);
-                    fk.enter(mu);
-                    if (ch[mu].phaseC()) {
-                        gaps[1 + mu] = ch[mu].gap;
-                        finish(mu, ch[mu].Mr, ch[mu].Nr, ch[mu].sh, ch[mu].k);
-                        done[mu] = true;
-                    }
-                    fk.leave();
-                }
-            fk.join();
-        }
-    }
-    for (int mu = 0; mu < 3; ++mu) {
-        if (done[mu]) continue;
-        // dense route = the oracle's algorithm: eigendecompositions of both Grams, SVD of R1 R2
-        const int N2 = (int)(nn[mu] * nn[mu]);
-        size_t mk = ws_mark();
-        Ten Mr, Nr;
-        std::vector<double> sh;
-        double *sf;
-        int k;
-        {
-            Ten V1 = ws_tensor("in", {N2, N2}), V2 = ws_tensor("jn", {N2, N2});
-            double *l1 = ws_doubles(N2), *l2 = ws_doubles(N2);
-            std::vector<double> lam1 = sym_eig(GL[mu].p, N2, V1.p, l1);
-            std::vector<double> lam2 = sym_eig(GR[mu].p, N2, V2.p, l2);
-            const int kl = num_rank(lam1, -1), kr = num_rank(lam2, -1);
-            if (kl < 1 || kr < 1) fail(-34, "squeezer: Gram matrix is numerically zero");
-            // R1 = Lambda^1/2 V^T (rows of V1 scaled), R2^T likewise
-            scale_leg(V1.p, (long long)kl * N2, N2, kl, l1, 2);
-            scale_leg(V2.p, (long long)kr * N2, N2, kr, l2, 2);
-            Ten R1 = V1, R2 = V2;
-            R1.legs[0].n = kl;
-            R2.legs[0].n = kr;
-            Ten Fm = ws_tensor("ji", {kr, kl});        // buffer = column-major F = R1 R2 (kl x kr)
-            contract(R2, R1, Fm);
-            Ten Vf = ws_tensor("kj", {kr, kr});
-            sf = ws_doubles(kr);
-            jacobi_svd(Fm.p, kl, kr, Vf.p, sf, 1, 0, 0, 0);   // F V = U diag(s): Fm rows -> U_k[i] s_k
-            sh = d2h(sf, kr);
-            sh.resize(std::min(kl, kr));
-            k = num_rank(sh, chi);
-            if (k < 1) fail(-34, "squeezer: R1 R2 is numerically zero");
-            gaps[1 + mu] = rel_gap(sh, k);
-            Ten Vk = Vf, Uk = Fm.as("ki");
-            Vk.legs[0].n = k;
-            Uk.legs[0].n = k;
-            Mr = ws_tensor("nk", {N2, k});
-            Nr = ws_tensor("kn", {k, N2});
-            contract(R2, Vk, Mr);                       // M = R2 V s^-1/2
-            contract(Uk, R1, Nr);                       // N = s^-1/2 U^T R1, U = Fm rows / s
-            scale_leg(Mr.p, Mr.size(), 1, k, sf, 3);
-            scale_leg(Nr.p, Nr.size(), N2, k, sf, 5);
-        }
-        finish(mu, Mr, Nr, sh, k);
-        ws_release(mk);
+    if (!overlapped) {
+        squeeze_wave({0, 1, 2}, nullptr);
+        for (int mu = 0; mu < 3; ++mu)
+            if (!done[mu]) squeeze_dense(mu);
     }
     stage_mark(6);
 
     // =================== O7 contraction (Eqs. 13-14) ===================
+    // (i) E M^(4) and (ii) . F need the lone-leg squeezer only: when the squeezers are overlapped, both sides'
+    // (i), (ii) run on the main stream while the grouped-leg squeezers finish on their chains
+    Ten Pt_pre[2];
+    bool pre_done = false;
+    if (overlapped) {
+        const long long m3 = kq[2];
+        const double per_x = 8.0 * ((double)kd * a * n3 * m3 + (double)kd * m3 * kd * gs);
+        const long long xc = std::max<long long>(1, std::min<long long>(n0, (long long)(8.0e9 / per_x)));
+        const double chains = 4.0 * std::max<double>(64 << 20, 6.0 * 8.0 * (double)n1 * n1 * n1 * n1);
+        const double need = 8.0 * ((double)n0 * kd * a * n3 * m3 + 2.0 * (double)n0 * kd * m3 * kd * gs) + chains + (256 << 20);
+        if (xc == n0 && (double)(c.hi - c.lo) > need) {
+            Ten EM = ws_tensor("xkaTw", {n0, kd, a, n3, m3});
+            for (int side = 0; side < 2; ++side) Pt_pre[side] = ws_tensor("xkwlg", {n0, kd, m3, kd, gs});
+            auto side0 = [&]() {
+                contract(E.as("xkta"), Ms[2].as("tTw"), EM);
+                contract(EM, F.as("alTg"), Pt_pre[0]);
+            };
+            auto side1 = [&]() {
+                // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
+                contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkatw"));
+                contract(EM.as("xkatw"), G.as("altg"), Pt_pre[1]);   // Pt[x, kD, w, kY, g]
+            };
+            // (handing the second side to the main stream only after the chains have ended, so that it gets every
+            // SM, measured slower: the chains outlast the first side and the main stream idles meanwhile)
+            squeeze_wave({0, 1}, [&]() {
+                side0();
+                side1();
+            });
+            pre_done = true;
+        } else {
+            squeeze_wave({0, 1}, nullptr);
+        }
+        for (int mu = 0; mu < 2; ++mu)
+            if (!done[mu]) squeeze_dense(mu);
+    }
     const long long m1 = kq[0], m2 = kq[1], m3 = kq[2];
     const long long nd[4] = {n0, m1, m2, m3};
     int new_dims[4];
@@ -1457,13 +1602,21 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             contract(U[3].as("PQl"), Ns[1].as("nqQ"), V2);
         }
         contract(W1, V2, Qt);
+        Ten out = new_view(side == 0 ? phi_new : psi_new).as("xmnwg");
+        if (pre_done) {   // (iv)
+            if (side == 0)
+                contract(Pt_pre[0], Qt, out);
+            else
+                contract(Pt_pre[1].as("xlwkg"), Qt, out);
+            ws_release(mk);
+            continue;
+        }
         // (i)-(ii)-(iv) of Eqs. 13-14 in slabs of the direction-0 leg so that E M^(4) (r chi^5) and
         // P (r^2 chi^5) stay below ~8 GB (one slab = the whole tensor up to chi ~ 40)
         const double per_x = 8.0 * ((double)kd * a * n3 * m3 + (double)kd * m3 * kd * gs);
         const long long xc = std::max<long long>(1, std::min<long long>(n0, (long long)(8.0e9 / per_x)));
         Ten EM = ws_tensor("xkaTw", {xc, kd, a, n3, m3});
         Ten Pt = ws_tensor("xkwlg", {xc, kd, m3, kd, gs});
-        Ten out = new_view(side == 0 ? phi_new : psi_new).as("xmnwg");
         auto slab = [](Ten t, long long x0, long long cnt) {   // legs[0] is the direction-0 leg
             t.p += x0 * t.legs[0].stride;
             t.legs[0].n = cnt;
@@ -1552,6 +1705,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     c.state_low = !c.state_low;
     c.state_bytes = 2 * new_cap;
     spec[9] = {lnc};
+    for (int mu = 0; mu < 3; ++mu) c.sq_hist[direction - 1][mu] = sq_hist_new[mu];
     for (int i = 0; i < 10; ++i) c.spec[i] = spec[i];
     for (int i = 0; i < 4; ++i) {
         c.iso_pending[i] = iso_lazy[i];
