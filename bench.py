@@ -484,7 +484,11 @@ def run_ours(args, cfg, name):
                 "launches": g_n, "share_of_step_time": g_ms / ms if ms > 0 else None,
                 "small_tile_kernel": {"tflops": s_fl / (s_ms * 1e-3) / 1e12 if s_ms > 0 else 0.0,
                                       "share_of_step_time": s_ms / ms if ms > 0 else None},
-                "whole_step_gemm_tflops": flops / (ms * 1e-3) / 1e12}
+                "whole_step_gemm_tflops": flops / (ms * 1e-3) / 1e12,
+                "note": ("achieved = flop-weighted over ALL launches of the kernel inside the timed steps, as they run there: "
+                         "steps (i), (ii) of the contraction and the grouped-leg Gram chains run on 140 of the 148 SMs beside the "
+                         "squeezer chains (DESIGN.md section 4), and a third of the launches are one-wave shapes; the same kernel "
+                         "alone on the machine: 34.2-35.1 TFLOP/s on the hot shapes (profiles/r2_gemm_persistent_full.md)")}
 
     line = None
     if rank == 0:
