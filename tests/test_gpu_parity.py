@@ -292,3 +292,33 @@ def test_critical_temperature_bisection(tt):
     needs chi ~ 50 for 0.1 %); it must land in the neighbourhood of the Monte Carlo value T_c = 6.68."""
     Tc = tt.critical_temperature(chi=8, r=2, q=2, seed=5, T_lo=5.0, T_hi=8.5, n_steps=12, iters=8)
     assert 6.4 < Tc < 7.2, Tc
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 15])
+def test_robust_routes_give_the_same_step(tt, mask):
+    """Every stage has a fast route and a robust route that follows the oracle's algorithm step by step
+    (tatrg_set_routes): bit 0 plain chi^4-dimensional bond-swap operator instead of the
+    reduced chi^3 core, bit 1 Householder TSQR instead of Cholesky-QR, bit 2 dense eigendecompositions instead
+    of Cholesky + subspace iteration in the squeezers, bit 3 sequential isometries.  Config 2 (chi = 16), 10
+    steps: from step 5 on every fast route is taken by default (GPU against GPU)."""
+    import paper_2412_14104_b200 as t
+    beta, chi, r, q, seed, n = 1 / 6.65, 16, 2, 2, 20241215, 10
+    runs = []
+    for m_ in (0, mask):
+        tt.set_routes(m_)
+        try:
+            tt.init_ising_tensor(beta, 0.0)
+            rec = []
+            for m in range(n):
+                tt.coarse_grain(m % 4 + 1, chi, r, q, seed)
+                rec.append((tt.log_Z_per_site(), {k: tt.get_spectrum(k) for k in t.SPECTRA if k != "ln_c"}))
+            runs.append(rec)
+        finally:
+            tt.set_routes(0)
+    for m in range(n):
+        (l0, s0), (l1, s1) = runs[0][m], runs[1][m]
+        assert abs(l1 / l0 - 1) <= LNZ_RTOL, (m, l0, l1)
+        for k in s0:
+            assert len(s0[k]) == len(s1[k]), (m, k)
+            if len(s0[k]):
+                assert spectrum_deviation(k, s0[k], s1[k]) <= SPEC_TOL, (m, k, spectrum_deviation(k, s0[k], s1[k]))
