@@ -203,6 +203,163 @@ __global__ void __launch_bounds__(1024) ts_dot_reduce_kernel(const __grid_consta
     }
 }
 
+// ---------------------------------------------------------------------------------------
+// DMMA versions (the default when the 16-byte alignment conditions hold).  At 4 flop per byte (ts_apply) and
+// 8 flop per byte (ts_dot) these passes need 26 - 52 TFLOP/s to run at HBM speed: out of reach of scalar FMAs
+// fed from shared memory (the kernels above reach 0.25 - 0.48 of the copy bandwidth), within reach of the FP64
+// tensor pipe with the small operand / the accumulators in registers and the rows read straight from global
+// memory with 16-byte loads -- no shared-memory staging at all.
+__device__ __forceinline__ void ts_dmma(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1)
+                 : "d"(a), "d"(b));
+}
+
+// Y[r, n] (+)= alpha sum_c X[r, c] W[c, n], K, N <= 32 (even).  A warp takes 8 rows at a time: lane (lr, lk)
+// loads X[row lr][8 g + 2 lk, +1] (the DMMA k order is free: step (g, e) sums k = 8 g + 2 lk + e), W lives in
+// registers as B fragments, the D fragments are rows of Y stored with 16-byte stores.
+constexpr int TSD_NT = 128;   // threads per CTA of the DMMA streaming kernels (several CTAs per SM)
+
+__global__ void __launch_bounds__(TSD_NT, 4) ts_apply_dmma_kernel(const __grid_constant__ GemmParams p)
+{
+    // W as B fragments in fragment order: ws[g][j][lane] = (W[8 g + 2 lk][8 j + lr], W[8 g + 2 lk + 1][8 j + lr]):
+    // one conflict-free 16-byte load per two DMMAs (64 registers of W per thread would leave one CTA per SM)
+    __shared__ double2 ws[4][4][32];
+    const int lane = threadIdx.x & 31, lr = lane >> 2, lk = lane & 3;
+    const int K = p.K, N = p.N;
+    for (int i = threadIdx.x; i < 4 * 4 * 32; i += TSD_NT) {
+        const int l = i & 31, j = (i >> 5) & 3, g = i >> 7;
+        const int k = 8 * g + 2 * (l & 3), n = 8 * j + (l >> 2);
+        double2 v;
+        v.x = (k < K && n < N) ? p.B[map_off(p.bk, k) + map_off(p.bn, n)] : 0.0;
+        v.y = (k + 1 < K && n < N) ? p.B[map_off(p.bk, k + 1) + map_off(p.bn, n)] : 0.0;
+        ws[g][j][l] = v;
+    }
+    __syncthreads();
+    const long long nblk = ((long long)p.M + 7) / 8;
+    const long long nwarp = (long long)gridDim.x * (TSD_NT / 32);
+    constexpr int U = 2;   // blocks of 8 rows in flight per warp: all loads are issued before the first DMMA
+    for (long long blk0 = (long long)blockIdx.x * (TSD_NT / 32) + (threadIdx.x >> 5); blk0 < nblk; blk0 += U * nwarp) {
+        double2 a[U][4];
+        long long row[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            row[u] = (blk0 + u * nwarp) * 8 + lr;
+            const bool valid = row[u] < p.M;
+            const double *xr = p.A + (valid ? map_off(p.am, (unsigned)row[u]) : 0);
+#pragma unroll
+            for (int g = 0; g < 4; ++g)
+                a[u][g] = (valid && 8 * g + 2 * lk < K) ? *reinterpret_cast<const double2 *>(xr + 8 * g + 2 * lk) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            double acc[4][2];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[j][0] = acc[j][1] = 0.0;
+#pragma unroll
+            for (int g = 0; g < 4; ++g) {
+                double2 wv[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) wv[j] = ws[g][j][lane];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) ts_dmma(acc[j][0], acc[j][1], a[u][g].x, wv[j].x);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) ts_dmma(acc[j][0], acc[j][1], a[u][g].y, wv[j].y);
+            }
+            if (row[u] < p.M) {
+                double *yr = p.C + map_off(p.cm, (unsigned)row[u]);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int n = 8 * j + 2 * lk;
+                    if (n < N) {
+                        double2 *c = reinterpret_cast<double2 *>(yr + n);
+                        double2 v = make_double2(p.alpha * acc[j][0], p.alpha * acc[j][1]);
+                        if (p.accumulate) {
+                            const double2 o = *c;
+                            v.x += o.x;
+                            v.y += o.y;
+                        }
+                        *c = v;
+                    }
+                }
+            }
+        }
+    }
+}
+
+// C[i, j] = sum_r A[r, i] B[r, j], M, N <= 32 (even).  A warp takes 4 rows at a time: lane (lr, lk) loads
+// A[row lk][4 lr .. 4 lr + 3] and B likewise; fragment i of the A operand stands for the columns 4 lr + i,
+// fragment j of the B operand for the columns 4 lr + j (free choices), so one pair of 16-byte loads feeds 16
+// DMMAs.  SYM (A and B are the same matrix: the Gram of a Cholesky-QR pass): the fragment pairs i < j are the
+// transposes of the pairs j < i and are left out (10 DMMAs per 4 rows).
+template <bool SYM>
+__global__ void __launch_bounds__(TSD_NT, 4) ts_dot_dmma_kernel(const __grid_constant__ GemmParams p, double *__restrict__ partial)
+{
+    __shared__ double red[32][33];
+    const int t = threadIdx.x, lane = t & 31, lr = lane >> 2, lk = lane & 3;
+    const int M = p.M, N = p.N;
+    double acc[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+    const long long ngrp = ((long long)p.K + 3) / 4;
+    const long long nwarp = (long long)gridDim.x * (TSD_NT / 32);
+    constexpr int U = SYM ? 4 : 2;   // groups of 4 rows in flight per warp
+    for (long long grp0 = (long long)blockIdx.x * (TSD_NT / 32) + (t >> 5); grp0 < ngrp; grp0 += U * nwarp) {
+        double2 a0[U], a1[U], b0[U], b1[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const long long row = (grp0 + u * nwarp) * 4 + lk;
+            a0[u] = a1[u] = b0[u] = b1[u] = make_double2(0.0, 0.0);
+            if (row < p.K) {
+                const double *ar = p.A + map_off(p.ak, (unsigned)row) + 4 * lr;
+                if (4 * lr < M) a0[u] = *reinterpret_cast<const double2 *>(ar);
+                if (4 * lr + 2 < M) a1[u] = *reinterpret_cast<const double2 *>(ar + 2);
+                if (!SYM) {
+                    const double *br = p.B + map_off(p.bk, (unsigned)row) + 4 * lr;
+                    if (4 * lr < N) b0[u] = *reinterpret_cast<const double2 *>(br);
+                    if (4 * lr + 2 < N) b1[u] = *reinterpret_cast<const double2 *>(br + 2);
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double a[4] = {a0[u].x, a0[u].y, a1[u].x, a1[u].y};
+            const double b[4] = {SYM ? a0[u].x : b0[u].x, SYM ? a0[u].y : b0[u].y, SYM ? a1[u].x : b1[u].x, SYM ? a1[u].y : b1[u].y};
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (!SYM || i >= j) ts_dmma(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    // acc[i][j][e] = C[4 lr + i][4 (2 lk + e) + j]; the warps of the CTA are added one after the other
+    for (int i = t; i < 32 * 33; i += TSD_NT) (&red[0][0])[i] = 0.0;
+    __syncthreads();
+    for (int w = 0; w < TSD_NT / 32; ++w) {
+        if ((t >> 5) == w) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        if (SYM && i < j) continue;
+                        const int ca = 4 * lr + i, cb = 4 * (2 * lk + e) + j;
+                        red[ca][cb] += acc[i][j][e];
+                        if (SYM && i > j) red[cb][ca] += acc[i][j][e];
+                    }
+        }
+        __syncthreads();
+    }
+    double *P = partial + (long long)blockIdx.x * M * N;
+    for (int idx = t; idx < M * N; idx += TSD_NT) P[idx] = red[idx / N][idx % N];
+}
+
+bool even4(const Map4 &m) { return !(m.s0 & 1) && !(m.s1 & 1) && !(m.s2 & 1) && !(m.s3 & 1); }
+
 bool single_unit(const Map4 &m) { return m.n0 == TATRG_RADIX_INF && m.s0 == 1; }
 
 int g_sms = 0;
@@ -266,6 +423,14 @@ bool tensor_gemm_ts(const GemmParams &p)
     // rows x K times K x N: A rows contiguous along k, C rows contiguous along n
     // (up to 32 columns: above that the DFMA pipe, not HBM, bounds these kernels and the DMMA tiles win)
     if (p.M >= 16384 && p.K <= 32 && p.N <= 32 && p.K >= 1 && single_unit(p.ak) && single_unit(p.cn)) {
+        if (!(p.K & 1) && !(p.N & 1) && !((uintptr_t)p.A & 15) && !((uintptr_t)p.C & 15) && even4(p.am) && even4(p.cm)) {
+            const long long nblk = ((long long)p.M + 7) / 8;
+            const int grid = (int)std::min<long long>((nblk + 7) / 8, 16LL * sms());
+            ts_apply_dmma_kernel<<<grid, TSD_NT, 0, stream()>>>(p);
+            TATRG_LAUNCH_CHECK();
+            count_launch();
+            return true;
+        }
         if (p.N <= 32)
             launch_apply<16>(p);
         else
@@ -274,6 +439,24 @@ bool tensor_gemm_ts(const GemmParams &p)
     }
     // (M x rows)(rows x N): both operands contiguous along their small index
     if (p.K >= 16384 && p.M <= 32 && p.N <= 32 && single_unit(p.am) && single_unit(p.bn)) {
+        if (!(p.M & 1) && !(p.N & 1) && !((uintptr_t)p.A & 15) && !((uintptr_t)p.B & 15) && even4(p.ak) && even4(p.bk)) {
+            const bool sym = p.A == p.B && p.M == p.N && p.ak.n0 == p.bk.n0 && p.ak.n1 == p.bk.n1 && p.ak.n2 == p.bk.n2 &&
+                             p.ak.s0 == p.bk.s0 && p.ak.s1 == p.bk.s1 && p.ak.s2 == p.bk.s2 && p.ak.s3 == p.bk.s3;
+            const long long ngrp = ((long long)p.K + 3) / 4;
+            const int grid = (int)std::min<long long>((ngrp + 63) / 64, 8LL * sms());
+            size_t mark = ws_mark();
+            double *partial = ws_doubles((long long)grid * p.M * p.N);
+            if (sym)
+                ts_dot_dmma_kernel<true><<<grid, TSD_NT, 0, stream()>>>(p, partial);
+            else
+                ts_dot_dmma_kernel<false><<<grid, TSD_NT, 0, stream()>>>(p, partial);
+            TATRG_LAUNCH_CHECK();
+            ts_dot_reduce_kernel<<<(p.M * p.N + 31) / 32, 1024, 0, stream()>>>(p, partial, grid);
+            TATRG_LAUNCH_CHECK();
+            count_launch(2);
+            ws_release(mark);
+            return true;
+        }
         const int w = p.M > p.N ? p.M : p.N;
         if (w <= 8)
             launch_dot<1>(p);
