@@ -33,10 +33,6 @@ __device__ __forceinline__ void mbar_init(unsigned bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void mbar_arrive(unsigned bar)
-{
-    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}\n" ::"r"(bar) : "memory");
-}
 __device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes)
 {
     asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}\n" ::"r"(bar), "r"(bytes) : "memory");
@@ -79,12 +75,12 @@ __global__ void __launch_bounds__(NT, 1)
                      const __grid_constant__ GemmParams p, const int total_tiles, const int c_vec)
 {
     extern __shared__ __align__(1024) unsigned char smem_raw[];
-    __shared__ unsigned long long bars[2 * STAGES];
+    __shared__ unsigned long long bars[STAGES];
     __shared__ int done[STAGES];
     // SWIZZLE_128B wants 1024-byte aligned boxes
     const unsigned base = ((unsigned)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
     const unsigned As = base, Bs = base + STAGES * A_STAGE_BYTES;
-    const unsigned full0 = (unsigned)__cvta_generic_to_shared(bars), empty0 = full0 + 8 * STAGES;
+    const unsigned full0 = (unsigned)__cvta_generic_to_shared(bars);
 
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     const int tiles_m = (p.M + BM - 1) / BM;
@@ -92,7 +88,6 @@ __global__ void __launch_bounds__(NT, 1)
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(full0 + 8 * s, 1);
-            mbar_init(empty0 + 8 * s, NT);
             done[s] = 0;
         }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");

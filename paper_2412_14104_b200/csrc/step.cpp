@@ -29,6 +29,9 @@ namespace tatrg {
 namespace {
 
 constexpr double RANK_TOL = 1e-14;     // reading G9
+// SMs the persistent GEMM leaves free while chains of small kernels run beside it (measured at c3: 4 -> 81.7 ms
+// per step, 8 -> 79.7, 12 -> 80.3, 20 -> 81.2)
+constexpr int CHAIN_SM_RESERVE = 8;
 constexpr double CLUSTER_TOL = 1e-8;   // reading G12
 
 std::vector<double> d2h(const double *p, long long n)
@@ -676,7 +679,10 @@ struct OrthoChain {
 // Both bases of the reduced bond swap; false when either matricisation is rank deficient or too
 // ill conditioned for two Cholesky-QR passes (|G2 - I| > 0.05).
 // Main stream: G1_A, G1_D, Q1_A, G2_A, Q1_D, G2_D; side streams: chol(G1_A) under G1_D, chol(G1_D) under Q1_A.
-bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
+// during_last (optional): main-stream work that needs only the first factor Q1 of D's basis (the projection of the
+// sketch) is enqueued beside the last, latency-bound factorisations of the two bases.
+bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD,
+                       const std::function<void(const RedBasis &)> &during_last = nullptr)
 {
     Ctx &c = ctx();
     if (!c.pinned) TATRG_CUDA_CHECK(cudaMallocHost((void **)&c.pinned, Ctx::PINNED_BYTES));
@@ -704,17 +710,27 @@ bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD)
     for (int i = 0; i < 2 && ok; ++i) ok = ch[i].usable() || (ch[i].failed_factor() && ch[i].redo_shifted());
     for (int i = 0; i < 2 && ok; ++i)
         if (ch[i].err >= 0.05) ok = ch[i].extra_pass();
+    bool during_done = false;
     if (ok) {
-        Fork fk(2);
+        const size_t chain_bytes = std::max<size_t>((size_t)32 << 20, (size_t)(4 * ch[0].nk * ch[0].nk * 8));
+        const bool beside = during_last && c.hi - c.lo > 2 * chain_bytes + ((size_t)64 << 20);
+        Fork fk(2, beside, beside ? chain_bytes : 0);
         for (int i = 0; i < 2; ++i) {
             fk.enter(i);
             ch[i].phase2_factor();
             fk.leave();
         }
+        if (beside) {
+            c.sm_reserve = CHAIN_SM_RESERVE;
+            during_last(ch[1].o);
+            c.sm_reserve = 0;
+            during_done = true;
+        }
         for (int i = 0; i < 2; ++i) fk.sync(i);
         fk.join();
     }
     for (int i = 0; i < 2 && ok; ++i) ok = ch[i].phase2();
+    if (ok && during_last && !during_done) during_last(ch[1].o);
     bA = ch[0].o;
     bD = ch[1].o;
     return ok;
@@ -1004,21 +1020,20 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     if (!(c.routes & ROUTE_PLAIN_SWAP) && nT >= 2 * nk && nk >= 16) {
         size_t mk = ws_mark();
         RedBasis bA, bD;
-        if (ortho_factor_pair(A, D, bA, bD)) {
-            trace_mark("swap: bases of A, D");
+        // Omega_red[b,l,z] = sum_l' L2inv_D[l,l'] sum_uvw Q1_D[uvw,l'] Omega[b,uvw,z]: the first product (the
+        // chi^4 x r chi sketch against Q1_D, a machine-filling GEMM) needs Q1_D only and runs beside the last
+        // factorisations of the two bases
+        Ten om_red = ws_tensor("blz", {a, nk, ell});
+        Ten t1 = ws_tensor("bmz", {a, nk, ell});
+        auto project = [&](const RedBasis &bd) {
+            Ten omega = get_input(0, dim, ell, cfg, "rz");
+            contract(bd.Q1.as("uvwm"), Ten::make(omega.p, "buvwz", {a, n1, n2, n3, ell}), t1);
+        };
+        if (ortho_factor_pair(A, D, bA, bD, project)) {
+            trace_mark("swap: bases of A, D, sketch projection");
             const long long rdim = a * nk;
             const int ellr = (int)std::min<long long>(ell, rdim);
-            // Omega_red[b,l,z] = sum_l' L2inv_D[l,l'] sum_uvw Q1_D[uvw,l'] Omega[b,uvw,z]
-            Ten om_red = ws_tensor("blz", {a, nk, ell});
-            {
-                size_t mk2 = ws_mark();
-                Ten omega = get_input(0, dim, ell, cfg, "rz");
-                Ten t1 = ws_tensor("bmz", {a, nk, ell});
-                contract(bD.Q1.as("uvwm"), Ten::make(omega.p, "buvwz", {a, n1, n2, n3, ell}), t1);
-                contract(bD.L2inv.as("lm"), t1, om_red);
-                ws_release(mk2);
-            }
-            trace_mark("swap: sketch projection");
+            contract(bD.L2inv.as("lm"), t1, om_red);
             Ten Z = ws_tensor("cabz", {n0, a, a, ell});
             auto apply = [&](const double *w, double *out) {     // m w : [(b,l), z] -> [(a,k), z]
                 contract(bD.R.as("lca"), Ten::make(const_cast<double *>(w), "blz", {a, nk, ell}), Z);
@@ -1132,10 +1147,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     // others, and chains that give up, are left to squeeze_dense).  main_work (may be empty) is enqueued on
     // the main stream once the chains' factorisations are under way and runs beside them: the persistent GEMM
     // leaves SM_RESERVE SMs to the chains meanwhile.
-    constexpr int SM_RESERVE = 8;   // measured at c3: 4 -> 81.7 ms, 8 -> 79.7, 12 -> 80.3, 20 -> 81.2 per step
+    constexpr int SM_RESERVE = CHAIN_SM_RESERVE;
     int sq_hist_new[3] = {0, 0, 0};
     auto squeeze_wave = [&](const std::vector<int> &mus, const std::function<void()> &main_work,
-                            const std::function<void()> &tail_work = nullptr) {
+                            const std::function<void()> &tail_work = nullptr, int reserve = -1) {
         SqChain ch[3];
         std::vector<int> act;
         long long n2max = 0;
@@ -1174,7 +1189,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         trace_mark("sq chain 0: cholesky x2");
         fk.leave();
         if (main_work) {
-            c.sm_reserve = SM_RESERVE;
+            c.sm_reserve = reserve >= 0 ? reserve : SM_RESERVE;
             main_work();
             c.sm_reserve = 0;
         }
