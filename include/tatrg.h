@@ -55,10 +55,12 @@ int init_ising_tensor(double beta, double h);
  * A sigma D, RSVD bond swap to Gamma = A X sigma Y D (Eq. 1), oversampled
  * isometries U^A..U^D by RSVD (Eqs. 2-3), triad tensors E..L (Eqs. 4-11), squeezers
  * M^(mu), N^(mu) (Eq. 12), contraction to Phi, Psi (Eqs. 13-14), normalisation.
- *   chi >= 1 bond dimension, r >= 1 oversampling (internal lines r*chi), q >= 0 RSVD
- *   iterations, seed: master seed of the Gaussian sketches (sub-seeds per SURVEY.md 8(d);
- *   sketches are generated on the host by the shared seeded generator and uploaded inside
- *   this call unless tatrg_set_sketch supplied them). */
+ *   chi in 1..64 bond dimension, r >= 1 oversampling (internal lines r*chi <= 256: the paper's r = 7 up to
+ *   chi = 36), q >= 0 RSVD iterations, seed: master seed of the Gaussian sketches (sub-seeds per
+ *   SURVEY.md 8(d)).  Every Gaussian input the caller did not supply with tatrg_set_sketch is generated
+ *   on the device by the library's implementation of the shared seeded recipe (tatrg_fill_gauss).
+ *   TATRG_EINVAL: bad arguments, or a supplied input whose size is not the one this step needs;
+ *   TATRG_ENOMEM: workspace too small; TATRG_ENUM: the tensor or a Gram matrix is numerically zero. */
 int coarse_grain(int direction, int chi, int r, int q, uint64_t seed);
 
 /* Same step without the triad decomposition: plain ATRG with bond swapping, O(chi^9)
@@ -82,7 +84,10 @@ size_t tatrg_workspace_bytes_atrg(int chi, int r);           /* the same for coa
  *        5 gauge reference for A/D [(i0..i3), a]; 6..8 gauge references of the squeezers.
  * data: n doubles, row-major in the rotated frame;
  * on_device != 0: device pointer, must stay valid until coarse_grain returns;
- * on_device == 0: host pointer, copied (H2D) inside the next coarse_grain. */
+ * on_device == 0: host pointer (pinned or pageable), copied (H2D) by the library's copy stream inside the next
+ * coarse_grain, which does not return before the copy has ended.  n must equal rows * cols of
+ * tatrg_sketch_shape for the step that consumes it: a mismatch makes that coarse_grain fail with TATRG_EINVAL
+ * (nothing is generated in its place). */
 int tatrg_set_sketch(int which, const double *data, size_t n, int on_device);
 /* Shape the next coarse_grain(direction, chi, r) will ask for input `which`
  * (rows, cols; 0,0 if unused).  For which = 0,5 the bond after canonicalisation is assumed
@@ -170,7 +175,7 @@ int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N,
  * generator's values up to the last-bit differences of log / sincos. */
 int tatrg_fill_gauss(double *out, uint64_t n, uint64_t seed, uint64_t step, uint64_t which);
 
-/* Thin QR with R_ii >= 0 of the row-major m x n matrix Y (device; m >= n, n <= 64): Q overwrites
+/* Thin QR with R_ii >= 0 of the row-major m x n matrix Y (device; m >= n, n <= 256): Q overwrites
  * Y, R (n x n row-major upper triangular) goes to R (device).  The "QR decomposition in the RSVD"
  * of PAPER.md:106 / the canonical form of PAPER.md:37 (Householder TSQR, robust to rank deficiency). */
 int tatrg_qr_pos(double *Y, int64_t m, int n, double *R);
@@ -182,7 +187,7 @@ int tatrg_qr_pos(double *Y, int64_t m, int n, double *R);
  * 1 if a pivot was not positive (A then holds garbage), < 0 on error. */
 int tatrg_cholesky(double *A, int n, double shift_rel, double *Linv);
 
-/* Cholesky-QR of the tall row-major m x n block Y (device, n <= 64): `passes` (1..3) rounds of
+/* Cholesky-QR of the tall row-major m x n block Y (device, n <= 256): `passes` (1..3) rounds of
  * {C = Y^T Y (+ shift_rel * max diag in the first round), C = L L^T, Y <- Y L^-T}; Q overwrites Y and
  * R (device, n x n row-major, may be NULL) receives the accumulated upper-triangular factor.  The
  * orthonormalisation inside the subspace iterations ("iterations of the QR decomposition").

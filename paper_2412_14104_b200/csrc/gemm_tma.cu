@@ -1,10 +1,11 @@
 // gemm_tma.cu -- TMA-fed variant of the persistent 128x128 tensor-GEMM tile (gemm_p.cu) for operands that a
 // rank-2 FP64 tensor map describes: A row-major [M][K] (k contiguous), B row-major [K][N] (n contiguous),
-// C through its maps.  Same tile, same warp layout (16 warps x (32 x 32)), same BK = 32 x 3 stages, same
-// mbarrier ring; the difference is the producer: one thread issues cp.async.bulk.tensor copies (10 boxes
+// C through its maps.  Same tile, same warp layout (16 warps x (32 x 32)), same BK = 32 x 3 stages; the
+// difference is the producer: one thread issues cp.async.bulk.tensor copies (10 boxes
 // per stage: A as two 128 x 16 boxes, B as eight 32 x 16 boxes, inner extent 128 bytes = the span of
-// CU_TENSOR_MAP_SWIZZLE_128B) and arms the stage's "full" barrier with the byte count, instead of every
-// thread issuing four 16-byte cp.async per operand with its own address arithmetic.
+// CU_TENSOR_MAP_SWIZZLE_128B) and arms the stage's "full" mbarrier with the byte count, instead of every
+// thread issuing four 16-byte cp.async per operand with its own address arithmetic; a stage is refilled by
+// the last warp that leaves it (a shared counter per stage instead of an "empty" mbarrier).
 //
 // Shared-memory layout = what the TMA unit writes under SWIZZLE_128B: inside a box, row i (128 bytes)
 // holds its eight 16-byte chunks at chunk ^ (i & 7).  The fragment loads stay LDS.128 and conflict free by

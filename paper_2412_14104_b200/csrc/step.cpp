@@ -1505,7 +1505,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         }
         if (overlapped) {
             stage_mark(5);
-            squeeze_wave({2}, gram_grouped);
+            squeeze_wave({2}, gram_grouped);   // (4 - 20 reserved SMs make no difference here: this chain is latency-bound)
             if (!done[2]) squeeze_dense(2);
         } else {
             gram_grouped();

@@ -51,3 +51,18 @@ def test_reference_arm_runs_on_rank0_only():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                           "--steps", "1", "--warmup", "1"], env=env, capture_output=True, text=True, timeout=120)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_timed_steps_stay_inside_the_schedule():
+    """bench.py times steps of the config's own 40-step schedule only (BASELINE.json c3: 'steps 9...40'): the
+    driver's K = 20, W = 5 is one segment, steps 14..33; a K that does not fit is split into segments that each
+    start from a fresh init + ramp-up + warm-up."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.timed_segments(8, 5, 20) == [list(range(13, 33))]
+    segs = bench.timed_segments(8, 5, 40)
+    assert [len(s) for s in segs] == [27, 13] and all(s[0] == 13 and s[-1] < 40 for s in segs)
+    assert bench.timed_segments(4, 1, 3, sched=8) == [[5, 6, 7]]
+    import pytest
+    with pytest.raises(ValueError):
+        bench.timed_segments(8, 32, 1)
