@@ -107,7 +107,9 @@ int tatrg_get_spectrum(int which, double *host_out, int cap);
  * Eq. 12) instead of Cholesky + subspace iteration, bit 3 the four isometries one after the other with
  * synchronous solvers (Eqs. 2-3).  For tests: both routes must give the same step.  Bit 4 feeds the persistent
  * tensor-GEMM tile from TMA (cp.async.bulk.tensor, rank-2 FP64 tensor maps) instead of per-thread cp.async where
- * the operands are plain row-major matrices (an alternative producer, not a fallback).  0 = default. */
+ * the operands are plain row-major matrices (an alternative producer, not a fallback).  Bit 5 runs the subspace
+ * iteration of the squeezers as separate launches (products, Cholesky-QR passes) instead of the one resident grid
+ * of sq_iter.cu.  0 = default; mask in 0..63, else TATRG_EINVAL. */
 int tatrg_set_routes(int mask);
 
 /* Oversampled isometries of the LAST coarse_grain step (Eqs. 2-3; I, J, K, L of Eqs. 8-11),
@@ -193,6 +195,19 @@ int tatrg_cholesky(double *A, int n, double shift_rel, double *Linv);
  * orthonormalisation inside the subspace iterations ("iterations of the QR decomposition").
  * Returns 0, 1 if a factorisation broke down, < 0 on error. */
 int tatrg_cholqr(double *Y, int64_t m, int n, int passes, double shift_rel, double *R);
+
+/* The subspace iteration of one squeezer as one launch (Eq. 12): for the
+ * row-major n x n matrix F (device, n >= 64) and the n x 64 start block `start` (device, row-major),
+ *   Q <- orth(F start);  `iters` (>= 1) times { Qt <- orth(F^T Q); Q <- orth(F Qt) };  Qt R <- F^T Q,
+ * orth = one Cholesky-QR pass with a relative diagonal shift of 1e-13 (only the span is carried on), two unshifted
+ * passes for the last Q and for the closing factorisation F^T Q = Qt R.  Q, Qt: device, n x 64 row-major, written;
+ * R: device, 64 x 64 row-major upper triangular (may be NULL); minmax (device, 4 doubles, may be NULL): smallest and
+ * largest diagonal entry of the first Cholesky factor of the last Q and of the closing factorisation.  The singular
+ * values of R converge to the leading singular values of F.  `grid` = number of resident CTAs wanted (adjusted so
+ * that every CTA owns between 1 and 16 blocks of 8 rows).  Uses the scratch workspace; synchronises the stream.
+ * Returns 0, 1 if a Cholesky factorisation met a non-positive pivot, < 0 on error (TATRG_EINVAL: arguments). */
+int tatrg_subspace_iteration(const double *F, int n, const double *start, double *Q, double *Qt, int iters, int grid,
+                             double *R, double *minmax);
 
 /* One-sided Jacobi SVD of the column-major m x n matrix G (device, ld = m): on exit G = U diag(s)
  * with orthogonal columns sorted by decreasing norm, V (n x n column-major, device) such that

@@ -24,7 +24,7 @@ EXPORTS = [
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name", "tatrg_get_h2d",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
-    "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
+    "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_subspace_iteration", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
     "tatrg_last_error", "tatrg_destroy",
 ]
 
@@ -82,6 +82,7 @@ def lib():
             "tatrg_qr_pos": (c_i, [c_vp, c_i64, c_i, c_vp]),
             "tatrg_cholesky": (c_i, [c_vp, c_i, c_d, c_vp]),
             "tatrg_cholqr": (c_i, [c_vp, c_i64, c_i, c_i, c_d, c_vp]),
+            "tatrg_subspace_iteration": (c_i, [c_vp, c_i, c_vp, c_vp, c_vp, c_i, c_i, c_vp, c_vp]),
             "tatrg_jacobi_svd": (c_i, [c_vp, c_i, c_i, c_vp, c_vp]),
             "tatrg_sumsq": (c_i, [c_vp, c_i64, c_vp]),
             "tatrg_dot": (c_i, [c_vp, c_vp, c_i64, c_vp]),
@@ -195,6 +196,7 @@ def get_spectrum(which) -> np.ndarray:
 
 
 ROUTE_PLAIN_SWAP, ROUTE_HOUSEHOLDER_QR, ROUTE_DENSE_SQUEEZER, ROUTE_SEQUENTIAL_ISO, ROUTE_TMA_PRODUCER = 1, 2, 4, 8, 16
+ROUTE_UNFUSED_SQUEEZER = 32
 
 
 def set_routes(mask=0):
@@ -364,6 +366,18 @@ def cholqr(Y, R=None, passes=2, shift_rel=0.0) -> bool:
     m, n = Y.shape
     rc = lib().tatrg_cholqr(Y.data_ptr(), int(m), int(n), int(passes), float(shift_rel),
                             R.data_ptr() if R is not None else None)
+    if rc < 0:
+        _check(rc)
+    return rc == 0
+
+
+def subspace_iteration(F, start, Q, Qt, iters, grid=16, R=None, minmax=None) -> bool:
+    """Fused subspace iteration of a squeezer on the n x n matrix F with the n x 64 start block (sq_iter.cu)."""
+    _require_cuda()
+    n = F.shape[0]
+    rc = lib().tatrg_subspace_iteration(F.data_ptr(), int(n), start.data_ptr(), Q.data_ptr(), Qt.data_ptr(), int(iters),
+                                        int(grid), R.data_ptr() if R is not None else None,
+                                        minmax.data_ptr() if minmax is not None else None)
     if rc < 0:
         _check(rc)
     return rc == 0

@@ -10,6 +10,7 @@
 #include <stdlib.h>
 
 #include "ctx.h"
+#include "sq_iter.h"
 
 namespace tatrg {
 
@@ -332,7 +333,7 @@ int tatrg_get_spectrum(int which, double *host_out, int cap)
 
 int tatrg_set_routes(int mask)
 {
-    if (mask < 0 || mask > 31) return set_error(TATRG_EINVAL, "tatrg_set_routes: mask must be in 0..31");
+    if (mask < 0 || mask > 63) return set_error(TATRG_EINVAL, "tatrg_set_routes: mask must be in 0..63");
     ctx().routes = mask;
     return TATRG_OK;
 }
@@ -536,6 +537,45 @@ int tatrg_cholqr(double *Y, int64_t m, int n, int passes, double shift_rel, doub
         int *flag = (int *)ws_alloc(sizeof(int));
         TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
         cholqr_async(Y, m, n, passes, shift_rel, flag, nullptr, R);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+    });
+    return rc < 0 ? rc : (h ? 1 : 0);
+}
+
+int tatrg_subspace_iteration(const double *F, int n, const double *start, double *Q, double *Qt, int iters, int grid,
+                             double *R, double *minmax)
+{
+    int h = 0;
+    int rc = guarded([&] {
+        if (!F || !start || !Q || !Qt || n < 64 || iters < 1 || 2 * iters + 2 > SQ_MAXSTEPS || grid < 1)
+            fail(TATRG_EINVAL, "tatrg_subspace_iteration: need F, start, Q, Qt, n >= 64, 1 <= iters <= %d, grid >= 1", SQ_MAXSTEPS / 2 - 1);
+        scratch_begin();
+        int *flag = (int *)ws_alloc(sizeof(int));
+        TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
+        SqIterParams p{};
+        double *Ft = ws_doubles((long long)n * n);
+        transpose_small(F, Ft, n, n);
+        p.F = F;
+        p.Ft = Ft;
+        p.start = start;
+        p.buf[0] = Q;
+        p.buf[1] = Qt;
+        p.Rout = R;
+        p.ratio = ws_doubles(4);
+        p.flag = flag;
+        p.shift = 1e-13;
+        p.N2 = n;
+        int ns = 0;
+        p.steps[ns++] = SQ_FROM_START;
+        for (int it = 0; it < iters; ++it) {
+            p.steps[ns++] = SQ_TRANS;
+            p.steps[ns++] = it == iters - 1 ? (SQ_TWO_PASSES | (1 << SQ_RATIO_SHIFT)) : 0;
+        }
+        p.steps[ns++] = SQ_TRANS | SQ_TWO_PASSES | (2 << SQ_RATIO_SHIFT) | SQ_WANT_R;
+        p.nsteps = ns;
+        sq_iter_launch(p, grid, ws_doubles((long long)sq_iter_scratch_doubles(sq_iter_grid(n, grid))));
+        if (minmax) TATRG_CUDA_CHECK(cudaMemcpyAsync(minmax, p.ratio, 4 * sizeof(double), cudaMemcpyDeviceToDevice, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
     });

@@ -5,128 +5,53 @@
 // trailing update are tensor-GEMM launches (gemm.cu), so all O(n^3) work runs on the FP64 tensor
 // pipe.
 #include "ctx.h"
+#include "chol64.cuh"
 
 namespace tatrg {
 
 namespace {
 
-constexpr int NB = 64;       // diagonal block
-constexpr int CH_NT = 256;
+constexpr int NB = CH64;      // diagonal block
+constexpr int CH_NT = CH64_NT;
 
 // One CTA: A (nb x nb, row-major, leading dimension lda, lower triangle used) -> L in place
-// (lower; strict upper part of the block zeroed), Linv (nb x nb row-major, ld NB, lower) = L^-1.
-// A pivot <= 0 (or NaN) raises *flag.
-//
-// Right-looking, register tiled: thread (ty, tx) of the 16 x 16 grid owns the cyclic 4 x 4 sub-blocks
-// S[ty+16a][tx+16b] of the (symmetrised) block and of W = L^-1 (forward substitution L W = I fused
-// into the same loop).  Per step j the pivot column of S and the pivot row of W go through a
-// double-buffered shared-memory line: one barrier per step.  A block smaller than 64 is padded
-// with the identity.
+// (lower; strict upper part of the block zeroed), Linv (nb x nb row-major, ld ldinv, lower) = L^-1.
+// A pivot <= 0 (or NaN) raises *flag.  The factorisation itself: chol64.cuh.
 __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ A, long long lda, int nb,
                                                           double *__restrict__ Linv, int *__restrict__ flag,
                                                           double *__restrict__ dminmax, double shift_rel,
                                                           long long ldinv)
 {
-    __shared__ double col[2][NB];
-    __shared__ double wrow[2][NB];
-    __shared__ double diag[NB];
-    __shared__ int bad;
+    __shared__ Chol64Smem sm;
     const int t = threadIdx.x, ty = t >> 4, tx = t & 15;
-    if (t == 0) bad = 0;
     double s[4][4], w[4][4];
 #pragma unroll
     for (int a = 0; a < 4; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
-            const int i = ty + 16 * a, c = tx + 16 * b;
+            const int i = 4 * ty + a, c = 4 * tx + b;
             const int r = i > c ? i : c, cc = i > c ? c : i;   // lower-triangle source
             s[a][b] = (r < nb) ? A[r * lda + cc] : (i == c ? 1.0 : 0.0);
-            w[a][b] = (i == c) ? 1.0 : 0.0;
-            if (i == c) diag[i] = (i < nb) ? s[a][b] : 0.0;
+            if (i == c) sm.diag[i] = (i < nb) ? s[a][b] : 0.0;
         }
     __syncthreads();
-    if (shift_rel > 0.0) {   // A + shift_rel * max_i A_ii on the diagonal
-        double mx = 0.0;
-        for (int i = 0; i < NB; ++i) mx = fmax(mx, diag[i]);
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = 0; b < 4; ++b)
-                if (ty + 16 * a == tx + 16 * b && ty + 16 * a < nb) s[a][b] += shift_rel * mx;
-        __syncthreads();
-    }
-#pragma unroll 1
-    for (int j = 0; j < NB; ++j) {
-        const int buf = j & 1, bj = j >> 4;
-        if (tx == (j & 15)) {
-#pragma unroll
-            for (int a = 0; a < 4; ++a) {
-                double v = s[a][0];
-                if (bj == 1) v = s[a][1];
-                if (bj == 2) v = s[a][2];
-                if (bj == 3) v = s[a][3];
-                col[buf][ty + 16 * a] = v;
-            }
-        }
-        if (ty == (j & 15)) {
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                double v = w[0][b];
-                if (bj == 1) v = w[1][b];
-                if (bj == 2) v = w[2][b];
-                if (bj == 3) v = w[3][b];
-                wrow[buf][tx + 16 * b] = v;
-            }
-        }
-        __syncthreads();
-        double piv = col[buf][j];
-        if (!(piv > 0.0)) {
-            if (t == 0) bad = 1;
-            piv = 1.0;
-        }
-        const double rd = rsqrt(piv), d = piv * rd;   // one special-function chain instead of sqrt + divide
-        if (t == 0) diag[j] = d;
-        double li[4], lc[4], wj[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const int i = ty + 16 * a;
-            li[a] = (i > j) ? col[buf][i] * rd : 0.0;
-        }
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            const int c = tx + 16 * b;
-            lc[b] = (c > j) ? col[buf][c] * rd : 0.0;
-            wj[b] = wrow[buf][c] * rd;
-        }
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const int i = ty + 16 * a;
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                const int c = tx + 16 * b;
-                s[a][b] = fma(-li[a], lc[b], s[a][b]);
-                if (c == j) s[a][b] = (i > j) ? li[a] : (i == j ? d : 0.0);   // finished column of L
-                w[a][b] = (i == j) ? wj[b] : fma(-li[a], wj[b], w[a][b]);
-            }
-        }
-    }
+    chol64_factor(s, w, sm.wk, sm.diag, &sm.bad, nb, shift_rel);
 #pragma unroll
     for (int a = 0; a < 4; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
-            const int i = ty + 16 * a, c = tx + 16 * b;
+            const int i = 4 * ty + a, c = 4 * tx + b;
             if (i < nb && c < nb) {
                 A[i * lda + c] = (c <= i) ? s[a][b] : 0.0;
                 Linv[i * ldinv + c] = (c <= i) ? w[a][b] : 0.0;
             }
         }
-    __syncthreads();
-    if (t == 0 && bad) *flag = 1;
+    if (t == 0 && sm.bad) *flag = 1;
     if (t == 0 && dminmax) {
-        double lo = diag[0], hi = diag[0];
+        double lo = sm.diag[0], hi = sm.diag[0];
         for (int j = 1; j < nb; ++j) {
-            lo = fmin(lo, diag[j]);
-            hi = fmax(hi, diag[j]);
+            lo = fmin(lo, sm.diag[j]);
+            hi = fmax(hi, sm.diag[j]);
         }
         dminmax[0] = lo;
         dminmax[1] = hi;

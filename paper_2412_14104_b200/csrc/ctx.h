@@ -9,7 +9,8 @@ namespace tatrg {
 enum Stage { ST_CANON = 0, ST_SWAP, ST_ISO, ST_TRIAD, ST_GRAM, ST_SQUEEZE, ST_CONTRACT, ST_NORM, ST_COUNT };
 
 // tatrg_set_routes: forces the robust routes of the step (for tests: fast and robust routes must agree)
-enum Route { ROUTE_PLAIN_SWAP = 1, ROUTE_HOUSEHOLDER_QR = 2, ROUTE_DENSE_SQUEEZER = 4, ROUTE_SEQUENTIAL_ISO = 8, ROUTE_TMA_PRODUCER = 16 };
+enum Route { ROUTE_PLAIN_SWAP = 1, ROUTE_HOUSEHOLDER_QR = 2, ROUTE_DENSE_SQUEEZER = 4, ROUTE_SEQUENTIAL_ISO = 8, ROUTE_TMA_PRODUCER = 16,
+             ROUTE_UNFUSED_SQUEEZER = 32 };
 
 struct Input {
     const double *ptr = nullptr;

@@ -18,6 +18,7 @@
 #include <functional>
 
 #include "ctx.h"
+#include "sq_iter.h"
 
 extern "C" {
 uint64_t si_subseed(uint64_t seed, uint64_t step, uint64_t which);
@@ -32,6 +33,7 @@ constexpr double RANK_TOL = 1e-14;     // reading G9
 // SMs the persistent GEMM leaves free while chains of small kernels run beside it (measured at c3: 4 -> 81.7 ms
 // per step, 8 -> 79.7, 12 -> 80.3, 20 -> 81.2)
 constexpr int CHAIN_SM_RESERVE = 8;
+constexpr int LONE_SM_RESERVE = 16;   // ... to the lone-leg squeezer beside the grouped-leg Gram chains (its iteration is one resident grid)
 constexpr double CLUSTER_TOL = 1e-8;   // reading G12
 
 std::vector<double> d2h(const double *p, long long n)
@@ -416,6 +418,10 @@ struct SqChain {
     Back *back = nullptr;
     std::vector<double> sh;
     int more = 0, k = 0, hist = 0, iters_done = 0, planned = 0;
+    int grid = 0;          // > 0: the iteration runs as one launch of that many CTAs (sq_iter.cu), b = 64 only
+    const double *start = nullptr;
+    double *Ft = nullptr;  // F^T: both products of the fused iteration read rows
+    std::vector<unsigned char> steps;
     double gap = INFINITY;
     Ten Mr, Nr;
     static constexpr double it_shift = 1e-13;
@@ -433,8 +439,13 @@ struct SqChain {
     // estimate: only the singular values are wanted, to two or three digits (iteration count)
     void enqueue_ritz(bool estimate = false)
     {
-        mulFt(Q, Qt);
-        cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
+        if (grid > 0) {
+            steps.push_back(SQ_TRANS | SQ_TWO_PASSES | (2 << SQ_RATIO_SHIFT) | SQ_WANT_R);
+            launch_fused();
+        } else {
+            mulFt(Q, Qt);
+            cholqr_async(Qt, N2, b, 2, 0.0, flag, ratio + 2, Rb);
+        }
         if (b <= 64)
             svd_small_async(Rb, b, b, V, sv, flag, estimate ? 1e-4 : 0.0);
         else
@@ -442,6 +453,26 @@ struct SqChain {
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(back->s, sv, b * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+    }
+    // the half steps collected in `steps` as one launch (sq_iter.cu)
+    void launch_fused()
+    {
+        SqIterParams p{};
+        p.F = F.p;
+        p.Ft = Ft;
+        p.start = start;
+        p.buf[0] = Q;
+        p.buf[1] = Qt;
+        p.Rout = Rb;
+        p.ratio = ratio;
+        p.flag = flag;
+        p.shift = it_shift;
+        p.N2 = N2;
+        p.nsteps = (int)steps.size();
+        if (p.nsteps > SQ_MAXSTEPS) fail(-22, "squeezer: %d half steps in one launch", p.nsteps);
+        std::copy(steps.begin(), steps.end(), p.steps);
+        sq_iter_launch(p, grid, ws_doubles((long long)sq_iter_scratch_doubles(sq_iter_grid(N2, grid))));
+        steps.clear();
     }
     // after the chain's stream has been synchronised
     bool read_back()
@@ -474,6 +505,10 @@ struct SqChain {
         back = reinterpret_cast<Back *>(pinned);
         F = ws_tensor("ij", {N2, N2});
         contract(LL, LR, F);                               // F = L_L^T L_R
+        if (grid > 0) {
+            Ft = ws_doubles((long long)N2 * N2);
+            transpose_small(F.p, Ft, N2, N2);
+        }
         ratio = ws_doubles(4);
         Ten om = solver_start_block(N2, b, mu, "jz");
         Q = ws_doubles((long long)N2 * b);
@@ -483,15 +518,26 @@ struct SqChain {
         sv = ws_doubles(b);
         // Subspace iteration Q <- orth(F orth(F^T Q)).  Between iterations one (shifted) Cholesky-QR
         // pass is enough: only the span is carried on; the blocks that enter a Ritz step get two.
-        mulF(om.p, Q);
-        cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
-        iters_done = hist > 0 ? hist : 2;
-        for (int it = 0; it < iters_done; ++it) {
-            const bool last = it == iters_done - 1;
-            mulFt(Q, Qt);
-            cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
-            mulF(Qt, Q);
-            cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
+        // (fused: a few iterations more than the last count cost less than a second Ritz step would)
+        iters_done = hist > 0 ? hist + (grid > 0 ? 2 : 0) : 2;
+        if (grid > 0) {
+            start = om.p;
+            steps.clear();
+            steps.push_back(SQ_FROM_START);
+            for (int it = 0; it < iters_done; ++it) {
+                steps.push_back(SQ_TRANS);
+                steps.push_back(it == iters_done - 1 ? (SQ_TWO_PASSES | (1 << SQ_RATIO_SHIFT)) : 0);
+            }
+        } else {
+            mulF(om.p, Q);
+            cholqr_async(Q, N2, b, 1, it_shift, flag, nullptr, nullptr);
+            for (int it = 0; it < iters_done; ++it) {
+                const bool last = it == iters_done - 1;
+                mulFt(Q, Qt);
+                cholqr_async(Qt, N2, b, 1, it_shift, flag, nullptr, nullptr);
+                mulF(Qt, Q);
+                cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
+            }
         }
         enqueue_ritz(hist <= 0);
     }
@@ -514,6 +560,11 @@ struct SqChain {
     {
         for (int it = 0; it < more; ++it) {
             const bool last = it == more - 1;
+            if (grid > 0) {
+                steps.push_back(last ? (SQ_TWO_PASSES | (1 << SQ_RATIO_SHIFT)) : 0);
+                if (!last) steps.push_back(SQ_TRANS);
+                continue;
+            }
             mulF(Qt, Q);                                   // Qt = orth(F^T Q) from the Ritz step / the loop
             cholqr_async(Q, N2, b, last ? 2 : 1, last ? 0.0 : it_shift, flag, last ? ratio : nullptr, nullptr);
             if (!last) {
@@ -1176,6 +1227,12 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         }
         for (int mu : act) ch[mu].prep();
         const int na = (int)act.size();
+        const int rsv = reserve >= 0 ? reserve : SM_RESERVE;
+        // the iteration of a chain as one resident grid (sq_iter.cu), one CTA per SM: beside the main stream's GEMMs
+        // a lone chain takes the SMs those leave free (two chains side by side keep the separate launches: a
+        // resident grid that does not fit into the reserve would hold back CTAs of the persistent GEMM)
+        for (int mu : act)
+            ch[mu].grid = ((c.routes & ROUTE_UNFUSED_SQUEEZER) || ch[mu].b != 64) ? 0 : (main_work ? (na == 1 ? rsv : 0) : 32);
         const size_t chain_bytes = main_work ? std::max<size_t>((size_t)64 << 20, (size_t)(6 * n2max * n2max * 8)) : 0;
         Fork fk(2 * na, (bool)main_work, chain_bytes);
         for (int i = 0; i < na; ++i)           // the two Cholesky factorisations of a chain side by side
@@ -1189,7 +1246,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         trace_mark("sq chain 0: cholesky x2");
         fk.leave();
         if (main_work) {
-            c.sm_reserve = reserve >= 0 ? reserve : SM_RESERVE;
+            c.sm_reserve = rsv;
             main_work();
             c.sm_reserve = 0;
         }
@@ -1505,7 +1562,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         }
         if (overlapped) {
             stage_mark(5);
-            squeeze_wave({2}, gram_grouped);   // (4 - 20 reserved SMs make no difference here: this chain is latency-bound)
+            squeeze_wave({2}, gram_grouped, nullptr, LONE_SM_RESERVE);
             if (!done[2]) squeeze_dense(2);
         } else {
             gram_grouped();

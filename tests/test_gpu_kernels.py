@@ -210,6 +210,41 @@ def test_cholqr_single_shifted_pass_spans_the_block(tt):
     assert np.abs(Q - Qr @ (Qr.T @ Q)).max() < 1e-9
 
 
+@pytest.mark.parametrize("n,grid,iters", [(1024, 16, 6), (1024, 8, 6), (256, 32, 8), (289, 7, 8), (400, 64, 8), (1000, 9, 6)])
+def test_subspace_iteration_fused(tt, n, grid, iters):
+    """The squeezer's subspace iteration as one resident grid (sq_iter.cu; Eq. 12, DESIGN.md
+    "Squeezers") against LAPACK: on a matrix whose singular values fall off as 10^(-i/16) (s_64 = 1e-4 s_1: the block
+    stays well inside what two Cholesky-QR passes can orthonormalise), `iters` iterations with a block of 64 give
+    orthonormal Q, Qt, the factorisation F^T Q = Qt R, and in R the leading 32 singular values of F to 1e-12
+    (neglected part (s_65/s_32)^(2 iters + 1) = 1e-27 at 6 iterations).  Sizes: several row blocks per CTA, one
+    row block per CTA, n odd (scalar operand loads), n not a multiple of 8 (ragged last block)."""
+    import torch
+    rng = np.random.default_rng(n + grid)
+    Ul, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    Vr, _ = np.linalg.qr(rng.standard_normal((n, n)))
+    sv = 10.0 ** (-np.arange(n) / 16.0)
+    sv[100:] = sv[100] * 10.0 ** (-np.arange(n - 100) / 400.0)     # a long, nearly flat tail below 1e-6
+    F = (Ul * sv) @ Vr.T
+    start = rng.standard_normal((n, 64))
+    dF, dS = _dev(F), _dev(start)
+    dQ = torch.zeros(n, 64, dtype=torch.float64, device="cuda")
+    dQt = torch.zeros(n, 64, dtype=torch.float64, device="cuda")
+    dR = torch.zeros(64, 64, dtype=torch.float64, device="cuda")
+    dmm = torch.zeros(4, dtype=torch.float64, device="cuda")
+    assert tt.subspace_iteration(dF, dS, dQ, dQt, iters, grid=grid, R=dR, minmax=dmm)
+    Q, Qt, R, mm = dQ.cpu().numpy(), dQt.cpu().numpy(), dR.cpu().numpy(), dmm.cpu().numpy()
+    assert np.abs(Q.T @ Q - np.eye(64)).max() < 1e-13
+    assert np.abs(Qt.T @ Qt - np.eye(64)).max() < 1e-13
+    assert np.abs(np.tril(R, -1)).max() == 0.0
+    assert np.abs(F.T @ Q - Qt @ R).max() < 1e-14
+    s_it = np.linalg.svd(R, compute_uv=False)
+    assert np.abs(s_it[:32] - sv[:32]).max() < 1e-12, np.abs(s_it[:32] - sv[:32]).max()
+    assert 0 < mm[0] <= mm[1] and 0 < mm[2] <= mm[3]
+    # the span of Q holds the leading left singular vectors
+    P = Ul[:, :32] - Q @ (Q.T @ Ul[:, :32])
+    assert np.abs(P * sv[:32]).max() < 1e-12
+
+
 @pytest.mark.parametrize("M,N,K", [(1000, 64, 300), (4096, 40, 1024), (130, 64, 20000), (40, 3000, 256),
                                    (1024, 1024, 32768), (200, 200, 9000)])
 def test_tensor_gemm_tile_variants(tt, M, N, K):

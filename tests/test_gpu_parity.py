@@ -294,12 +294,13 @@ def test_critical_temperature_bisection(tt):
     assert 6.4 < Tc < 7.2, Tc
 
 
-@pytest.mark.parametrize("mask", [1, 2, 4, 8, 15])
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 15, 32])
 def test_robust_routes_give_the_same_step(tt, mask):
     """Every stage has a fast route and a robust route that follows the oracle's algorithm step by step
     (tatrg_set_routes): bit 0 plain chi^4-dimensional bond-swap operator instead of the
     reduced chi^3 core, bit 1 Householder TSQR instead of Cholesky-QR, bit 2 dense eigendecompositions instead
-    of Cholesky + subspace iteration in the squeezers, bit 3 sequential isometries.  Config 2 (chi = 16), 10
+    of Cholesky + subspace iteration in the squeezers, bit 3 sequential isometries, bit 5 the squeezers' subspace
+    iteration as separate launches instead of the one resident grid of sq_iter.cu.  Config 2 (chi = 16), 10
     steps: from step 5 on every fast route is taken by default (GPU against GPU)."""
     import paper_2412_14104_b200 as t
     beta, chi, r, q, seed, n = 1 / 6.65, 16, 2, 2, 20241215, 10
