@@ -1229,10 +1229,12 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         const int na = (int)act.size();
         const int rsv = reserve >= 0 ? reserve : SM_RESERVE;
         // the iteration of a chain as one resident grid (sq_iter.cu), one CTA per SM: beside the main stream's GEMMs
-        // a lone chain takes the SMs those leave free (two chains side by side keep the separate launches: a
-        // resident grid that does not fit into the reserve would hold back CTAs of the persistent GEMM)
-        for (int mu : act)
-            ch[mu].grid = ((c.routes & ROUTE_UNFUSED_SQUEEZER) || ch[mu].b != 64) ? 0 : (main_work ? (na == 1 ? rsv : 0) : 32);
+        // it takes the SMs those leave free, so two chains run their grids one after the other (resident grids that
+        // do not fit into the reserve together would hold back CTAs of the persistent GEMM)
+        bool fused = !(c.routes & ROUTE_UNFUSED_SQUEEZER);
+        for (int mu : act) fused = fused && ch[mu].b == 64;
+        for (int mu : act) ch[mu].grid = fused ? (main_work ? rsv : 32) : 0;
+        const bool one_grid_at_a_time = fused && main_work && na > 1;
         const size_t chain_bytes = main_work ? std::max<size_t>((size_t)64 << 20, (size_t)(6 * n2max * n2max * 8)) : 0;
         Fork fk(2 * na, (bool)main_work, chain_bytes);
         for (int i = 0; i < na; ++i)           // the two Cholesky factorisations of a chain side by side
@@ -1251,6 +1253,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             c.sm_reserve = 0;
         }
         for (int i = 0; i < na; ++i) {
+            if (one_grid_at_a_time && i > 0) fk.side_after_side(2 * i, 2 * (i - 1));
             fk.enter(2 * i);
             ch[act[i]].phaseA(fk.pinned(2 * i));
             fk.leave();
@@ -1265,8 +1268,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 fprintf(stderr, "tatrg-trace squeezer mu %d: hist %d done %d planned %d more %d ok %d\n", act[i], ch[act[i]].hist,
                         ch[act[i]].iters_done, ch[act[i]].planned, ch[act[i]].more, (int)ch[act[i]].ok);
         }
-        for (int i = 0; i < na; ++i)
+        for (int i = 0, prev = -1; i < na; ++i)
             if (ch[act[i]].ok && ch[act[i]].more > 0) {
+                if (one_grid_at_a_time && prev >= 0) fk.side_after_side(2 * i, 2 * prev);
+                prev = i;
                 fk.enter(2 * i);
                 ch[act[i]].phaseB();
                 fk.leave();
