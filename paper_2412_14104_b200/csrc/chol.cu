@@ -4,6 +4,7 @@
 // NB x NB diagonal block is factored and inverted by one CTA in shared memory, the panel and the
 // trailing update are tensor-GEMM launches (gemm.cu), so all O(n^3) work runs on the FP64 tensor
 // pipe.
+#include <algorithm>
 #include "ctx.h"
 #include "chol64.cuh"
 
@@ -55,6 +56,182 @@ __global__ void __launch_bounds__(CH_NT) chol_block_kernel(double *__restrict__ 
         }
         dminmax[0] = lo;
         dminmax[1] = hi;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The blocked factorisation as ONE resident grid (n > 64).  Launched panel by panel it is 3 dependent launches per
+// 64 columns (diagonal block, panel, trailing update): 48 launches and 1.2 - 1.5 ms for n = 1024, nearly all of it
+// launch and dependency latency -- and a squeezer chain starts with two of them.  Here G CTAs stay resident and
+// meet at two grid-wide barriers per panel:
+//   every CTA factors the diagonal block itself (chol64.cuh: identical code on identical bytes; no barrier and no
+//   broadcast of L_jj^-1 needed), the warps of all CTAs share out the rows of the panel L21 = A21 L_jj^-T (DMMA,
+//   B fragments from L_jj^-1 in shared memory)  -> barrier ->  the CTAs share out the 64 x 64 tiles of the lower
+//   triangle of the trailing block, A22[I][K] -= L21[I] L21[K]^T, both operands staged in shared memory -> barrier.
+constexpr int CR_LD = 68;
+
+struct CholResSmem {
+    union {
+        Chol64Work wk;
+        struct {
+            double LI[NB][CR_LD];
+            double LK[NB][CR_LD];
+        } t;
+    };
+    double Ls[NB][CR_LD];   // L_jj^-1
+    double diag[NB];
+    int bad;
+};
+
+__device__ __forceinline__ void cr_dmma(double &d0, double &d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(d0), "+d"(d1)
+                 : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cr_grid_barrier(unsigned *bar, unsigned &target)
+{
+    target += gridDim.x;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;\n" ::"l"(bar) : "memory");
+        unsigned v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(CH_NT, 1) chol_resident_kernel(double *__restrict__ A, int n, double *__restrict__ Linv,
+                                                                 long long ldinv, long long inv_step,
+                                                                 int *__restrict__ flag, unsigned *__restrict__ bar)
+{
+    extern __shared__ __align__(16) unsigned char cr_smem[];
+    CholResSmem &sm = *reinterpret_cast<CholResSmem *>(cr_smem);
+    const int t = threadIdx.x, warp = t >> 5, lane = t & 31, g = lane >> 2, q = lane & 3;
+    const int ty = t >> 4, tx = t & 15;
+    unsigned target = 0;
+    for (int j0 = 0; j0 < n; j0 += NB) {
+        const int nb = n - j0 < NB ? n - j0 : NB;
+        // ---- diagonal block, by every CTA
+        double s[4][4], w[4][4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int i = 4 * ty + a, c = 4 * tx + b;
+                const int r = i > c ? i : c, cc = i > c ? c : i;   // lower-triangle source
+                s[a][b] = (r < nb) ? __ldcg(A + (long long)(j0 + r) * n + j0 + cc) : (i == c ? 1.0 : 0.0);
+                if (i == c) sm.diag[i] = (i < nb) ? s[a][b] : 0.0;
+            }
+        __syncthreads();
+        chol64_factor(s, w, sm.wk, sm.diag, &sm.bad, nb, 0.0);
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int i = 4 * ty + a, c = 4 * tx + b;
+                sm.Ls[i][c] = (c <= i) ? w[a][b] : 0.0;
+                if (blockIdx.x == 0 && i < nb && c < nb)
+                    Linv[(j0 / NB) * inv_step + i * ldinv + c] = (c <= i) ? w[a][b] : 0.0;
+            }
+        if (blockIdx.x == 0 && t == 0 && sm.bad) *flag = 1;
+        __syncthreads();
+        const int below = n - j0 - NB;   // rows under the diagonal block
+        if (below > 0) {
+            // ---- panel: 8-row units shared out over all warps of the grid; in place (a unit's rows are its own)
+            const int nu = (below + 7) / 8;
+            for (int u = blockIdx.x * (CH_NT / 32) + warp; u < nu; u += gridDim.x * (CH_NT / 32)) {
+                const int r = j0 + NB + 8 * u + g;
+                double *row = A + (long long)(r < n ? r : 0) * n + j0;
+                double af[16];
+#pragma unroll
+                for (int ks = 0; ks < 16; ++ks) af[ks] = (r < n) ? __ldcg(row + 4 * ks + q) : 0.0;
+#pragma unroll
+                for (int cb = 0; cb < 8; ++cb) {
+                    double d0 = 0.0, d1 = 0.0;
+#pragma unroll
+                    for (int ks = 0; ks < 16; ++ks) cr_dmma(d0, d1, af[ks], sm.Ls[cb * 8 + g][ks * 4 + q]);
+                    if (r < n) {
+                        row[cb * 8 + 2 * q] = d0;
+                        row[cb * 8 + 2 * q + 1] = d1;
+                    }
+                }
+            }
+        }
+        cr_grid_barrier(bar, target);   // the panel is complete; nobody reads the old diagonal block any more
+        if (blockIdx.x == 0) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const int i = 4 * ty + a, c = 4 * tx + b;
+                    if (i < nb && c < nb) A[(long long)(j0 + i) * n + j0 + c] = (c <= i) ? s[a][b] : 0.0;
+                }
+        }
+        if (below <= 0) break;
+        // ---- trailing update: tiles (I, K), K <= I, of the blocks under / right of the panel
+        const int nbk = (below + NB - 1) / NB, ntile = nbk * (nbk + 1) / 2;
+        for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+            int I = (int)((sqrtf(8.0f * tile + 1.0f) - 1.0f) * 0.5f);
+            while (I * (I + 1) / 2 > tile) --I;
+            while ((I + 1) * (I + 2) / 2 <= tile) ++I;
+            const int K = tile - I * (I + 1) / 2;
+            const int ri = j0 + NB + I * NB, rk = j0 + NB + K * NB;
+            __syncthreads();   // the previous tile's fragments have been read
+            {   // all loads in flight before the first store (thread t: column t & 63 of rows (t >> 6) + 4 i)
+                const int cc = t & 63, rr0 = t >> 6;
+                double vi[16], vk[16];
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const int rr = rr0 + 4 * i;
+                    vi[i] = (ri + rr < n) ? __ldcg(A + (long long)(ri + rr) * n + j0 + cc) : 0.0;
+                    vk[i] = (K != I && rk + rr < n) ? __ldcg(A + (long long)(rk + rr) * n + j0 + cc) : 0.0;
+                }
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    sm.t.LI[rr0 + 4 * i][cc] = vi[i];
+                    sm.t.LK[rr0 + 4 * i][cc] = vk[i];
+                }
+            }
+            __syncthreads();
+            const double(*LK)[CR_LD] = (K != I) ? sm.t.LK : sm.t.LI;
+            double acc[8][2];
+#pragma unroll
+            for (int cb = 0; cb < 8; ++cb) acc[cb][0] = acc[cb][1] = 0.0;
+#pragma unroll
+            for (int ks = 0; ks < 16; ++ks) {
+                const double a = sm.t.LI[warp * 8 + g][ks * 4 + q];
+#pragma unroll
+                for (int cb = 0; cb < 8; ++cb) cr_dmma(acc[cb][0], acc[cb][1], a, LK[cb * 8 + g][ks * 4 + q]);
+            }
+            const int r = ri + warp * 8 + g;
+            if (r < n) {
+                double *row = A + (long long)r * n + rk;
+                double old[8][2];
+#pragma unroll
+                for (int cb = 0; cb < 8; ++cb) {
+                    const int c = cb * 8 + 2 * q;
+                    old[cb][0] = (rk + c < n) ? __ldcg(row + c) : 0.0;
+                    old[cb][1] = (rk + c + 1 < n) ? __ldcg(row + c + 1) : 0.0;
+                }
+#pragma unroll
+                for (int cb = 0; cb < 8; ++cb) {
+                    const int c = cb * 8 + 2 * q;
+                    if (rk + c < n) row[c] = old[cb][0] - acc[cb][0];
+                    if (rk + c + 1 < n) row[c + 1] = old[cb][1] - acc[cb][1];
+                }
+            }
+        }
+        cr_grid_barrier(bar, target);
+    }
+    // ---- strict upper triangle of the result: zero
+    const long long total = (long long)n * n;
+    for (long long i = (long long)blockIdx.x * CH_NT + t; i < total; i += (long long)gridDim.x * CH_NT) {
+        const int r = (int)(i / n), c = (int)(i - (long long)r * n);
+        if (c > r && (c / NB) > (r / NB)) A[i] = 0.0;   // (inside the diagonal blocks CTA 0 has written the zeros)
     }
 }
 
@@ -145,6 +322,24 @@ void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full,
     }
     if (Linv_full) fill_zero(Linv_full, (long long)n * n);
     chol_attr();
+    const int want_ctas = ctx().chol_ctas;
+    if (n > NB && want_ctas > 0) {
+        // one resident grid (chol_resident_kernel); the inverted diagonal blocks go to Linv_full's diagonal blocks or
+        // (not wanted) to one scratch block
+        static bool res_attr = false;
+        if (!res_attr) {
+            TATRG_CUDA_CHECK(cudaFuncSetAttribute(chol_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(CholResSmem)));
+            res_attr = true;
+        }
+        unsigned *bar = reinterpret_cast<unsigned *>(ws_alloc(sizeof(unsigned)));
+        TATRG_CUDA_CHECK(cudaMemsetAsync(bar, 0, sizeof(unsigned), stream()));
+        const int grid = std::max(1, std::min(want_ctas, (n + NB - 1) / NB * 2));
+        chol_resident_kernel<<<grid, CH_NT, sizeof(CholResSmem), stream()>>>(A, n, Linv_full ? Linv_full : Linv, Linv_full ? n : NB,
+                                                                         Linv_full ? (long long)NB * n + NB : 0, flag, bar);
+        TATRG_LAUNCH_CHECK();
+        count_launch();
+        count_flops((double)n * n * n / 3.0);
+    } else {
     for (int j0 = 0; j0 < n; j0 += NB) {
         const int nb = n - j0 < NB ? n - j0 : NB;
         double *Ajj = A + (long long)j0 * n + j0;
@@ -169,6 +364,7 @@ void cholesky_lower_async(double *A, int n, double shift_rel, double *Linv_full,
     zero_upper_kernel<<<blocks, 256, 0, stream()>>>(A, n);
     TATRG_LAUNCH_CHECK();
     count_launch();
+    }
     if (Linv_full) {
         // L^-1 from the inverted diagonal blocks, doubling the block size:
         // inv([L11 0; L21 L22]) = [inv11 0; -inv22 L21 inv11, inv22]; equal pairs of one level are one batched GEMM

@@ -59,6 +59,7 @@ struct Ctx {
     Input in[9];
     int sq_hist[4][3] = {};                 // subspace iterations each squeezer needed, per direction (step.cpp: SqChain)
     int sm_reserve = 0;                     // SMs the persistent GEMM leaves to concurrent chains (step.cpp)
+    int chol_ctas = 16;                     // CTAs of the resident blocked Cholesky (chol.cu); 0: one launch per panel step
     int routes = 0;                         // mask of Route: robust routes forced by tatrg_set_routes
     bool keep_iso = false;                  // tatrg_keep_isometries: host copies of U^A, U^X, U^Y, U^D of the last step
     std::vector<double> iso[4];

@@ -766,11 +766,13 @@ bool ortho_factor_pair(const Ten &A, const Ten &D, RedBasis &bA, RedBasis &bD,
         const size_t chain_bytes = std::max<size_t>((size_t)32 << 20, (size_t)(4 * ch[0].nk * ch[0].nk * 8));
         const bool beside = during_last && c.hi - c.lo > 2 * chain_bytes + ((size_t)64 << 20);
         Fork fk(2, beside, beside ? chain_bytes : 0);
+        if (beside) c.chol_ctas = CHAIN_SM_RESERVE / 2;
         for (int i = 0; i < 2; ++i) {
             fk.enter(i);
             ch[i].phase2_factor();
             fk.leave();
         }
+        c.chol_ctas = 16;
         if (beside) {
             c.sm_reserve = CHAIN_SM_RESERVE;
             during_last(ch[1].o);
@@ -1237,12 +1239,14 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         const bool one_grid_at_a_time = fused && main_work && na > 1;
         const size_t chain_bytes = main_work ? std::max<size_t>((size_t)64 << 20, (size_t)(6 * n2max * n2max * 8)) : 0;
         Fork fk(2 * na, (bool)main_work, chain_bytes);
+        c.chol_ctas = main_work ? std::max(2, rsv / (2 * na)) : 16;   // resident grids (chol.cu) that fit into the reserve together
         for (int i = 0; i < na; ++i)           // the two Cholesky factorisations of a chain side by side
             for (int w = 0; w < 2; ++w) {
                 fk.enter(2 * i + w);
                 ch[act[i]].factor(w);
                 fk.leave();
             }
+        c.chol_ctas = 16;
         for (int i = 0; i < na; ++i) fk.side_after_side(2 * i, 2 * i + 1);
         fk.enter(0);
         trace_mark("sq chain 0: cholesky x2");
