@@ -16,7 +16,9 @@ namespace tatrg {
 
 namespace {
 
-constexpr int SJ_NT = 1024;
+constexpr int SJ_NT = 1024;   // eig_small_kernel
+constexpr int SV_NT = 256;    // svd_small_kernel: 8 warps x 4 pairs, 8 lanes per pair
+constexpr int SV_LPP = 8;     // lanes per pair
 constexpr int SJ_MAX = 64;
 
 __device__ __forceinline__ double warp_sum(double v)
@@ -42,29 +44,38 @@ __device__ __forceinline__ void rr_pair(int round, int pi, int npad, int &p, int
     }
 }
 
+// column stride of the working array: rows of G, rows of V, and a pad that spreads the four pairs of a warp
+// over the shared-memory banks
+__host__ __device__ inline int svd_small_ld(int m, int n) { return m + n + (((m + n) & 15) == 0 ? 8 : 0); }
+
 // G: m x n column-major (ld = m) in global; on exit G = U diag(s) sorted, V (n x n column-major), s[n].
-__global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ Gg, int m, int n,
+// A round of the round-robin ordering rotates n/2 disjoint column pairs.  A pair is latency, not work (one dot
+// product, ~40 dependent FP64 operations for the rotation, 2 (m + n) updated entries), and the FP64 pipe issues
+// one warp instruction whatever the number of lanes that need it: so a warp takes FOUR pairs, eight lanes each
+// (the rotation is computed once per warp instruction for four pairs), and 8 warps cover the 32 pairs of n = 64.
+__global__ void __launch_bounds__(SV_NT) svd_small_kernel(double *__restrict__ Gg, int m, int n,
                                                          double *__restrict__ Vg, double *__restrict__ sg,
                                                          double tol, int max_sweeps, int *__restrict__ fail_flag)
 {
     extern __shared__ double sm[];
-    const int ld = m + n;              // column j = sm[j*ld .. j*ld+m) (G part) then n entries of V
+    const int ld = svd_small_ld(m, n);   // column j = sm[j*ld .. j*ld+m) (G part) then n entries of V
     double *W = sm;
     __shared__ int nrot;
     __shared__ double fro2_s;
     __shared__ double nrm[SJ_MAX];
     __shared__ int perm[SJ_MAX];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-    constexpr int NW = SJ_NT / 32;
+    constexpr int NW = SV_NT / 32;
+    constexpr unsigned FULL = 0xffffffffu;
 
-    for (int i = t; i < n * ld; i += SJ_NT) {
+    for (int i = t; i < n * ld; i += SV_NT) {
         int j = i / ld, r = i - j * ld;
         W[i] = (r < m) ? Gg[(long long)j * m + r] : ((r - m == j) ? 1.0 : 0.0);
     }
     __syncthreads();
     {   // Frobenius norm (for the dead-column rule)
         double a = 0.0;
-        for (int i = t; i < n * ld; i += SJ_NT) {
+        for (int i = t; i < n * ld; i += SV_NT) {
             int r = i % ld;
             if (r < m) a = fma(W[i], W[i], a);
         }
@@ -77,6 +88,7 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
     const double dead = 1e-40 * fro2_s;
     const double tol2 = tol * tol;
     const int npad = n + (n & 1);
+    const int sub = lane & (SV_LPP - 1), grp = lane / SV_LPP;
     int sweep = 0;
     for (; n > 1 && sweep < max_sweeps; ++sweep) {
         if (t == 0) nrot = 0;
@@ -90,20 +102,27 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
         }
         __syncthreads();
         for (int round = 0; round < npad - 1; ++round) {
-            for (int pi = warp; pi < npad / 2; pi += NW) {
-                int p, q;
-                rr_pair(round, pi, npad, p, q);
-                if (q >= n) continue;
+            // every lane of the warp runs through the same instructions (no branch of its own before the shuffles)
+            for (int pi0 = warp * (32 / SV_LPP); pi0 < npad / 2; pi0 += NW * (32 / SV_LPP)) {
+                const int pi = pi0 + grp;
+                int p = 0, q = 0;
+                if (pi < npad / 2) rr_pair(round, pi, npad, p, q);
+                const bool valid = pi < npad / 2 && q < n;
+                if (!valid) p = q = 0;
                 double *cp = W + p * ld, *cq = W + q * ld;
                 const double aa = nrm[p], bb = nrm[q];
-                if (aa == 0.0 && bb == 0.0) continue;
-                double ab = 0.0;
-                for (int i = lane; i < m; i += 32) ab = fma(cp[i], cq[i], ab);
-                ab = warp_sum(ab);
-                const bool swap = aa < bb;
+                double ab0 = 0.0, ab1 = 0.0;
+                for (int i = sub; i < m; i += 2 * SV_LPP) {
+                    ab0 = fma(cp[i], cq[i], ab0);
+                    if (i + SV_LPP < m) ab1 = fma(cp[i + SV_LPP], cq[i + SV_LPP], ab1);
+                }
+                double ab = ab0 + ab1;
+                for (int o = SV_LPP / 2; o > 0; o >>= 1) ab += __shfl_xor_sync(FULL, ab, o);
+                const bool live = valid && !(aa == 0.0 && bb == 0.0);
+                const bool swap = live && aa < bb;
                 double c = 1.0, s = 0.0, na2 = aa, nb2 = bb;
                 bool rot = false;
-                if (aa > dead && bb > dead && ab * ab > tol2 * aa * bb) {
+                if (live && aa > dead && bb > dead && ab * ab > tol2 * aa * bb) {
                     // tan of the rotation angle: the smaller root of t^2 + 2 zeta t - 1 = 0, zeta = (bb - aa) / (2 ab)
                     const double dlt = bb - aa;
                     const double tt = copysign(2.0 * fabs(ab), dlt * ab) / (fabs(dlt) + sqrt(fma(dlt, dlt, 4.0 * ab * ab)));
@@ -112,19 +131,21 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
                     na2 = aa - tt * ab;
                     nb2 = bb + tt * ab;
                     rot = true;
-                    if (lane == 0) atomicAdd(&nrot, 1);
                 }
-                if (!rot && !swap) continue;
-                for (int i = lane; i < ld; i += 32) {
-                    double a = cp[i], b = cq[i];
-                    double na = c * a - s * b, nb = s * a + c * b;
-                    cp[i] = swap ? nb : na;
-                    cq[i] = swap ? na : nb;
+                if (rot || swap) {
+                    for (int i = sub; i < m + n; i += SV_LPP) {
+                        double a = cp[i], b = cq[i];
+                        double na = c * a - s * b, nb = s * a + c * b;
+                        cp[i] = swap ? nb : na;
+                        cq[i] = swap ? na : nb;
+                    }
+                    if (sub == 0) {
+                        nrm[p] = swap ? nb2 : na2;
+                        nrm[q] = swap ? na2 : nb2;
+                        if (rot) atomicAdd(&nrot, 1);
+                    }
                 }
-                if (lane == 0) {
-                    nrm[p] = swap ? nb2 : na2;
-                    nrm[q] = swap ? na2 : nb2;
-                }
+                __syncwarp();
             }
             __syncthreads();
         }
@@ -147,12 +168,12 @@ __global__ void __launch_bounds__(SJ_NT) svd_small_kernel(double *__restrict__ G
         perm[r] = t;
     }
     __syncthreads();
-    for (int i = t; i < n * ld; i += SJ_NT) {
+    for (int i = t; i < n * ld; i += SV_NT) {
         int j = i / ld, r = i - j * ld;
         double v = W[perm[j] * ld + r];
         if (r < m)
             Gg[(long long)j * m + r] = v;
-        else
+        else if (r < m + n)
             Vg[(long long)j * n + (r - m)] = v;
     }
     if (t < n) sg[t] = nrm[perm[t]];
@@ -270,7 +291,7 @@ void set_attr()
 {
     if (attr_done) return;
     TATRG_CUDA_CHECK(cudaFuncSetAttribute(svd_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(SJ_MAX * 2 * SJ_MAX * sizeof(double))));
+                                          (int)(SJ_MAX * svd_small_ld(SJ_MAX, SJ_MAX) * sizeof(double))));
     TATRG_CUDA_CHECK(cudaFuncSetAttribute(eig_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)(2 * SJ_MAX * (SJ_MAX + 1) * sizeof(double))));
     attr_done = true;
@@ -284,8 +305,8 @@ void svd_small_async(double *G, int m, int n, double *V, double *s, int *flag_de
     set_attr();
     const int mn = m > n ? m : n;
     const double tol = tol_override > 0.0 ? tol_override : 8.0 * sqrt((double)(mn > 16 ? mn : 16)) * 1.1102230246251565e-16;
-    const size_t smem = (size_t)n * (m + n) * sizeof(double);
-    svd_small_kernel<<<1, SJ_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag_dev);
+    const size_t smem = (size_t)n * svd_small_ld(m, n) * sizeof(double);
+    svd_small_kernel<<<1, SV_NT, smem, stream()>>>(G, m, n, V, s, tol, 100, flag_dev);
     TATRG_LAUNCH_CHECK();
     count_launch();
 }
