@@ -218,6 +218,19 @@ int tatrg_jacobi_svd(double *G, int m, int n, double *V, double *s);
 /* Norm / trace reductions of the normalisation and of tTr T = <Phi,Psi> (Eq. 15):
  * out_dev[0] = sum x^2, resp. sum x*y; x *= 1/sqrt(*sumsq_dev).  All pointers device. */
 int tatrg_sumsq(const double *x, int64_t n, double *out_dev);
+
+/* tatrg_sumsq for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): out_dev[0] = sum_i x[i]^2 (the squared Frobenius norm of the step's normalisation,
+ * PAPER.md:119 Eq. 15) by the same two kernels on the same grid as tatrg_sumsq -- the result is equal to the last
+ * bit -- with the per-CTA partial sums in a static device array of the library (1184 doubles = 9472 bytes per GPU,
+ * held from library load to process exit) instead of the workspace.  Needs no tatrg_set_workspace, calls no
+ * cudaMalloc / cudaFree or any allocating routine, and does not synchronise: the two kernels are enqueued on the
+ * stream of tatrg_set_stream (default stream if none).  x: device, n doubles (n >= 0; n = 0 gives 0); out_dev:
+ * device, 1 double, written.  n > TATRG_SUMSQ_STATIC_MAX_N is rejected with TATRG_EINVAL and nothing is launched.
+ * All calls share the static array (it keeps the last call's partial sums; nothing in it has to start at zero):
+ * calls whose kernels overlap on the GPU race -- order them on one stream or with events. */
+#define TATRG_SUMSQ_STATIC_MAX_N (1LL << 32)   /* elements (32 GiB of doubles; chi^5 at chi = 64 is 2^30) */
+int tatrg_sumsq_static(const double *x, int64_t n, double *out_dev);
 int tatrg_dot(const double *x, const double *y, int64_t n, double *out_dev);
 int tatrg_scale_by_rsqrt(double *x, int64_t n, const double *sumsq_dev);
 

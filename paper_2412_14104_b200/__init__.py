@@ -24,7 +24,7 @@ EXPORTS = [
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name", "tatrg_get_h2d",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
-    "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_subspace_iteration", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_dot", "tatrg_scale_by_rsqrt",
+    "tatrg_fill_gauss", "tatrg_qr_pos", "tatrg_cholesky", "tatrg_cholqr", "tatrg_subspace_iteration", "tatrg_jacobi_svd", "tatrg_sumsq", "tatrg_sumsq_static", "tatrg_dot", "tatrg_scale_by_rsqrt",
     "tatrg_last_error", "tatrg_destroy",
 ]
 
@@ -85,6 +85,7 @@ def lib():
             "tatrg_subspace_iteration": (c_i, [c_vp, c_i, c_vp, c_vp, c_vp, c_i, c_i, c_vp, c_vp]),
             "tatrg_jacobi_svd": (c_i, [c_vp, c_i, c_i, c_vp, c_vp]),
             "tatrg_sumsq": (c_i, [c_vp, c_i64, c_vp]),
+            "tatrg_sumsq_static": (c_i, [c_vp, c_i64, c_vp]),
             "tatrg_dot": (c_i, [c_vp, c_vp, c_i64, c_vp]),
             "tatrg_scale_by_rsqrt": (c_i, [c_vp, c_i64, c_vp]),
             "tatrg_last_error": (ctypes.c_char_p, []),
@@ -393,6 +394,14 @@ def jacobi_svd(G, V, s):
 
 def sumsq(x, out):
     _check(lib().tatrg_sumsq(x.data_ptr(), x.numel(), out.data_ptr()))
+
+
+SUMSQ_STATIC_MAX_N = 1 << 32
+
+
+def sumsq_static(x, out, n=None):
+    """sumsq without workspace or allocation (static device scratch of the library); n defaults to x.numel()."""
+    _check(lib().tatrg_sumsq_static(x.data_ptr(), x.numel() if n is None else int(n), out.data_ptr()))
 
 
 def dot(x, y, out):

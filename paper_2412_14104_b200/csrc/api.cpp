@@ -599,6 +599,17 @@ int tatrg_sumsq(const double *x, int64_t n, double *out_dev)
     });
 }
 
+int tatrg_sumsq_static(const double *x, int64_t n, double *out_dev)
+{
+    return guarded([&] {
+        if (!out_dev || n < 0 || (n > 0 && !x)) fail(TATRG_EINVAL, "tatrg_sumsq_static: need out_dev, n >= 0 and x for n > 0");
+        if (n > (int64_t)TATRG_SUMSQ_STATIC_MAX_N)
+            fail(TATRG_EINVAL, "tatrg_sumsq_static: n = %lld exceeds the maximum of %lld elements", (long long)n,
+                 (long long)TATRG_SUMSQ_STATIC_MAX_N);
+        sumsq_static(x, n, out_dev);
+    });
+}
+
 int tatrg_dot(const double *x, const double *y, int64_t n, double *out_dev)
 {
     return guarded([&] {

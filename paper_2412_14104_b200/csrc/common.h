@@ -124,6 +124,7 @@ void eig_small(const double *S, int n, double *V, double *lam);   // symmetric S
 // reduce.cu
 void sumsq(const double *x, long long n, double *out);                       // out[0] = sum x^2
 void dot(const double *x, const double *y, long long n, double *out);        // out[0] = sum x y
+void sumsq_static(const double *x, long long n, double *out);                // sumsq with static scratch: no workspace, no allocation
 void scale_by_rsqrt(double *x, long long n, const double *sumsq_dev);        // x *= 1/sqrt(*sumsq)
 // x[i, c] *= f(v[c]) for a row-major (rows x cols) array; mode 0: v, 1: 1/v, 2: sqrt(v), 3: 1/sqrt(v), 4: v^2
 void scale_cols(double *x, long long rows, int cols, const double *v, int mode);

@@ -5,6 +5,13 @@
 //   deterministic two-pass reductions (no atomics).
 #include "common.h"
 
+// Scratch of sumsq_static (below): the per-CTA partial sums of the two-pass reduction, one slot per CTA of the
+// largest grid (148 x 8 = 1184 doubles = 9472 bytes).  A file-scope device array: every GPU that loads the library
+// holds it until the process exits; no call allocates it.  In HOST code this name is a host-side stand-in, not a
+// device address -- the launcher below asks the runtime for the address (cudaGetSymbolAddress) once per device.
+#define TATRG_SUMSQ_STATIC_SLOTS (148 * 8)
+static __device__ __align__(256) double g_sumsq_static_partials[TATRG_SUMSQ_STATIC_SLOTS];
+
 namespace tatrg {
 
 namespace {
@@ -198,6 +205,32 @@ void dot(const double *x, const double *y, long long n, double *out)
     TATRG_LAUNCH_CHECK();
     count_launch(2);
     ws_release(mark);
+}
+
+// sumsq without any allocation and without the caller's workspace (tatrg_sumsq_static): the same two kernels on the
+// same grid as sumsq -- the result is the same to the last bit -- with the partial sums in the file-scope array
+// g_sumsq_static_partials.  Its device address is looked up once per device, with that device current.  Nothing in
+// the array has to start at zero: pass 1 writes every slot that pass 2 reads.  All calls share the array, so two
+// calls whose kernels overlap on the GPU (different streams, no dependency between them) race.
+void sumsq_static(const double *x, long long n, double *out)
+{
+    constexpr int MAX_DEVICES = 64;
+    static double *scratch_of_device[MAX_DEVICES] = {};
+    int dev = -1;
+    TATRG_CUDA_CHECK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) fail(-22, "sumsq_static: device ordinal %d not supported", dev);
+    if (!scratch_of_device[dev]) {
+        void *p = nullptr;
+        TATRG_CUDA_CHECK(cudaGetSymbolAddress(&p, g_sumsq_static_partials));
+        scratch_of_device[dev] = static_cast<double *>(p);
+    }
+    double *partial = scratch_of_device[dev];
+    const int g = grid_for(n, 8);
+    if (g > TATRG_SUMSQ_STATIC_SLOTS) fail(-22, "sumsq_static: %d partial sums exceed the %d static slots", g, TATRG_SUMSQ_STATIC_SLOTS);
+    reduce_pass1<0><<<g, RED_THREADS, 0, stream()>>>(x, nullptr, n, partial);
+    reduce_pass2<<<1, RED_THREADS, 0, stream()>>>(partial, g, out);
+    TATRG_LAUNCH_CHECK();
+    count_launch(2);
 }
 
 void scale_by_rsqrt(double *x, long long n, const double *sumsq_dev)
