@@ -522,6 +522,9 @@ GEMM_SHAPES = {   # the c3 (chi=32, r=2) contraction shapes of SURVEY.md 8(a), p
     "a6_iv_Phi=P.Q": (32768, 1024, 4096),
     "a2_G1_Z=D.w": (1024, 2048, 32768),
     "a2_G2_Y=A.Z": (32768, 2048, 1024),
+    # the isometry operator S = K K_w^T applied to a 64-column block (a3; the 128 x 64 CTA tile of gemm_big.cu)
+    "a3_iso_t=K.w": (32768, 64, 1024),
+    "a3_iso_y=Kt.t": (1024, 64, 32768),
 }
 
 
