@@ -1407,17 +1407,24 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 }
             };
             Ten om = get_input(1 + i, n12, kk, cfg, "rz");
-            Ten Qi = ws_tensor("rz", {n12, kk}), SQ = ws_tensor("ry", {n12, kk});
+            Ten Qi = ws_tensor("rz", {n12, kk});
             S_op(om.p, Qi.p);
             orth(Qi.p, q == 0);
             for (int it = 0; it < q; ++it) {
-                S_op(Qi.p, SQ.p);
-                d2d(Qi.p, SQ.p, n12 * kk);
+                S_op(Qi.p, Qi.p);        // (the block is read by the first product only)
                 orth(Qi.p, it == q - 1);
             }
-            S_op(Qi.p, SQ.p);
+            // Ritz matrix H = Q^T S Q = (K Q)^T (K_w Q): a Gram matrix of t1 = K Q (weighted with R for the two
+            // middle chains) -- the product with K^T back to the pair space, half of an application of S, is
+            // not needed for it
             Ten Hm = ws_tensor("zy", {kk, kk});
-            contract(Qi, SQ, Hm);
+            contract(Kt.as("xpqta"), Ten::make(Qi.p, "pqz", {n1, n2, kk}), t1);
+            if (mid) {
+                contract(t1, Rm, t2);
+                contract(t1.as("xtbz"), t2.as("xtby"), Hm);
+            } else {
+                contract(t1.as("xtaz"), t1.as("xtay"), Hm);
+            }
             Ten Vt = ws_tensor("kz", {kk, kk});
             double *lam = ws_doubles(kk);
             if (fast && kk > 64) {
