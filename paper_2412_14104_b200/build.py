@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libtatrg.so")
-CU = ["gemm.cu", "gemm_big.cu", "gemm_p.cu", "gemm_tma.cu", "ts.cu", "rng.cu", "reduce.cu", "qr.cu", "jacobi.cu", "jacobi_small.cu", "gauge.cu", "chol.cu", "sq_iter.cu"]
+CU = ["gemm.cu", "gemm_big.cu", "gemm_p.cu", "gemm_tma.cu", "ts.cu", "rng.cu", "reduce.cu", "qr.cu", "jacobi.cu", "jacobi_small.cu", "gauge.cu", "chol.cu", "sq_iter.cu", "cholqr_fused.cu"]
 CPP = ["tensor.cpp", "step.cpp", "api.cpp"]
 GAUSS = os.path.join(ROOT, "seeded_inputs", "gauss.c")   # the shared seeded INPUT generator
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

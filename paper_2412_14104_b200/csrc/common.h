@@ -109,6 +109,9 @@ void tsqr(double *Y, long long m, int n, double *Rout);
 // receives the accumulated triangular factor.  The caller checks the flag when it next synchronises.
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
                   double *Rout);
+// cholqr_fused.cu : the same for blocks of <= 64 columns (1 or 2 passes) as one resident grid; false = not taken
+bool cholqr_fused(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
+                  double *Rout);
 // jacobi.cu : one-sided Jacobi SVD of `batch` column-major m x n matrices (ld = m), m >= n.
 // On exit G = U*diag(s) (columns orthogonal, sorted by decreasing norm), V (n x n, column
 // major) accumulates the rotations (G_in * V = G_out), s[n] = column norms (descending).

@@ -312,6 +312,7 @@ void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, i
                   double *Rout)
 {
     if (n < 1 || n > 256 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
+    if (cholqr_fused(Y, m, n, passes, shift_rel, flag_dev, ratio_dev, Rout)) return;   // <= 64 columns: one resident grid
     size_t mark = ws_mark();
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten T = ws_tensor("rd", {m, n});

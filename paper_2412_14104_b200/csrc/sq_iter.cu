@@ -303,19 +303,30 @@ __global__ void __launch_bounds__(SQ_NT, 1) sq_iter_kernel(const __grid_constant
                 __syncthreads();
             }
         }
-        // ---- R = L2^T L1^T of a two-pass step (R[i][j] = sum_k L2[k][i] L1[j][k]); one pass: R = L1^T
+        // ---- R = L2^T L1^T of a two-pass step (R[i][j] = sum_k L2[k][i] L1[j][k]); one pass: R = L1^T.  The factors
+        // are staged in shared memory first (from global memory this short loop of dependent loads took 100 us)
         if (blockIdx.x == 0 && (code & SQ_WANT_R) && p.Rout) {
-            const double *L1 = p.Lkeep, *L2 = p.Lkeep + SQ_B * SQ_B;
+            constexpr int LDS_ = SQ_B + 1;
+            double *L1s = &sm.Bs[0][0][0], *L2s = L1s + SQ_B * LDS_;   // 2 x 64 x 65 doubles fit into the staging ring
+            static_assert(2 * SQ_B * LDS_ <= SQ_NST * SQ_BK * SQ_LDB, "staging ring too small for the two factors");
+            __syncthreads();
+            for (int e = t; e < SQ_B * SQ_B; e += SQ_NT) {
+                L1s[(e >> 6) * LDS_ + (e & 63)] = __ldcg(p.Lkeep + e);
+                L2s[(e >> 6) * LDS_ + (e & 63)] = passes == 2 ? __ldcg(p.Lkeep + SQ_B * SQ_B + e) : 0.0;
+            }
+            __syncthreads();
             for (int e = t; e < SQ_B * SQ_B; e += SQ_NT) {
                 const int i = e / SQ_B, j = e % SQ_B;
                 double sum = 0.0;
                 if (passes == 2) {
-                    for (int k = i; k < SQ_B; ++k) sum = fma(__ldcg(L2 + k * SQ_B + i), __ldcg(L1 + j * SQ_B + k), sum);
+#pragma unroll 4
+                    for (int k = i; k < SQ_B; ++k) sum = fma(L2s[k * LDS_ + i], L1s[j * LDS_ + k], sum);
                 } else {
-                    sum = __ldcg(L1 + j * SQ_B + i);
+                    sum = L1s[j * LDS_ + i];
                 }
                 p.Rout[e] = sum;
             }
+            __syncthreads();
         }
         if (st + 1 < p.nsteps) grid_barrier(p.bar, target);
     }

@@ -345,6 +345,7 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
             int f;
             double r[4];
         } h;
+        trace_mark("rsvd: subspace iteration");
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&h.f, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaMemcpyAsync(h.r, ratio, 4 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
         TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
@@ -365,6 +366,7 @@ RsvdOut rsvd(F1 apply, F2 apply_t, const Ten &omega, long long rows, long long c
     double *V = ws_doubles((long long)ell * ell);
     double *s = ws_doubles(ell);
     jacobi_svd(Rb, ell, ell, V, s, 1, 0, 0, 0);   // R_B^T V = U diag(s)
+    trace_mark("rsvd: svd of the core");
     RsvdOut out;
     out.s_full = d2h(s, ell);
     out.s_dev = s;
@@ -481,6 +483,29 @@ struct SqChain {
         // a failed factorisation / Jacobi, or a block too ill conditioned for two Cholesky-QR passes
         return back->flag == 0 && back->ratio[0] > 1e-5 * back->ratio[1] && back->ratio[2] > 1e-5 * back->ratio[3];
     }
+    // The block was too ill conditioned for two Cholesky-QR passes while no factorisation failed (s_b / s_1 below
+    // ~1e-5: at the ordered fixed point the spectrum of F decays that fast): the same Ritz step with Householder
+    // TSQR, which needs no condition.  Q still spans the right subspace.  Synchronous on the chain's stream.
+    bool too_ill_conditioned() const
+    {
+        return back->flag == 0 && !(back->ratio[0] > 1e-5 * back->ratio[1] && back->ratio[2] > 1e-5 * back->ratio[3]) &&
+               back->ratio[0] > 0.0 && back->ratio[2] > 0.0;
+    }
+    void ritz_robust()
+    {
+        double *Rtmp = ws_doubles((long long)b * b);
+        tsqr(Q, N2, b, Rtmp);
+        mulFt(Q, Qt);
+        tsqr(Qt, N2, b, Rb);
+        if (b <= 64)
+            svd_small_async(Rb, b, b, V, sv, flag);
+        else
+            jacobi_svd(Rb, b, b, V, sv, 1, 0, 0, 0);
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(back->s, sv, b * sizeof(double), cudaMemcpyDeviceToHost, stream()));
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(stream()));
+        for (int i = 0; i < 4; ++i) back->ratio[i] = 1.0;   // orthonormal by construction
+    }
     // on the main stream, before any fork: the buffers of the two Cholesky factors
     void prep()
     {
@@ -544,6 +569,9 @@ struct SqChain {
     // iteration count from the measured decay rho = s_b / s_chi: rho^(2p+1) < 1e-13
     bool plan()
     {
+        if (getenv("TATRG_TRACE"))
+            fprintf(stderr, "tatrg-trace squeezer mu %d read-back: flag %d ratios %.2e/%.2e %.2e/%.2e s_1 %.3e s_chi %.3e s_b %.3e\n", mu, back->flag,
+                    back->ratio[0], back->ratio[1], back->ratio[2], back->ratio[3], back->s[0], back->s[chi - 1], back->s[b - 1]);
         if (!read_back()) return false;
         if (!(sh[chi - 1] > 1e-6 * sh[0])) return false;
         const double rho = sh[b - 1] / sh[chi - 1];
@@ -1267,6 +1295,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         fk.leave();
         for (int i = 0; i < na; ++i) {
             fk.sync(2 * i);
+            if (ch[act[i]].too_ill_conditioned()) {
+                fk.enter(2 * i);
+                ch[act[i]].ritz_robust();
+                fk.leave();
+            }
             ch[act[i]].ok = ch[act[i]].plan();
             if (getenv("TATRG_TRACE"))
                 fprintf(stderr, "tatrg-trace squeezer mu %d: hist %d done %d planned %d more %d ok %d\n", act[i], ch[act[i]].hist,
@@ -1285,6 +1318,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 const int mu = act[i];
                 if (ch[mu].more > 0) fk.sync(2 * i);
                 fk.enter(2 * i);
+                if (ch[mu].more > 0 && ch[mu].too_ill_conditioned()) ch[mu].ritz_robust();
                 if (ch[mu].phaseC()) {
                     gaps[1 + mu] = ch[mu].gap;
                     finish(mu, ch[mu].Mr, ch[mu].Nr, ch[mu].sh, ch[mu].k);
