@@ -167,7 +167,10 @@ double tatrg_probe_fp64_peak(int mode, int iters);
  *   idx = d0 + n0*(d1 + n1*(d2 + n2*d3))  ->  d0*s0 + d1*s1 + d2*s2 + d3*s3   (element offsets),
  * given as 7 int64 {n0, n1, n2, s0, s1, s2, s3} (radix <= 0 = unused level) in `maps` (host), in
  * the order am, ak, bk, bn, cm, cn, ab, bb, cb (63 values; the last three map the batch index).
- * A, B, C: device.  accumulate != 0: C += .  M, N >= 0, K >= 1, batch in 1..65535. */
+ * A, B, C: device.  accumulate: bit 0 set: C += ; bit 1 set: the caller promises B[k][n] = 0 for k > n (a
+ * triangular factor applied from the right, as in Q1 = T L^-T of the bond swap's Cholesky-QR; the zeros must be
+ * there: the hint only lets the kernel skip whole k tiles of them, the result is the same bit for bit).
+ * M, N >= 0, K >= 1, batch in 1..65535. */
 int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N, int K, int batch,
                       const int64_t *maps, double alpha, int accumulate);
 

@@ -325,16 +325,17 @@ def make_map(levels):
     return n + s
 
 
-def tensor_gemm(A, B, C, M, N, K, maps, batch=1, alpha=1.0, accumulate=False):
+def tensor_gemm(A, B, C, M, N, K, maps, batch=1, alpha=1.0, accumulate=False, tri_b=False):
     """maps: dict with keys am, ak, bk, bn, cm, cn (and optionally ab, bb, cb), each a list of
-    (size, stride) levels.  A, B, C: torch CUDA float64 tensors."""
+    (size, stride) levels.  A, B, C: torch CUDA float64 tensors.  tri_b: B[k][n] = 0 for k > n is promised
+    (bit 1 of the C entry's `accumulate` argument)."""
     _require_cuda()
     flat = []
     for key in ("am", "ak", "bk", "bn", "cm", "cn", "ab", "bb", "cb"):
         flat += make_map(maps.get(key, [(1, 0)]))
     arr = np.asarray(flat, dtype=np.int64)
     _check(lib().tatrg_tensor_gemm(A.data_ptr(), B.data_ptr(), C.data_ptr(), int(M), int(N), int(K),
-                                   int(batch), arr.ctypes.data, float(alpha), int(accumulate)))
+                                   int(batch), arr.ctypes.data, float(alpha), (1 if accumulate else 0) | (2 if tri_b else 0)))
 
 
 def fill_gauss(out, seed: int, step: int, which: int):

@@ -491,7 +491,8 @@ int tatrg_tensor_gemm(const double *A, const double *B, double *C, int M, int N,
         p.bb = map_from(maps + 49);
         p.cb = map_from(maps + 56);
         p.alpha = alpha;
-        p.accumulate = accumulate;
+        p.accumulate = accumulate & 1;
+        p.tri_b = (accumulate & 2) ? 1 : 0;
         p.a_kfast = llabs(p.ak.s0) < llabs(p.am.s0) || p.am.s0 == 0;
         p.b_kfast = llabs(p.bk.s0) < llabs(p.bn.s0) || p.bn.s0 == 0;
         tensor_gemm(p);

@@ -52,11 +52,19 @@ struct GemmParams {
     int ktiles_per_split;  // in units of BK
     double *partial;       // [ksplit][batch][M][N]
     int tiles_n;           // set by the launcher: column tiles of the chosen CTA tile
+    int tri_b;             // the caller promises B[k][n] = 0 for k > n (a triangular factor applied from the right):
+                           // the persistent tile skips the k tiles that hold only those zeros (same result bit for bit)
 };
 
-// algorithmic flops of one launch (a symmetric lower-only output counts its lower triangle)
+// algorithmic flops of one launch (a symmetric lower-only output counts its lower triangle, a triangular
+// B its non-zero part)
 inline double gemm_flops(const GemmParams &p)
 {
+    if (p.tri_b) {   // sum over n of min(K, n + 1)
+        const double full = p.N > p.K ? (double)(p.N - p.K) * p.K : 0.0;
+        const double t = (double)(p.N < p.K ? p.N : p.K);
+        return 2.0 * (double)p.M * (0.5 * t * (t + 1.0) + full) * p.batch;
+    }
     const double mn = p.lower_only ? 0.5 * p.M * ((double)p.N + 1.0) : (double)p.M * p.N;
     return 2.0 * mn * (double)p.K * p.batch;
 }

@@ -176,12 +176,20 @@ struct TileCoord {
 
 // per_z: live tiles of one (split, batch) slice.  lower_only (symmetric output, M = N): only the tiles on
 // or below the diagonal are enumerated, row by row: index l -> (tm, tn <= tm), l = tm (tm + 1) / 2 + tn
+template <bool TRI>
 __device__ __forceinline__ TileCoord decode_tile(const GemmParams &p, int tile, int tiles_m, int per_z)
 {
     TileCoord c;
     const int z = tile / per_z;
     const int r = tile - z * per_z;
-    if (p.lower_only) {
+    if (TRI) {
+        // triangular B: column tile tn costs tn + 1 units.  Tiles come in pairs (tn, tiles_n - 1 - tn) of one
+        // row band, every pair the same work; a CTA takes whole pairs (see next_tile in the kernel)
+        const int half = p.tiles_n >> 1, q = r >> 1;
+        const int tm = q / half, jp = q - tm * half;
+        c.m0 = tm * BM;
+        c.n0 = ((r & 1) ? p.tiles_n - 1 - jp : jp) * BN;
+    } else if (p.lower_only) {
         int tm = (int)((sqrtf(8.0f * (float)r + 1.0f) - 1.0f) * 0.5f);
         while ((tm + 1) * (tm + 2) / 2 <= r) ++tm;
         while (tm * (tm + 1) / 2 > r) --tm;
@@ -200,7 +208,7 @@ __device__ __forceinline__ TileCoord decode_tile(const GemmParams &p, int tile, 
     return c;
 }
 
-template <bool A_KF, bool B_KF, bool VEC>
+template <bool A_KF, bool B_KF, bool VEC, bool TRI>
 __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ GemmParams p, const int total_tiles, const int c_flags)
 {
     extern __shared__ __align__(128) double smem[];
@@ -259,20 +267,27 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
     Loader<B_KF, VEC> lb;
     la.init_thread(t);
     lb.init_thread(t);
-    int p_tile = blockIdx.x, p_kt = 0, p_nkt = 0, p_kbeg = 0, p_kend = 0;
+    int p_tile = 0, p_kt = 0, p_nkt = 0, p_kbeg = 0, p_kend = 0;
     unsigned p_it = 0;
-    auto k_range = [&](int split, int &kb, int &ke) {
+    auto k_range = [&](const TileCoord &c, int &kb, int &ke) {
         kb = 0;
         ke = p.K;
         if (p.ksplit > 1) {
-            kb = min(p.K, split * p.ktiles_per_split * 16);
+            kb = min(p.K, c.split * p.ktiles_per_split * 16);
             ke = min(p.K, kb + p.ktiles_per_split * 16);
         }
+        if (TRI) ke = min(ke, c.n0 + BN);   // B[k][n] = 0 for k > n
+    };
+    // tile walk of this CTA: blockIdx.x, + gridDim.x, ...; with a triangular B whole pairs (2 q, 2 q + 1)
+    const int tile_first = TRI ? 2 * (int)blockIdx.x : (int)blockIdx.x;
+    auto next_tile = [&](int tile) {
+        if (TRI) return (tile & 1) ? tile + 2 * (int)gridDim.x - 1 : tile + 1;
+        return tile + (int)gridDim.x;
     };
     auto prod_setup = [&]() {
         if (p_tile >= total_tiles) return;
-        const TileCoord c = decode_tile(p, p_tile, tiles_m, per_z);
-        k_range(c.split, p_kbeg, p_kend);
+        const TileCoord c = decode_tile<TRI>(p, p_tile, tiles_m, per_z);
+        k_range(c, p_kbeg, p_kend);
         p_nkt = (p_kend - p_kbeg + BK - 1) / BK;
         p_kt = 0;
         la.init(p.A + map_off(p.ab, c.bz), p.am, c.m0, p.M, t);
@@ -287,20 +302,21 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
         mbar_arrive_on_cp_async(full0 + 8 * slot);
         ++p_it;
         if (++p_kt == p_nkt) {
-            p_tile += gridDim.x;
+            p_tile = next_tile(p_tile);
             prod_setup();
         }
     };
+    p_tile = tile_first;
     prod_setup();
 #pragma unroll 1
     for (int s = 0; s < STAGES - 1; ++s) produce();
 
     // ---- consumer
     unsigned it = 0;
-    for (int c_tile = blockIdx.x; c_tile < total_tiles; c_tile += gridDim.x) {
-        const TileCoord tc = decode_tile(p, c_tile, tiles_m, per_z);
+    for (int c_tile = tile_first; c_tile < total_tiles; c_tile = next_tile(c_tile)) {
+        const TileCoord tc = decode_tile<TRI>(p, c_tile, tiles_m, per_z);
         int kb, ke;
-        k_range(tc.split, kb, ke);
+        k_range(tc, kb, ke);
         const int nkt = (ke - kb + BK - 1) / BK;
 #pragma unroll 1
         for (int kt = 0; kt < nkt; ++kt, ++it) {
@@ -451,30 +467,32 @@ bool even(long long s) { return (s & 1LL) == 0; }
 bool upper_even(const Map4 &m) { return even(m.s1) && even(m.s2) && even(m.s3); }
 bool all_even(const Map4 &m) { return even(m.s0) && upper_even(m); }
 
-template <bool A_KF, bool B_KF, bool VEC>
+template <bool A_KF, bool B_KF, bool VEC, bool TRI>
 void launch_p(const GemmParams &p_in, int num_sms)
 {
     constexpr size_t smem = (size_t)STAGES * 2 * TILE * sizeof(double);
     static bool attr_done = false;
-    auto kern = tgemm_p_kernel<A_KF, B_KF, VEC>;
+    auto kern = tgemm_p_kernel<A_KF, B_KF, VEC, TRI>;
     if (!attr_done) {
         TATRG_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
     GemmParams p = p_in;
+    const double flops = gemm_flops(p);
     p.tiles_n = (p.N + BN - 1) / BN;
     const long long tm = (p.M + BM - 1) / BM;
     if (p.lower_only && tm != p.tiles_n) fail(-22, "tensor_gemm: a symmetric (lower_only) output needs M = N");
+    p.tri_b = TRI ? 1 : 0;
     const long long tiles = (p.lower_only ? tm * (tm + 1) / 2 : tm * p.tiles_n) * p.batch * (p.ksplit > 1 ? p.ksplit : 1);
-    if (tiles > 0x7fffffffLL) fail(-22, "tensor_gemm: too many tiles");
+    if (tiles > 0x3fffffffLL) fail(-22, "tensor_gemm: too many tiles");
     // while independent chains of small kernels run beside the step's big products, some SMs are left to them
-    const unsigned grid = (unsigned)std::min<long long>(tiles, std::max(1, num_sms - ctx().sm_reserve));
+    const unsigned grid = (unsigned)std::min<long long>(TRI ? tiles / 2 : tiles, std::max(1, num_sms - ctx().sm_reserve));
     // 16-byte stores of column pairs: bit 0 for C through its maps, bit 1 for the split-K partial sums
     int c_flags = 0;
     if (((uintptr_t)p.C & 15) == 0 && p.cn.s0 == 1 && even_or_inf(p.cn.n0) && upper_even(p.cn) && all_even(p.cm) && all_even(p.cb))
         c_flags |= 1;
     if ((p.N & 1) == 0 && ((uintptr_t)p.partial & 15) == 0) c_flags |= 2;
-    const int slot = prof_begin(gemm_flops(p), 1);
+    const int slot = prof_begin(flops, 1);
     kern<<<grid, NT, smem, stream()>>>(p, (int)tiles, c_flags);
     prof_end(slot);
     TATRG_LAUNCH_CHECK();
@@ -519,16 +537,26 @@ bool tensor_gemm_persistent(const GemmParams &p, int num_sms)
     const bool vb = bkf ? vec_ok(p.B, p.bk, p.bn, p.bb) : vec_ok(p.B, p.bn, p.bk, p.bb);
     // 16-byte copies along k need the k ranges of the split-K parts to start at even k: they do (units of 16)
     const bool vec = va && vb;
+    // the triangular-B hint is taken (16-byte copy variants only) when the column tiles pair up; else the zeros
+    // are multiplied as usual
+    const bool tri = p.tri_b && vec && !p.lower_only && p.ksplit <= 1 && (((p.N + BN - 1) / BN) & 1) == 0;
+    if (tri) {
+        if (akf)
+            bkf ? launch_p<true, true, true, true>(p, num_sms) : launch_p<true, false, true, true>(p, num_sms);
+        else
+            bkf ? launch_p<false, true, true, true>(p, num_sms) : launch_p<false, false, true, true>(p, num_sms);
+        return true;
+    }
     if (akf) {
         if (bkf)
-            vec ? launch_p<true, true, true>(p, num_sms) : launch_p<true, true, false>(p, num_sms);
+            vec ? launch_p<true, true, true, false>(p, num_sms) : launch_p<true, true, false, false>(p, num_sms);
         else
-            vec ? launch_p<true, false, true>(p, num_sms) : launch_p<true, false, false>(p, num_sms);
+            vec ? launch_p<true, false, true, false>(p, num_sms) : launch_p<true, false, false, false>(p, num_sms);
     } else {
         if (bkf)
-            vec ? launch_p<false, true, true>(p, num_sms) : launch_p<false, true, false>(p, num_sms);
+            vec ? launch_p<false, true, true, false>(p, num_sms) : launch_p<false, true, false, false>(p, num_sms);
         else
-            vec ? launch_p<false, false, true>(p, num_sms) : launch_p<false, false, false>(p, num_sms);
+            vec ? launch_p<false, false, true, false>(p, num_sms) : launch_p<false, false, false, false>(p, num_sms);
     }
     return true;
 }

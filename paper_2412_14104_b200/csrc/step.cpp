@@ -688,7 +688,7 @@ struct OrthoChain {
         d2d(G1.p, G1copy.p, nk * nk);
         TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));   // the failed attempt raised it
         if (!cholesky_lower(G1.p, (int)nk, 1e-13, L1inv.p)) return false;
-        contract(T.as("cpqtb"), L1inv, o.Q1);
+        contract(T.as("cpqtb"), L1inv, o.Q1, 1.0, false, false, true);
         contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
         max_dev_identity(G2.p, (int)nk, dev);
         err = d2h(dev, 1)[0];
@@ -697,7 +697,8 @@ struct OrthoChain {
     }
     void basis()                                                                                 // main
     {
-        contract(T.as("cpqtb"), L1inv, o.Q1);                          // Q1 = T2 L1^-T
+        // Q1 = T2 L1^-T: L1inv[k][(c,b)] = 0 for (c,b) > k, the k tiles of zeros are skipped (tri_b)
+        contract(T.as("cpqtb"), L1inv, o.Q1, 1.0, false, false, true);
         contract(o.Q1.as("pqtk"), o.Q1.as("pqtl"), G2, 1.0, false, true);
         max_dev_identity(G2.p, (int)nk, dev);
         TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
@@ -724,7 +725,7 @@ struct OrthoChain {
         {
             size_t mk = ws_mark();
             Ten Q2 = ws_tensor("pqtl", {o.Q1.legs[0].n, o.Q1.legs[1].n, o.Q1.legs[2].n, nk});
-            contract(o.Q1.as("pqtk"), L2inv.as("lk"), Q2);
+            contract(o.Q1.as("pqtk"), L2inv.as("lk"), Q2, 1.0, false, false, true);
             d2d(o.Q1.p, Q2.p, Q2.size());
             ws_release(mk);
         }

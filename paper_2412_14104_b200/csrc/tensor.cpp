@@ -115,7 +115,7 @@ long long total(const std::vector<GLeg> &g)
 
 }  // namespace
 
-void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accumulate, bool lower_only)
+void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accumulate, bool lower_only, bool tri_b)
 {
     std::vector<GLeg> gb, gm, gn, gk;  // strides: batch (A,B,C); m (A,C); n (B,C); k (A,B)
     std::string seen;
@@ -173,6 +173,7 @@ void contract(const Ten &A, const Ten &B, const Ten &C, double alpha, bool accum
     p.alpha = alpha;
     p.accumulate = accumulate ? 1 : 0;
     p.lower_only = (lower_only && M == N) ? 1 : 0;
+    p.tri_b = tri_b ? 1 : 0;
     // loader order: walk whichever index has the smaller leading stride in that operand
     long long am0 = gm.empty() ? (1LL << 60) : gm[0].s[0];
     long long ak0 = gk.empty() ? (1LL << 60) : gk[0].s[0];

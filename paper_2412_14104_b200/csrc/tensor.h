@@ -36,7 +36,10 @@ Ten ws_tensor(const char *names, std::initializer_list<long long> dims);
 // Legs in A, B and C: batch; A and C: rows; B and C: columns.  Any other pattern is an error.
 // lower_only: C is a symmetric matrix (rows and columns enumerate the same index in the same order);
 // only its lower triangle is guaranteed to be written.
+// tri_b: the caller promises that B, as a (summed index) x (column index) matrix in the order of the legs' memory
+// strides in A resp. B, vanishes for summed index > column index (a triangular factor applied from the
+// right): the k tiles of zeros are skipped.
 void contract(const Ten &A, const Ten &B, const Ten &C, double alpha = 1.0, bool accumulate = false,
-              bool lower_only = false);
+              bool lower_only = false, bool tri_b = false);
 
 }  // namespace tatrg

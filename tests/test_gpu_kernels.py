@@ -396,3 +396,36 @@ def test_tensor_gemm_tma_producer_matches(tt):
         ref = -0.5 * (A @ B) + C0
         assert np.abs(res[1] - ref).max() <= 4e-11 * np.sqrt(K), (M, N, K)
         assert np.abs(res[1] - res[0]).max() <= 1e-12 * np.sqrt(K), (M, N, K)
+
+
+@pytest.mark.parametrize("b_kfast", [False, True])
+def test_tensor_gemm_triangular_b_hint(tt, b_kfast):
+    """tri_b (bit 1 of tatrg_tensor_gemm's `accumulate`): B[k][n] = 0 for k > n, as in Q1 = T L^-T of the bond
+    swap's Cholesky-QR.  The persistent tile skips the k tiles of zeros and walks the column tiles in
+    pairs of equal work; the result is the same bit for bit as without the hint, and equal to numpy's.  Cases: an
+    even number of column tiles (hint taken) with ragged M, K < N, K > N, batch 2; an odd number of column tiles
+    and a split-K shape (hint dropped)."""
+    import torch
+    rng = np.random.default_rng(11 + b_kfast)
+    for (M, N, K, batch) in ((4100, 1024, 1024, 1), (3000, 768, 512, 2), (2500, 1000, 1200, 1), (4096, 640, 640, 1),
+                             (256, 256, 20000, 1)):
+        A = rng.standard_normal((batch, M, K))
+        B = np.triu(rng.standard_normal((batch, K, N)))          # zero for k > n
+        if b_kfast:
+            bufB = np.ascontiguousarray(B.transpose(0, 2, 1))
+            bk, bn = [(K, 1)], [(N, K)]
+        else:
+            bufB = B
+            bk, bn = [(K, N)], [(N, 1)]
+        C0 = rng.standard_normal((batch, M, N))
+        maps = dict(am=[(M, K)], ak=[(K, 1)], bk=bk, bn=bn, cm=[(M, N)], cn=[(N, 1)],
+                    ab=[(batch, M * K)], bb=[(batch, K * N)], cb=[(batch, M * N)])
+        res = []
+        for hint in (False, True):
+            dA, dB, dC = _dev(A), _dev(bufB), _dev(C0)
+            tt.tensor_gemm(dA, dB, dC, M, N, K, maps, batch=batch, alpha=0.75, accumulate=True, tri_b=hint)
+            torch.cuda.synchronize()
+            res.append(dC.cpu().numpy())
+        ref = 0.75 * np.einsum("bmk,bkn->bmn", A, B) + C0
+        assert np.abs(res[1] - ref).max() <= 4e-11 * np.sqrt(K), (M, N, K, batch)
+        assert np.array_equal(res[0], res[1]), (M, N, K, batch)
