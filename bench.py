@@ -525,6 +525,8 @@ GEMM_SHAPES = {   # the c3 (chi=32, r=2) contraction shapes of SURVEY.md 8(a), p
     # the isometry operator S = K K_w^T applied to a 64-column block (a3; the 128 x 64 CTA tile of gemm_big.cu)
     "a3_iso_t=K.w": (32768, 64, 1024),
     "a3_iso_y=Kt.t": (1024, 64, 32768),
+    # Q1 = T L^-T of the bond swap's Cholesky-QR (a2): B upper triangular, the k tiles of zeros skipped (tri_b)
+    "a2_Q1=T.LinvT_tri": (32768, 1024, 1024),
 }
 
 
@@ -547,18 +549,22 @@ def run_gemm_micro(args):
             A = torch.randn(M, K, dtype=torch.float64, device="cuda")
             B = torch.randn(K, N, dtype=torch.float64, device="cuda")
             C = torch.empty(M, N, dtype=torch.float64, device="cuda")
+            tri = name.endswith("_tri")
+            if tri:
+                B = torch.triu(B).contiguous()
         maps = dict(am=[(M, K)], ak=[(K, 1)], bk=[(K, N)], bn=[(N, 1)], cm=[(M, N)], cn=[(N, 1)])
         for _ in range(3):
-            tt.tensor_gemm(A, B, C, M, N, K, maps)
+            tt.tensor_gemm(A, B, C, M, N, K, maps, tri_b=tri)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         reps = 10
         e0.record(stream)
         for _ in range(reps):
-            tt.tensor_gemm(A, B, C, M, N, K, maps)
+            tt.tensor_gemm(A, B, C, M, N, K, maps, tri_b=tri)
         e1.record(stream)
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / reps
-        out[name] = {"M": M, "N": N, "K": K, "ms": ms, "tflops": 2.0 * M * N * K / (ms * 1e-3) / 1e12}
+        flops = 2.0 * M * (N * (N + 1) // 2 if tri else N * K)   # tri (K = N): the non-zero part of B only
+        out[name] = {"M": M, "N": N, "K": K, "ms": ms, "tflops": flops / (ms * 1e-3) / 1e12}
         del A, B, C
     out["probe_dmma_tflops"] = tt.probe_fp64_peak(0, 1 << 14)
     print(json.dumps({"gemm_micro": out}), flush=True)

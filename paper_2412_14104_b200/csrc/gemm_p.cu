@@ -135,11 +135,23 @@ struct Loader {
         }
     }
 
-    __device__ __forceinline__ void load(unsigned stage_addr, const Map4 &mk, int k0, int k_end) const
+    // kshift >= 0: the summed index is a composite of two legs, the faster one a power of two (2^kshift): shift and
+    // mask instead of the integer divisions of map_off, which otherwise sit in front of every k tile's copies (2 % of
+    // the kernel's time on the contraction shapes, whose summed index is such a composite).  (The same treatment of
+    // the free-index and output maps, evaluated once per output tile, measured no gain.)
+    __device__ __forceinline__ void load(unsigned stage_addr, const Map4 &mk, int kshift, int k0, int k_end) const
     {
         const int k_left = k_end - (k0 + kl);
         const unsigned kk = (unsigned)(k0 + kl);
-        const long long ko = k_left <= 0 ? 0 : (mk.n0 == TATRG_RADIX_INF ? (long long)kk * mk.s0 : map_off(mk, kk));
+        long long ko = 0;
+        if (k_left > 0) {
+            if (mk.n0 == TATRG_RADIX_INF)
+                ko = (long long)kk * mk.s0;
+            else if (kshift >= 0)
+                ko = (long long)(kk & (mk.n0 - 1u)) * mk.s0 + (long long)(kk >> kshift) * mk.s1;
+            else
+                ko = map_off(mk, kk);
+        }
         const unsigned dst0 = stage_addr + soff0;
         if (interior && k_left >= (KF && VEC ? 2 : 1)) {
             const double *src = base + ko;
@@ -263,6 +275,10 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
         for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     // ---- producer cursor
+    auto pow2_shift = [](const Map4 &m) {
+        return (m.n0 != TATRG_RADIX_INF && m.n1 == TATRG_RADIX_INF && (m.n0 & (m.n0 - 1u)) == 0u) ? __ffs((int)m.n0) - 1 : -1;
+    };
+    const int a_kshift = pow2_shift(p.ak), b_kshift = pow2_shift(p.bk);
     Loader<A_KF, VEC> la;
     Loader<B_KF, VEC> lb;
     la.init_thread(t);
@@ -297,8 +313,8 @@ __global__ void __launch_bounds__(NT, 1) tgemm_p_kernel(const __grid_constant__ 
         if (p_tile >= total_tiles) return;
         const unsigned slot = p_it % STAGES, use = p_it / STAGES;
         if (use >= 1) mbar_wait(empty0 + 8 * slot, (use - 1) & 1u);
-        la.load(As + slot * (TILE * 8), p.ak, p_kbeg + p_kt * BK, p_kend);
-        lb.load(Bs + slot * (TILE * 8), p.bk, p_kbeg + p_kt * BK, p_kend);
+        la.load(As + slot * (TILE * 8), p.ak, a_kshift, p_kbeg + p_kt * BK, p_kend);
+        lb.load(Bs + slot * (TILE * 8), p.bk, b_kshift, p_kbeg + p_kt * BK, p_kend);
         mbar_arrive_on_cp_async(full0 + 8 * slot);
         ++p_it;
         if (++p_kt == p_nkt) {

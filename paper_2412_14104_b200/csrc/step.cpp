@@ -1210,6 +1210,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ms[mu] = ws_tensor("uok", {nn[mu], nn[mu], std::min<long long>(chi, N2)});
         Ns[mu] = ws_tensor("kuo", {std::min<long long>(chi, N2), nn[mu], nn[mu]});
     }
+    // M^(4) once more as [t, w, T]: step (i) of Eq. 13 then writes E M^(4) with the legs summed in (ii) last
+    Ten M3t = ws_tensor("twT", {n3, std::min<long long>(chi, n3 * n3), n3});
     bool done[3] = {false, false, false};
     // gauge (reading G12) P = N G_ref, then M W and W^T N into the step's squeezer buffers
     auto finish = [&](int mu, const Ten &Mr, const Ten &Nr, const std::vector<double> &sh, int k) {
@@ -1224,6 +1226,13 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ns[mu] = Ten::make(Ns[mu].p, "kuo", {k, nn[mu], nn[mu]});
         contract(Mr.as("na"), Wq, Ten::make(Ms[mu].p, "nb", {N2, k}));
         contract(Wq, Nr.as("an"), Ten::make(Ns[mu].p, "bn", {k, N2}));
+        if (mu == 2) {
+            M3t = Ten::make(M3t.p, "twT", {nn[2], k, nn[2]});
+            Ten Mr3;   // Mr[(t, T), a] with its row index split into the two legs
+            Mr3.p = Mr.p;
+            Mr3.legs = {Leg{'t', nn[2], nn[2] * Mr.legs[0].stride}, Leg{'T', nn[2], Mr.legs[0].stride}, Leg{'a', Mr.legs[1].n, Mr.legs[1].stride}};
+            contract(Mr3, Wq.as("aw"), M3t);
+        }
     };
     // The subspace-iteration squeezers of the directions `mus` as concurrent chains (large legs only; the
     // others, and chains that give up, are left to squeeze_dense).  main_work (may be empty) is enqueued on
@@ -1674,16 +1683,18 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         const double chains = 4.0 * std::max<double>(64 << 20, 6.0 * 8.0 * (double)n1 * n1 * n1 * n1);
         const double need = 8.0 * ((double)n0 * kd * a * n3 * m3 + 2.0 * (double)n0 * kd * m3 * kd * gs) + chains + (256 << 20);
         if (xc == n0 && (double)(c.hi - c.lo) > need) {
-            Ten EM = ws_tensor("xkaTw", {n0, kd, a, n3, m3});
+            // E M^(4) is stored with the legs summed in (ii) last, [x, k, w, (a, T)]: the A operand of (ii) is then
+            // a plain row-major 65536 x 1024 matrix (summed index contiguous), the faster operand layout
+            Ten EM = ws_tensor("xkwaT", {n0, kd, m3, a, n3});
             for (int side = 0; side < 2; ++side) Pt_pre[side] = ws_tensor("xkwlg", {n0, kd, m3, kd, gs});
             auto side0 = [&]() {
-                contract(E.as("xkta"), Ms[2].as("tTw"), EM);
+                contract(E.as("xkta"), M3t, EM);
                 contract(EM, F.as("alTg"), Pt_pre[0]);
             };
             auto side1 = [&]() {
                 // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
-                contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkatw"));
-                contract(EM.as("xkatw"), G.as("altg"), Pt_pre[1]);   // Pt[x, kD, w, kY, g]
+                contract(H.as("xkTa"), Ns[2].as("wtT"), EM.as("xkwat"));
+                contract(EM.as("xkwat"), G.as("altg"), Pt_pre[1]);   // Pt[x, kD, w, kY, g]
             };
             // (handing the second side to the main stream only after the chains have ended, so that it gets every
             // SM, measured slower: the chains outlast the first side and the main stream idles meanwhile)
@@ -1738,7 +1749,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         // P (r^2 chi^5) stay below ~8 GB (one slab = the whole tensor up to chi ~ 40)
         const double per_x = 8.0 * ((double)kd * a * n3 * m3 + (double)kd * m3 * kd * gs);
         const long long xc = std::max<long long>(1, std::min<long long>(n0, (long long)(8.0e9 / per_x)));
-        Ten EM = ws_tensor("xkaTw", {xc, kd, a, n3, m3});
+        Ten EM = ws_tensor("xkwaT", {xc, kd, m3, a, n3});
         Ten Pt = ws_tensor("xkwlg", {xc, kd, m3, kd, gs});
         auto slab = [](Ten t, long long x0, long long cnt) {   // legs[0] is the direction-0 leg
             t.p += x0 * t.legs[0].stride;
@@ -1749,13 +1760,13 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             const long long cnt = std::min(xc, n0 - x0);
             Ten EMs = slab(EM, 0, cnt), Pts = slab(Pt, 0, cnt), outs = slab(out, x0, cnt);
             if (side == 0) {
-                contract(slab(E.as("xkta"), x0, cnt), Ms[2].as("tTw"), EMs);
+                contract(slab(E.as("xkta"), x0, cnt), M3t, EMs);
                 contract(EMs, F.as("alTg"), Pts);
                 contract(Pts, Qt, outs);
             } else {
                 // H is the lower site: its lone leg is the "lower" index of N3[w, upper, lower]
-                contract(slab(H.as("xkTa"), x0, cnt), Ns[2].as("wtT"), EMs.as("xkatw"));
-                contract(EMs.as("xkatw"), G.as("altg"), Pts);   // Pt[x, kD, w, kY, g]
+                contract(slab(H.as("xkTa"), x0, cnt), Ns[2].as("wtT"), EMs.as("xkwat"));
+                contract(EMs.as("xkwat"), G.as("altg"), Pts);   // Pt[x, kD, w, kY, g]
                 contract(Pts.as("xlwkg"), Qt, outs);
             }
         }

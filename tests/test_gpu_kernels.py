@@ -429,3 +429,26 @@ def test_tensor_gemm_triangular_b_hint(tt, b_kfast):
         ref = 0.75 * np.einsum("bmk,bkn->bmn", A, B) + C0
         assert np.abs(res[1] - ref).max() <= 4e-11 * np.sqrt(K), (M, N, K, batch)
         assert np.array_equal(res[0], res[1]), (M, N, K, batch)
+
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 32, 32, 32, 32), (6, 10, 6, 24, 36, 30, 36), (4, 16, 8, 32, 30, 32, 36)])
+def test_tensor_gemm_persistent_tile_composite_maps(tt, dims):
+    """Step (ii) of Eq. 13 in miniature, P[x,k,w,l,g] = sum_{a,T} EM[x,k,a,T,w] F[a,l,T,g], through the
+    persistent tile: rows, columns, the summed index and the output are all composites of two or three tensor legs.
+    A power-of-two faster leg of the summed index takes the shift-and-mask evaluation of its map (gemm_p.cu:
+    Loader::load), other sizes the mixed-radix divisions; the third case mixes both kinds of leg sizes."""
+    import torch
+    x, k, a, T, w, l, g = dims
+    rng = np.random.default_rng(sum(dims))
+    EM, F = rng.standard_normal((x, k, a, T, w)), rng.standard_normal((a, l, T, g))
+    M, N, K = x * k * w, l * g, a * T
+    maps = dict(am=[(w, 1), (k, a * T * w), (x, k * a * T * w)], ak=[(T, w), (a, T * w)],
+                bk=[(T, g), (a, l * T * g)], bn=[(g, 1), (l, T * g)],
+                cm=[(w, l * g), (k, w * l * g), (x, k * w * l * g)], cn=[(g, 1), (l, g)])
+    dA, dB = _dev(EM), _dev(F)
+    dC = torch.zeros(x * k * w * l * g, dtype=torch.float64, device="cuda")
+    tt.tensor_gemm(dA, dB, dC, M, N, K, maps)
+    torch.cuda.synchronize()
+    ref = np.einsum("xkaTw,alTg->xkwlg", EM, F)
+    err = np.abs(dC.cpu().numpy().reshape(ref.shape) - ref).max()
+    assert err <= 4e-11 * np.sqrt(K), (dims, err)
