@@ -33,6 +33,24 @@ __host__ __device__ __forceinline__ long long map_off(const Map4 &m, unsigned i)
     return off;
 }
 
+// the same for the summed index in front of a k tile's copies: no integer division when it is one leg, or two
+// legs with a power-of-two faster one (the common cases; the divisions cost 2 % of the persistent GEMM's time on
+// the contraction shapes and more in the small tiles, whose threads evaluate the map up to 32 times per k tile)
+__host__ __device__ __forceinline__ long long map_off_k(const Map4 &m, unsigned i)
+{
+    if (m.n0 == TATRG_RADIX_INF) return (long long)i * m.s0;
+    if (m.n1 == TATRG_RADIX_INF && (m.n0 & (m.n0 - 1u)) == 0u) {
+#ifdef __CUDA_ARCH__
+        const int sh = __ffs((int)m.n0) - 1;
+#else
+        int sh = 0;
+        while ((1u << sh) < m.n0) ++sh;
+#endif
+        return (long long)(i & (m.n0 - 1u)) * m.s0 + (long long)(i >> sh) * m.s1;
+    }
+    return map_off(m, i);
+}
+
 inline Map4 map1(long long s) { return Map4{TATRG_RADIX_INF, TATRG_RADIX_INF, TATRG_RADIX_INF, 0, s, 0, 0, 0}; }
 
 // C[b][cm(m)+cn(n)] (+)= alpha * sum_k A[b][am(m)+ak(k)] * B[b][bk(k)+bn(n)]

@@ -126,7 +126,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
         if (p.a_kfast) {
             int kl = t % BK;
             bool kok = (k0 + kl) < p.K;
-            long long ko = kok ? map_off(p.ak, k0 + kl) : 0;
+            long long ko = kok ? map_off_k(p.ak, k0 + kl) : 0;
 #pragma unroll
             for (int u = 0; u < A_PT; ++u) {
                 int ml = t / BK + (NT / BK) * u;
@@ -139,14 +139,14 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
             for (int u = 0; u < A_PT; ++u) {
                 int kl = t / BM + (NT / BM) * u;
                 bool ok = a_base_ok && (k0 + kl) < p.K;
-                long long ko = ok ? map_off(p.ak, k0 + kl) : 0;
+                long long ko = ok ? map_off_k(p.ak, k0 + kl) : 0;
                 cp_async8(as + kl * LDA + ml, ok ? Ab + a_base + ko : p.A, ok);
             }
         }
         if (p.b_kfast) {
             int kl = t % BK;
             bool kok = (k0 + kl) < p.K;
-            long long ko = kok ? map_off(p.bk, k0 + kl) : 0;
+            long long ko = kok ? map_off_k(p.bk, k0 + kl) : 0;
 #pragma unroll
             for (int u = 0; u < B_PT; ++u) {
                 int nl = t / BK + (NT / BK) * u;
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32)
             for (int u = 0; u < B_PT; ++u) {
                 int kl = t / BN + (NT / BN) * u;
                 bool ok = b_base_ok && (k0 + kl) < p.K;
-                long long ko = ok ? map_off(p.bk, k0 + kl) : 0;
+                long long ko = ok ? map_off_k(p.bk, k0 + kl) : 0;
                 cp_async8(bs + kl * LDB + nl, ok ? Bb + b_base + ko : p.B, ok);
             }
         }

@@ -125,18 +125,7 @@ struct TileLoader {
     __device__ __forceinline__ void load(double *stage, const Map4 &mk, int k0, int K) const
     {
         const int k_left = K - (k0 + kl);
-        // no integer division in front of the copies when the summed index is one leg, or two legs with a
-        // power-of-two faster one (as in gemm_p.cu)
-        long long ko = 0;
-        if (k_left > 0) {
-            const unsigned kk = (unsigned)(k0 + kl);
-            if (mk.n0 == TATRG_RADIX_INF)
-                ko = (long long)kk * mk.s0;
-            else if (mk.n1 == TATRG_RADIX_INF && (mk.n0 & (mk.n0 - 1u)) == 0u)
-                ko = (long long)(kk & (mk.n0 - 1u)) * mk.s0 + (long long)(kk >> (__ffs((int)mk.n0) - 1)) * mk.s1;
-            else
-                ko = map_off(mk, kk);
-        }
+        const long long ko = k_left > 0 ? map_off_k(mk, (unsigned)(k0 + kl)) : 0;   // no integer division in the common cases
 #pragma unroll
         for (int j = 0; j < PER; ++j) {
             int n;   // valid elements of this copy
