@@ -133,8 +133,9 @@ void tsqr(double *Y, long long m, int n, double *Rout);
 // C = L L^T, Y <- Y L^-T}; no host synchronisation.  A failed factorisation raises *flag_dev (sticky);
 // ratio_dev (optional) receives min / max of the first pass's diag(L); Rout (optional, n x n row-major)
 // receives the accumulated triangular factor.  The caller checks the flag when it next synchronises.
+// src (optional): the block is read from there and Q written to Y (src itself is left alone).
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
-                  double *Rout);
+                  double *Rout, const double *src = nullptr);
 // cholqr_fused.cu : the same for blocks of <= 64 columns (1 or 2 passes) as one resident grid; false = not taken
 bool cholqr_fused(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
                   double *Rout);

@@ -309,21 +309,30 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
 }
 
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
-                  double *Rout)
+                  double *Rout, const double *src)
 {
     if (n < 1 || n > 256 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
-    if (cholqr_fused(Y, m, n, passes, shift_rel, flag_dev, ratio_dev, Rout)) return;   // <= 64 columns: one resident grid
+    if (src == Y) src = nullptr;
+    // <= 64 columns: one resident grid (in place)
+    if (src && !(n <= 32 && m >= 16384) && n <= 64) {
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(Y, src, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, stream()));
+        src = nullptr;
+    }
+    if (cholqr_fused(Y, m, n, passes, shift_rel, flag_dev, ratio_dev, Rout)) return;
     size_t mark = ws_mark();
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten T = ws_tensor("rd", {m, n});
     Ten C[3];
-    Ten cur = Ym, nxt = T;
+    // the passes alternate between Y and T such that the last one lands in Y; with a separate source the first
+    // pass reads it directly (no copy of the block)
+    Ten cur = src ? Ten::make(const_cast<double *>(src), "rc", {m, n}) : Ym;
     for (int p = 0; p < passes; ++p) {
+        Ten nxt = src ? (((passes - 1 - p) & 1) ? T : Ym) : (cur.p == Y ? T : Ym);
         C[p] = ws_tensor("cd", {n, n});
         contract(cur.as("rc"), cur.as("rd"), C[p]);
         Ten Linv = chol_inv(C[p], n, p == 0 ? shift_rel : 0.0, flag_dev, p == 0 ? ratio_dev : nullptr);
         contract(cur.as("rc"), Linv, nxt.as("rd"));       // Q[r,d] = sum_c Y[r,c] Linv[d,c]
-        std::swap(cur, nxt);
+        cur = nxt;
     }
     if (cur.p != Y) TATRG_CUDA_CHECK(cudaMemcpyAsync(Y, cur.p, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, stream()));
     if (Rout) {

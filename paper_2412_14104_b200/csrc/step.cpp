@@ -1029,11 +1029,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             for (int i = 0; i < 2; ++i) {
                 fk.enter(i);
                 QrBack *bk = reinterpret_cast<QrBack *>(fk.pinned(i));
-                d2d(Yq[i], src[i], R * g0);
                 int *flag = (int *)ws_alloc(sizeof(int));
                 double *ratio = ws_doubles(2);
                 TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
-                cholqr_async(Yq[i], R, g0, 2, 0.0, flag, ratio, Rq[i]);
+                cholqr_async(Yq[i], R, g0, 2, 0.0, flag, ratio, Rq[i], src[i]);   // reads Phi / Psi, writes Q
                 TATRG_CUDA_CHECK(cudaMemcpyAsync(&bk->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
                 TATRG_CUDA_CHECK(cudaMemcpyAsync(bk->ratio, ratio, 2 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
                 fk.leave();
