@@ -134,8 +134,10 @@ void tsqr(double *Y, long long m, int n, double *Rout);
 // ratio_dev (optional) receives min / max of the first pass's diag(L); Rout (optional, n x n row-major)
 // receives the accumulated triangular factor.  The caller checks the flag when it next synchronises.
 // src (optional): the block is read from there and Q written to Y (src itself is left alone).
+// last_Linv (optional, n x n row-major; passes >= 2): the last pass's factor is not applied but returned, Y then
+// holds Q' with Q = Q' last_Linv^T (the identity when the block took a route that applies every pass).
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
-                  double *Rout, const double *src = nullptr);
+                  double *Rout, const double *src = nullptr, double *last_Linv = nullptr);
 // cholqr_fused.cu : the same for blocks of <= 64 columns (1 or 2 passes) as one resident grid; false = not taken
 bool cholqr_fused(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
                   double *Rout);

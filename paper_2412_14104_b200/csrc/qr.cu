@@ -309,7 +309,7 @@ bool cholqr2(double *Y, long long m, int n, double *Rout)
 }
 
 void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, int *flag_dev, double *ratio_dev,
-                  double *Rout, const double *src)
+                  double *Rout, const double *src, double *last_Linv)
 {
     if (n < 1 || n > 256 || passes < 1 || passes > 3) fail(-22, "cholqr_async: n = %d, passes = %d not supported", n, passes);
     if (src == Y) src = nullptr;
@@ -318,19 +318,29 @@ void cholqr_async(double *Y, long long m, int n, int passes, double shift_rel, i
         TATRG_CUDA_CHECK(cudaMemcpyAsync(Y, src, sizeof(double) * m * n, cudaMemcpyDeviceToDevice, stream()));
         src = nullptr;
     }
-    if (cholqr_fused(Y, m, n, passes, shift_rel, flag_dev, ratio_dev, Rout)) return;
+    if (cholqr_fused(Y, m, n, passes, shift_rel, flag_dev, ratio_dev, Rout)) {
+        if (last_Linv) fill_identity(last_Linv, n);
+        return;
+    }
     size_t mark = ws_mark();
     Ten Ym = Ten::make(Y, "rc", {m, n});
     Ten T = ws_tensor("rd", {m, n});
     Ten C[3];
-    // the passes alternate between Y and T such that the last one lands in Y; with a separate source the first
-    // pass reads it directly (no copy of the block)
+    // the applies alternate between Y and T such that the last one lands in Y; with a separate source the first
+    // pass reads it directly (no copy of the block); with last_Linv the last factor is handed to the caller
+    // instead of being applied (a caller that multiplies Q by a small matrix anyway folds it into that)
+    const int applies = last_Linv ? passes - 1 : passes;
     Ten cur = src ? Ten::make(const_cast<double *>(src), "rc", {m, n}) : Ym;
     for (int p = 0; p < passes; ++p) {
-        Ten nxt = src ? (((passes - 1 - p) & 1) ? T : Ym) : (cur.p == Y ? T : Ym);
         C[p] = ws_tensor("cd", {n, n});
         contract(cur.as("rc"), cur.as("rd"), C[p]);
         Ten Linv = chol_inv(C[p], n, p == 0 ? shift_rel : 0.0, flag_dev, p == 0 ? ratio_dev : nullptr);
+        if (p >= applies) {
+            TATRG_CUDA_CHECK(cudaMemcpy2DAsync(last_Linv, sizeof(double) * n, Linv.p, sizeof(double) * Linv.legs[0].stride,
+                                               sizeof(double) * n, n, cudaMemcpyDeviceToDevice, stream()));
+            break;
+        }
+        Ten nxt = src ? (((applies - 1 - p) & 1) ? T : Ym) : (cur.p == Y ? T : Ym);
         contract(cur.as("rc"), Linv, nxt.as("rd"));       // Q[r,d] = sum_c Y[r,c] Linv[d,c]
         cur = nxt;
     }

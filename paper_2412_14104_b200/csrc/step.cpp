@@ -1012,6 +1012,9 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     const size_t canon_mark = ws_mark();
     Ten Qp = ws_tensor("rg", {R, g0}), Qs = ws_tensor("rg", {R, g0});
     Ten Rp = ws_tensor("gr", {g0, g0}), Rs = ws_tensor("hr", {g0, g0});
+    // the last Cholesky-QR factor of each side is not applied to the chi^5-sized block: Q = Q' L2inv^T, and every
+    // use of Q below is a product with a small matrix that absorbs it (one pass over the block less per side)
+    Ten L2ip = ws_tensor("gc", {g0, g0}), L2is = ws_tensor("gc", {g0, g0});
     {
         // the two tall QRs are independent: asynchronous Cholesky-QR2 on two streams; a side that is
         // rank deficient or too ill conditioned for it (the early steps) is redone by the robust route
@@ -1019,6 +1022,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         double *Yq[2] = {Qp.p, Qs.p};
         const double *src[2] = {c.phi, c.psi};
         double *Rq[2] = {Rp.p, Rs.p};
+        double *L2q[2] = {L2ip.p, L2is.p};
         if (!(c.routes & ROUTE_HOUSEHOLDER_QR) && R >= 16LL * g0 && R >= 512) {
             struct QrBack {
                 int flag;
@@ -1032,7 +1036,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 int *flag = (int *)ws_alloc(sizeof(int));
                 double *ratio = ws_doubles(2);
                 TATRG_CUDA_CHECK(cudaMemsetAsync(flag, 0, sizeof(int), stream()));
-                cholqr_async(Yq[i], R, g0, 2, 0.0, flag, ratio, Rq[i], src[i]);   // reads Phi / Psi, writes Q
+                cholqr_async(Yq[i], R, g0, 2, 0.0, flag, ratio, Rq[i], src[i], L2q[i]);   // reads Phi / Psi, writes Q'
                 TATRG_CUDA_CHECK(cudaMemcpyAsync(&bk->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
                 TATRG_CUDA_CHECK(cudaMemcpyAsync(bk->ratio, ratio, 2 * sizeof(double), cudaMemcpyDeviceToHost, stream()));
                 fk.leave();
@@ -1048,6 +1052,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             if (!qr_done[i]) {
                 d2d(Yq[i], src[i], R * g0);
                 tsqr(Yq[i], R, g0, Rq[i]);
+                fill_identity(L2q[i], (int)g0);
             }
     }
     trace_mark("canon: two tall QRs");
@@ -1068,8 +1073,9 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten QpR = rot_view(Qp.p, g0), QsR = rot_view(Qs.p, g0);
     Ten ref = get_input(5, R, a, cfg, "rb");
     Ten ref5 = Ten::make(ref.p, "xpqtb", {n0, n1, n2, n3, a});
-    Ten T1 = ws_tensor("gb", {g0, a});
-    contract(QpR.as("xpqtg"), ref5, T1);
+    Ten T1y = ws_tensor("cb", {g0, a}), T1 = ws_tensor("gb", {g0, a});
+    contract(QpR.as("xpqtc"), ref5, T1y);
+    contract(L2ip, T1y, T1);                // Q_Phi^T G_ref = L2inv (Q'^T G_ref)
     Ten Pg = ws_tensor("ab", {a, a});
     contract(u, T1, Pg);
     Ten Wg = gauge_rotation(Pg, spec[0], a);
@@ -1078,8 +1084,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     contract(Wg, v.as("ag"), v2);
     trace_mark("canon: gauge");
     Ten A = Ten::make(Abuf, "xpqta", {n0, n1, n2, n3, a}), D = Ten::make(Dbuf, "xpqta", {n0, n1, n2, n3, a});
-    contract(QpR.as("xpqtg"), u2.as("ag"), A);
-    contract(QsR.as("xpqtg"), v2.as("ag"), D);
+    Ten u3 = ws_tensor("ac", {a, g0}), v3 = ws_tensor("ac", {a, g0});
+    contract(u2.as("ag"), L2ip, u3);        // A = Q u2^T = Q' (L2inv^T u2^T)
+    contract(v2.as("ag"), L2is, v3);
+    contract(QpR.as("xpqtc"), u3, A);
+    contract(QsR.as("xpqtc"), v3, D);
     trace_mark("canon: A, D");
     ws_release(canon_mark);
     stage_mark(1);
