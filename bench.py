@@ -488,7 +488,7 @@ def run_ours(args, cfg, name):
                 "note": ("achieved = flop-weighted over ALL launches of the kernel inside the timed steps, as they run there: "
                          "steps (i), (ii) of the contraction and the grouped-leg Gram chains run on 140 of the 148 SMs beside the "
                          "squeezer chains (DESIGN.md section 4), and a third of the launches are one-wave shapes; the same kernel "
-                         "alone on the machine: 34.2-35.1 TFLOP/s on the hot shapes (profiles/r2_gemm_persistent_full.md)")}
+                         "alone on the machine: 34.0-35.0 TFLOP/s on the hot shapes (profiles/r2_gemm_persistent_full.md)")}
 
     line = None
     if rank == 0:

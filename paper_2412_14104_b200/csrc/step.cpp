@@ -1100,7 +1100,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     double *Ybuf = ws_doubles(dim * std::min<long long>(chi, ell));
     int gs = 0;
     double *sig = nullptr;
-    bool swapped = false;
+    bool swapped = false, x_scaled = false;
     // Reduced operator: M = (1 x Q_A) m (1 x Q_D)^T with A[c,I',b] = sum_k Q_A[I',k] R_A[k,c,b] and
     // D likewise (Q_A, Q_D orthonormal, nT x n0 a), m[(a k),(b l)] = sum_c sT_a R_D[l,c,a] R_A[k,c,b] sT_b.
     // Every iterate of the subspace iteration lies in the range of 1 x Q_A (resp. 1 x Q_D) and
@@ -1147,8 +1147,12 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 ws_release(mk2);
                 trace_mark("swap: rsvd of the core");
                 // expand: X[a,pqt,g] = sum_m Q1_A[pqt,m] sum_k L2inv_A[k,m] x[a,k,g]
+                double *sg = ws_doubles(gs);    // (the device copy inside rsvd's workspace has just been released)
+                h2d(sg, spec[1].data(), gs);
                 Ten t2 = ws_tensor("amg", {a, nk, gs});
                 contract(bA.L2inv.as("km"), Ten::make(xr, "akg", {a, nk, gs}), t2);
+                scale_leg(t2.p, t2.size(), 1, gs, sg, 0);   // X enters the rest of the step only as X sigma (Eq. 5)
+                x_scaled = true;
                 contract(bA.Q1.as("pqtm"), t2, Ten::make(Xbuf, "apqtg", {a, n1, n2, n3, gs}));
                 contract(bD.L2inv.as("km"), Ten::make(yr, "akg", {a, nk, gs}), t2);
                 contract(bD.Q1.as("pqtm"), t2, Ten::make(Ybuf, "apqtg", {a, n1, n2, n3, gs}));
@@ -1194,7 +1198,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     // X enters the rest of the step only as X sigma (Eq. 5): scaled in place; Y is needed both ways
     Ten Xs = X, Ys = ws_tensor("buvwg", {a, n1, n2, n3, gs});
     d2d(Ys.p, Y.p, Y.size());
-    scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
+    if (!x_scaled) scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
     scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
     trace_mark("swap: expansion, scaling");
     stage_mark(2);
