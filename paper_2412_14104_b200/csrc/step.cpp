@@ -1209,6 +1209,13 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     bool iso_lazy[4] = {false, false, false, false};
     double *Hkeep[4] = {nullptr, nullptr, nullptr, nullptr};
     int iso_kk = 0;
+    struct RitzBack {   // page-locked read-back of the deferred Ritz steps (r chi <= 64)
+        int flag[4];
+        double lam[4][64];
+    } *ritz_back = nullptr;
+    bool ritz_deferred[4] = {false, false, false, false};
+    double *ritz_V = nullptr, *ritz_lam = nullptr;
+    int *ritz_flag = nullptr;
     Ten E, F, G, H;
     long long kd = 0;
     Ten GL[3], GR[3];
@@ -1483,12 +1490,14 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             }
             Ten Vt = ws_tensor("kz", {kk, kk});
             double *lam = ws_doubles(kk);
-            if (fast && kk > 64) {
-                // Wide internal lines (r chi > 64): the Ritz rotation is left out of the path.  Gamma^triad
-                // depends on U only through its span (E I = A U U^T etc.: every oversampled line is summed
-                // over in Eqs. 13-14 and in the Grams of Eq. 12), so the orthonormal block Q itself is used
-                // as U; the kk x kk Ritz matrix H goes to the host and the spectrum S (a diagnostic of the
-                // step) is computed from it when it is asked for (resolve_iso_spectra).
+            if (fast) {
+                // The Ritz rotation is left out of the path.  Gamma^triad depends on U only through its span
+                // (E I = A U U^T etc.: every oversampled line is summed over in Eqs. 13-14 and in the Grams
+                // of Eq. 12), so the orthonormal block Q itself is used as U.  r chi <= 64: the eigenvalues
+                // of the Ritz matrix H (the spectrum S of the step) are computed by the one-CTA solver on a
+                // stream of their own BESIDE the triad tensors and Gram chains (below) and read at the end of
+                // the step -- four single-CTA kernels no longer hold up the machine.  Wider lines: H goes to
+                // the host and S is computed from it when it is asked for (resolve_iso_spectra).
                 d2d(U[i].p, Qi.p, n12 * kk);
                 d2d(Hkeep[i], Hm.p, (long long)kk * kk);
                 back->pad = nqr;
@@ -1496,23 +1505,19 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 2 * nqr * sizeof(double), cudaMemcpyDeviceToHost, stream()));
                 return;
             }
-            if (fast) {
-                eig_small_async(Hm.p, kk, Vt.p, lam, flag);
-                back->pad = nqr;
-                TATRG_CUDA_CHECK(cudaMemcpyAsync(&back->flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream()));
-                TATRG_CUDA_CHECK(cudaMemcpyAsync(back->ratio, ratio, 2 * nqr * sizeof(double), cudaMemcpyDeviceToHost, stream()));
-                TATRG_CUDA_CHECK(cudaMemcpyAsync(back->lam, lam, kk * sizeof(double), cudaMemcpyDeviceToHost, stream()));
-            } else {
-                std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);
-                spec[2 + i].resize(kk);
-                for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
-            }
+            std::vector<double> lh = sym_eig(Hm.p, kk, Vt.p, lam);   // the robust synchronous route
+            spec[2 + i].resize(kk);
+            for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(lh[j], 0.0));
             contract(Ten::make(Qi.p, "pqz", {n1, n2, kk}), Vt, U[i]);
         };
         bool iso_done[4] = {false, false, false, false};
         const bool wide = kk > 64;
-        if (wide)
-            for (int i = 0; i < 4; ++i) Hkeep[i] = ws_doubles((long long)kk * kk);   // outlives the chains' slices
+        for (int i = 0; i < 4; ++i) Hkeep[i] = ws_doubles((long long)kk * kk);   // outlives the chains' slices
+        if (!wide) {
+            ritz_V = ws_doubles(4LL * kk * kk);
+            ritz_lam = ws_doubles(4LL * kk);
+            ritz_flag = (int *)ws_alloc(4 * sizeof(int));
+        }
         if (!(c.routes & ROUTE_SEQUENTIAL_ISO) && kk <= 256 && q + 1 <= 8 && n12 >= (wide ? 2LL : 16LL) * kk) {   // the four isometries as concurrent chains
             Fork fk(4);
             for (int i = 0; i < 4; ++i) {
@@ -1526,21 +1531,37 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 bool ok = bk->flag == 0;
                 for (int j = 0; j < bk->pad; ++j) ok = ok && bk->ratio[2 * j] > 1e-5 * bk->ratio[2 * j + 1];
                 if (!ok) continue;   // ill conditioned block or no convergence: redone below
-                if (wide) {
+                iso_kk = kk;
+                if (wide)
                     iso_lazy[i] = true;
-                    iso_kk = kk;
-                } else {
-                    spec[2 + i].resize(kk);
-                    for (int j = 0; j < kk; ++j) spec[2 + i][j] = sqrt(std::max(bk->lam[j], 0.0));
-                }
+                else
+                    ritz_deferred[i] = true;
                 iso_done[i] = true;
             }
             fk.join();
+            // the deferred Ritz steps: one single-CTA eigensolver per isometry on side streams 4..7 (no Fork of this
+            // step has more than six chains), after everything the chains wrote; read back at the end of the step
+            if (!wide) {
+                TATRG_CUDA_CHECK(cudaMemsetAsync(ritz_flag, 0, 4 * sizeof(int), stream()));
+                TATRG_CUDA_CHECK(cudaEventRecord(c.fork_ev, stream()));
+                ritz_back = reinterpret_cast<RitzBack *>(fk.pinned(Ctx::MAX_CHAINS - 1));
+                cudaStream_t main_stream = c.stream;
+                for (int i = 0; i < 4; ++i) {
+                    if (!ritz_deferred[i]) continue;
+                    c.stream = c.side[4 + i];
+                    TATRG_CUDA_CHECK(cudaStreamWaitEvent(c.stream, c.fork_ev, 0));
+                    eig_small_async(Hkeep[i], kk, ritz_V + (long long)i * kk * kk, ritz_lam + (long long)i * kk, ritz_flag + i);
+                    TATRG_CUDA_CHECK(cudaMemcpyAsync(&ritz_back->flag[i], ritz_flag + i, sizeof(int), cudaMemcpyDeviceToHost, c.stream));
+                    TATRG_CUDA_CHECK(cudaMemcpyAsync(ritz_back->lam[i], ritz_lam + (long long)i * kk, kk * sizeof(double), cudaMemcpyDeviceToHost, c.stream));
+                    c.stream = main_stream;
+                }
+            }
         }
         for (int i = 0; i < 4; ++i)
             if (!iso_done[i]) {
                 size_t mk = ws_mark();
                 iso_lazy[i] = false;
+                ritz_deferred[i] = false;
                 iso_body(i, false, nullptr);
                 ws_release(mk);
             }
@@ -1852,6 +1873,18 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     c.state_bytes = 2 * new_cap;
     spec[9] = {lnc};
     for (int mu = 0; mu < 3; ++mu) c.sq_hist[direction - 1][mu] = sq_hist_new[mu];
+    // the deferred Ritz steps of the isometries ended long ago: collect the spectra S^A..S^D; a solver that did not
+    // converge, or kept isometries (tests: the Ritz vectors are wanted as well), leave the rest to resolve_iso_spectra
+    for (int i = 0; i < 4; ++i) {
+        if (!ritz_deferred[i]) continue;
+        TATRG_CUDA_CHECK(cudaStreamSynchronize(c.side[4 + i]));
+        if (ritz_back->flag[i] != 0 || c.keep_iso) {
+            iso_lazy[i] = true;
+            continue;
+        }
+        spec[2 + i].resize(iso_kk);
+        for (int j = 0; j < iso_kk; ++j) spec[2 + i][j] = sqrt(std::max(ritz_back->lam[i][j], 0.0));
+    }
     for (int i = 0; i < 10; ++i) c.spec[i] = spec[i];
     for (int i = 0; i < 4; ++i) {
         c.iso_pending[i] = iso_lazy[i];
