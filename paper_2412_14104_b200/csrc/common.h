@@ -165,6 +165,7 @@ void scale_rows(double *x, long long rows, long long cols, const double *v, int 
 // x[i] *= f(v[(i / inner) % n]) : scales a tensor along one leg (inner = its stride, n = its size);
 // mode 5: v^-3/2
 void scale_leg(double *x, long long total, long long inner, long long n, const double *v, int mode);
+void scale_inner_copy(const double *src, double *dst, long long total, long long n, const double *v);   // dst[.., c] = src[.., c] * v[c]
 void symmetrize(double *x, int n);                                            // x = (x + x^T)/2
 void fill_identity(double *x, int n);
 void fill_zero(double *x, long long n);

@@ -140,6 +140,21 @@ __global__ void scale_leg_kernel(double *__restrict__ x, long long total, long l
     for (long long i = tid; i < total; i += stride) x[i] *= scale_fn(v[(i / inner) % n], mode);
 }
 
+// dst[i] = src[i] * v[i % n] for the innermost leg (n even, 16-byte aligned buffers): two elements per thread
+__global__ void scale_inner_copy_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long pairs, int n,
+                                        const double *__restrict__ v)
+{
+    long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = tid; i < pairs; i += stride) {
+        const int c = (int)((2 * i) % n);
+        double2 a = src[i];
+        a.x *= v[c];
+        a.y *= v[c + 1];
+        dst[i] = a;
+    }
+}
+
 // x = (x + x^T)/2, n x n
 __global__ void symmetrize_kernel(double *x, int n)
 {
@@ -262,6 +277,21 @@ void scale_leg(double *x, long long total, long long inner, long long n, const d
 {
     if (total <= 0) return;
     scale_leg_kernel<<<grid_for(total), RED_THREADS, 0, stream()>>>(x, total, inner, n, v, mode);
+    TATRG_LAUNCH_CHECK();
+    count_launch();
+}
+
+// dst = src scaled along its innermost leg of size n (one pass instead of a copy and an in-place scaling)
+void scale_inner_copy(const double *src, double *dst, long long total, long long n, const double *v)
+{
+    if (total <= 0) return;
+    if ((n & 1) || (total & 1) || (((uintptr_t)src | (uintptr_t)dst) & 15)) {
+        TATRG_CUDA_CHECK(cudaMemcpyAsync(dst, src, sizeof(double) * total, cudaMemcpyDeviceToDevice, stream()));
+        scale_leg(dst, total, 1, n, v, 0);
+        return;
+    }
+    scale_inner_copy_kernel<<<grid_for(total / 2), RED_THREADS, 0, stream()>>>(reinterpret_cast<const double2 *>(src),
+                                                                              reinterpret_cast<double2 *>(dst), total / 2, (int)n, v);
     TATRG_LAUNCH_CHECK();
     count_launch();
 }

@@ -1197,9 +1197,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     Ten Y = Ten::make(Ybuf, "buvwg", {a, n1, n2, n3, gs});
     // X enters the rest of the step only as X sigma (Eq. 5): scaled in place; Y is needed both ways
     Ten Xs = X, Ys = ws_tensor("buvwg", {a, n1, n2, n3, gs});
-    d2d(Ys.p, Y.p, Y.size());
     if (!x_scaled) scale_leg(Xs.p, Xs.size(), 1, gs, sig, 0);
-    scale_leg(Ys.p, Ys.size(), 1, gs, sig, 0);
+    scale_inner_copy(Y.p, Ys.p, Y.size(), gs, sig);
     trace_mark("swap: expansion, scaling");
     stage_mark(2);
 
