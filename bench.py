@@ -570,6 +570,63 @@ def run_gemm_micro(args):
     print(json.dumps({"gemm_micro": out}), flush=True)
 
 
+def run_split_emulation(args, cfg, name):
+    """--split: what each of the two processes of the Phi / Psi split (tatrg_set_side_split; PAPER.md:167 'two GPUs
+    are used') does per step, timed on ONE GPU by playing them one after the other: the whole
+    step, then rank 1 (Psi only), then rank 0 (Phi only), the same steady-state steps each; the exchange is a device
+    copy of the other half (same bytes as the NVLink transfer it stands for, which is NOT measured here).  Not the
+    headline metric: prints a line of its own."""
+    import torch
+    import paper_2412_14104_b200 as tt
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libtatrg has no CPU fallback")
+    chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
+    K, W, ramp = args.steps, max(args.warmup, 0), cfg["ramp"]
+    tt.set_workspace(chi=chi, r=r, atrg=bool(cfg.get("atrg")))
+    step_fn = tt.coarse_grain_atrg if cfg.get("atrg") else tt.coarse_grain
+    stream = torch.cuda.Stream()
+    tt.set_stream(stream)
+    at = {"m": 0}
+
+    def one_pass(sides, exchange):
+        tt.set_side_split(sides, exchange)
+        try:
+            tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
+            pairs, lnz = [], []
+            for m in range(ramp + W + K):
+                at["m"] = m
+                ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                ev[0].record(stream)
+                step_fn(m % 4 + 1, chi, r, q, seed)
+                ev[1].record(stream)
+                if m >= ramp + W:
+                    pairs.append(ev)
+                lnz.append(tt.log_Z_per_site())
+            torch.cuda.synchronize()
+            return sum(a.elapsed_time(b) for a, b in pairs) / K, lnz
+        finally:
+            tt.set_side_split(3)
+
+    whole_phi, sent = [], []
+    ms_whole, lnz_whole = one_pass(3, lambda phi, psi: whole_phi.append(phi.clone()))
+
+    def exchange_rank1(phi, psi):
+        sent.append(psi.clone())
+        phi.copy_(whole_phi[at["m"]])
+
+    ms_r1, _ = one_pass(2, exchange_rank1)
+    ms_r0, lnz_r0 = one_pass(1, lambda phi, psi: psi.copy_(sent[at["m"]]))
+    half_bytes = int(whole_phi[-1].numel()) * 8
+    print(json.dumps({"mode": "Phi / Psi split over two GPUs, the two processes played one after the other on one GPU",
+                      "config": {"workload": workload_name(name, cfg), "steps": K, "warmup": W, "ramp": ramp},
+                      "whole_ms_per_step": ms_whole, "rank0_ms_per_step": ms_r0, "rank1_ms_per_step": ms_r1,
+                      "split_ms_per_step_without_link": max(ms_r0, ms_r1),
+                      "exchange": "device copy of the other half inside the step; over NVLink each process sends and "
+                                  "receives %d bytes per step (not measured: one GPU)" % half_bytes,
+                      "ln_Z_rank0_vs_whole_max_rel": max(abs(a / b - 1) for a, b in zip(lnz_r0, lnz_whole))}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -582,6 +639,7 @@ def main():
     ap.add_argument("--tma", action="store_true", help="with --gemm: feed the persistent tile from TMA instead of cp.async")
     ap.add_argument("--chi", type=int, default=None, help="override the bond dimension of the chosen config (scaling study)")
     ap.add_argument("--r", type=int, default=None, help="override the oversampling parameter r (the paper's figures use r = 7)")
+    ap.add_argument("--split", action="store_true", help="time the two halves of the two-GPU Phi / Psi split one after the other on one GPU")
     args = ap.parse_args()
     if args.gemm:
         run_gemm_micro(args)
@@ -593,6 +651,9 @@ def main():
         cfg["r"] = args.r
     if args.impl == "reference":
         run_reference(args, cfg, args.config)
+        return
+    if args.split:
+        run_split_emulation(args, cfg, args.config)
         return
     line = run_ours(args, cfg, args.config)
     rank = int(os.environ.get("RANK", "0"))

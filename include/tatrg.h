@@ -112,6 +112,25 @@ int tatrg_get_spectrum(int which, double *host_out, int cap);
  * of sq_iter.cu.  0 = default; mask in 0..63, else TATRG_EINVAL. */
 int tatrg_set_routes(int mask);
 
+/* Phi / Psi split of one step over two GPUs ("two GPUs are used", Fig. 6).
+ * The two halves of the contraction, Phi of Eq. 13 and Psi of Eq. 14 (for coarse_grain_atrg the
+ * two O(chi^9) products of PAPER.md:92), share no intermediate.  Two processes, one per GPU, run the same steps
+ * from the same state with the same seeds (everything up to the squeezers is computed by both: the same kernels
+ * on the same inputs give the same bits); sides = 1 makes this process contract Phi only, sides = 2 Psi only,
+ * 3 = both (default; an exchange_fn given with 3 is called as an observer of the two finished, not yet normalised
+ * tensors, NULL clears it).  After its half the library calls, once per step,
+ *     int exchange_fn(void *user, double *phi_dev, double *psi_dev, int64_t n, void *cuda_stream)
+ * (exchange_fn is passed as a plain pointer to a function of exactly this type): phi_dev / psi_dev (device) are
+ * the new, not yet normalised tensors of n doubles each, this process's half complete in the order of
+ * cuda_stream (the library's stream), the other half undefined.  The callback fills the other half (the binding:
+ * one NCCL all-gather over NVLink) so that it is complete in the order of cuda_stream when it returns, or after a
+ * synchronisation of its own; it returns 0, anything else fails the step with TATRG_ECUDA (state of the previous
+ * step intact).  The library then normalises both halves and commits the step as usual, so both processes end on
+ * the same state.  The callback must not call into the library.  sides outside 1..3, or one half without an
+ * exchange_fn: TATRG_EINVAL.  user is handed back unchanged; both pointers must stay valid until the next
+ * tatrg_set_side_split. */
+int tatrg_set_side_split(int sides, void *exchange_fn, void *user);
+
 /* Oversampled isometries of the LAST coarse_grain step (Eqs. 2-3; I, J, K, L of Eqs. 8-11),
  * for tests (the projector U U^T is gauge invariant and is what parity compares).  tatrg_keep_isometries(1)
  * makes every following step copy its four isometries to the host (one extra synchronisation per step);

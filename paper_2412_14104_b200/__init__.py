@@ -20,7 +20,7 @@ EXPORTS = [
     "init_ising_tensor", "coarse_grain", "coarse_grain_atrg", "log_Z_per_site",
     "tatrg_set_stream", "tatrg_set_workspace", "tatrg_workspace_bytes", "tatrg_workspace_bytes_atrg",
     "tatrg_workspace_peak",
-    "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_set_routes", "tatrg_keep_isometries", "tatrg_get_isometry", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
+    "tatrg_set_sketch", "tatrg_sketch_shape", "tatrg_set_routes", "tatrg_set_side_split", "tatrg_keep_isometries", "tatrg_get_isometry", "tatrg_get_spectrum", "tatrg_get_gaps", "tatrg_get_dims",
     "tatrg_get_tensors", "tatrg_order_parameter", "tatrg_get_stage_ms", "tatrg_stage_name", "tatrg_get_h2d",
     "tatrg_set_profile", "tatrg_get_gemm_profile",
     "tatrg_launch_count", "tatrg_gemm_flops", "tatrg_probe_fp64_peak", "tatrg_tensor_gemm",
@@ -63,6 +63,7 @@ def lib():
             "tatrg_sketch_shape": (c_i, [c_i, c_i, c_i, c_i, ctypes.POINTER(c_i64), ctypes.POINTER(c_i64)]),
             "tatrg_get_spectrum": (c_i, [c_i, c_vp, c_i]),
             "tatrg_set_routes": (c_i, [c_i]),
+            "tatrg_set_side_split": (c_i, [c_i, c_vp, c_vp]),
             "tatrg_keep_isometries": (c_i, [c_i]),
             "tatrg_get_isometry": (c_i, [c_i, c_vp, c_sz, ctypes.POINTER(c_i), ctypes.POINTER(c_i)]),
             "tatrg_get_gaps": (c_i, [c_vp]),
@@ -101,7 +102,8 @@ def lib():
 
 def _check(rc):
     if rc != 0:
-        raise TatrgError("libtatrg error %d: %s" % (rc, lib().tatrg_last_error().decode()))
+        cause = _keep.pop("exchange_error", None)    # an exception of the caller's exchange (set_side_split)
+        raise TatrgError("libtatrg error %d: %s" % (rc, lib().tatrg_last_error().decode())) from cause
 
 
 def _require_cuda():
@@ -203,6 +205,77 @@ ROUTE_UNFUSED_SQUEEZER = 32
 def set_routes(mask=0):
     """Forces the robust routes of coarse_grain (mask of ROUTE_*); 0 restores the defaults."""
     _check(lib().tatrg_set_routes(int(mask)))
+
+
+_EXCHANGE_T = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                               ctypes.c_void_p)
+
+
+class _DeviceDoubles:
+    """n doubles at a raw device address, for torch.as_tensor (no copy)."""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+
+def set_side_split(sides=3, exchange=None):
+    """tatrg_set_side_split: sides = 1 contracts Phi only, 2 Psi only, 3 both (default).  `exchange(phi, psi)` is a
+    Python callable that gets the two new tensors as flat torch views of the library's buffers, with the library's
+    stream current, and completes the half this process did not compute (two GPUs); with sides = 3
+    it only observes the two finished, not yet normalised tensors."""
+    import torch
+    if int(sides) == 3 and exchange is None:
+        _check(lib().tatrg_set_side_split(3, None, None))
+        _keep.pop("exchange", None)
+        return
+
+    def trampoline(_user, phi_ptr, psi_ptr, n, stream_ptr):
+        try:
+            stream = torch.cuda.ExternalStream(stream_ptr) if stream_ptr else torch.cuda.default_stream()
+            with torch.cuda.stream(stream):
+                phi = torch.as_tensor(_DeviceDoubles(phi_ptr, n), device="cuda")
+                psi = torch.as_tensor(_DeviceDoubles(psi_ptr, n), device="cuda")
+                exchange(phi, psi)
+            return 0
+        except BaseException as e:      # an exception must not unwind through the C frames
+            _keep["exchange_error"] = e
+            return 1
+
+    if exchange is None:
+        raise TatrgError("set_side_split: computing one half needs an exchange callable")
+    fn = _EXCHANGE_T(trampoline)
+    _check(lib().tatrg_set_side_split(int(sides), ctypes.cast(fn, ctypes.c_void_p), None))
+    _keep["exchange"] = fn
+
+
+def exchange_halves(phi, psi, rank, group=None):
+    """The one exchange of a split step: rank 0 of the two-process group owns Phi, rank 1 Psi; each sends its half
+    to the other and receives the other's, as one batch of point-to-point operations (NCCL: both directions of
+    the NVLink at once; ordered on the current stream).  Works on any pair of equally shaped tensors (gloo on CPU
+    in the tests)."""
+    import torch.distributed as dist
+    if dist.get_world_size(group) != 2:
+        raise TatrgError("the Phi / Psi split needs a group of exactly two processes")
+    peer = dist.get_global_rank(group, 1 - rank) if group is not None else 1 - rank
+    mine, other = (phi, psi) if rank == 0 else (psi, phi)
+    ops = [dist.P2POp(dist.isend, mine, peer, group), dist.P2POp(dist.irecv, other, peer, group)]
+    for w in dist.batch_isend_irecv(ops):
+        w.wait()
+
+
+def enable_phi_psi_split(group=None):
+    """Splits every following coarse_grain / coarse_grain_atrg step over the two processes (one GPU each) of
+    `group` (default: the world): this process contracts the half its group rank owns and exchange_halves
+    completes the other over NCCL.  Both processes must run the same calls from the same state with the same seeds."""
+    import torch.distributed as dist
+    rank = dist.get_rank(group)
+    if dist.get_world_size(group) != 2:
+        raise TatrgError("the Phi / Psi split needs a group of exactly two processes")
+    set_side_split(1 << rank, lambda phi, psi: exchange_halves(phi, psi, rank, group))
+
+
+def disable_phi_psi_split():
+    set_side_split(3)
 
 
 def keep_isometries(on=True):

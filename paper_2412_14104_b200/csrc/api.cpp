@@ -338,6 +338,17 @@ int tatrg_set_routes(int mask)
     return TATRG_OK;
 }
 
+int tatrg_set_side_split(int sides, void *exchange_fn, void *user)
+{
+    if (sides < 1 || sides > 3) return set_error(TATRG_EINVAL, "tatrg_set_side_split: sides must be 1 (Phi), 2 (Psi) or 3 (both)");
+    if (sides != 3 && !exchange_fn)
+        return set_error(TATRG_EINVAL, "tatrg_set_side_split: computing one half needs an exchange that supplies the other");
+    ctx().side_mask = sides;
+    ctx().exchange = reinterpret_cast<int (*)(void *, double *, double *, long long, void *)>(exchange_fn);
+    ctx().exchange_user = exchange_fn ? user : nullptr;
+    return TATRG_OK;
+}
+
 int tatrg_keep_isometries(int on)
 {
     ctx().keep_iso = on != 0;

@@ -61,6 +61,11 @@ struct Ctx {
     int sm_reserve = 0;                     // SMs the persistent GEMM leaves to concurrent chains (step.cpp)
     int chol_ctas = 16;                     // CTAs of the resident blocked Cholesky (chol.cu); 0: one launch per panel step
     int routes = 0;                         // mask of Route: robust routes forced by tatrg_set_routes
+    // Phi / Psi split over two GPUs (tatrg_set_side_split): the halves of the contraction this process
+    // computes (bit 0 Phi, bit 1 Psi) and the caller's exchange that completes the other half before the normalisation
+    int side_mask = 3;
+    int (*exchange)(void *user, double *phi, double *psi, long long n, void *stream) = nullptr;
+    void *exchange_user = nullptr;
     bool keep_iso = false;                  // tatrg_keep_isometries: host copies of U^A, U^X, U^Y, U^D of the last step
     std::vector<double> iso[4];
     int iso_rows = 0, iso_cols = 0;

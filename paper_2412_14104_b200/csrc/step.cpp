@@ -1731,8 +1731,8 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             // (handing the second side to the main stream only after the chains have ended, so that it gets every
             // SM, measured slower: the chains outlast the first side and the main stream idles meanwhile)
             squeeze_wave({0, 1}, [&]() {
-                side0();
-                side1();
+                if (c.side_mask & 1) side0();
+                if (c.side_mask & 2) side1();
             });
             pre_done = true;
         } else {
@@ -1757,6 +1757,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
     };
     if ((size_t)(n0 * m1 * m2 * m3 * gs) * 8 > new_cap) fail(-12, "internal: new state exceeds its reservation");
     for (int side = 0; side < 2 && mode == 0; ++side) {
+        if (!(c.side_mask >> side & 1)) continue;   // the other GPU's half (tatrg_set_side_split)
         size_t mk = ws_mark();
         Ten W1 = ws_tensor("qkPm", {n2, kd, n1, m1}), V2 = ws_tensor("Plqn", {n1, kd, n2, m2});
         Ten Qt = ws_tensor("klmn", {kd, kd, m1, m2});
@@ -1813,7 +1814,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ten T2 = ws_tensor("qtmsug", {n2, n3, m1, n2, n3, gs});    // . (X sigma) over (a, r)
         Ten T3 = ws_tensor("tmnug", {n3, m1, m2, n3, gs});         // . M2 over (q, s)
         Ten outP = new_view(phi_new), outS = new_view(psi_new);
-        for (long long x = 0; x < n0; ++x) {
+        for (long long x = 0; x < n0 && (c.side_mask & 1); ++x) {
             Ten Ax = Ten::make(A.p + x * (n1 * n2 * n3 * a), "pqta", {n1, n2, n3, a});
             contract(Ax, Ms[0].as("prm"), T1);
             contract(T1, Xs.as("arsug"), T2);
@@ -1827,7 +1828,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
         Ten S1 = ws_tensor("subpm", {n2, n3, a, n1, m1});          // per x: D[x] N1 over r
         Ten S2 = ws_tensor("sumqtg", {n2, n3, m1, n2, n3, gs});    // . Y over (b, p)
         Ten S3 = ws_tensor("umntg", {n3, m1, m2, n3, gs});         // . N2 over (q, s)
-        for (long long x = 0; x < n0; ++x) {
+        for (long long x = 0; x < n0 && (c.side_mask & 2); ++x) {
             Ten Dx = Ten::make(D.p + x * (n1 * n2 * n3 * a), "rsub", {n1, n2, n3, a});
             contract(Dx, Ns[0].as("mpr"), S1);
             contract(S1, Y.as("bpqtg"), S2);
@@ -1843,6 +1844,14 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
 
     // =================== O8 normalise, accumulate ln Z ===================
     const long long nnew = n0 * m1 * m2 * m3 * gs;
+    if (c.side_mask != 3 || c.exchange) {
+        // Phi / Psi split over two GPUs: this process contracted one half;
+        // the caller's exchange (one send / receive pair over NVLink in the binding) completes the other before
+        // the norms (with both halves contracted here the callback is an observer of the finished tensors)
+        if (!c.exchange) fail(-22, "coarse_grain: one half of the contraction is switched off and no exchange is set");
+        const int xrc = c.exchange(c.exchange_user, phi_new, psi_new, nnew, (void *)stream());
+        if (xrc != 0) fail(-5, "coarse_grain: the caller's exchange of the Phi / Psi halves failed (status %d)", xrc);
+    }
     double *ss = ws_doubles(2);
     sumsq(phi_new, nnew, ss);
     sumsq(psi_new, nnew, ss + 1);

@@ -1,6 +1,8 @@
 """N > 1 is "replicas only": no data-path collective exists.  What N > 1 adds is host
 logic in bench.py -- MAX over ranks of the device times, SUM of the counters, whole-job value, rank-0-only
-output of the reference arm -- covered here with world_size 2 over gloo on CPU."""
+output of the reference arm -- covered here with world_size 2 over gloo on CPU.  The one exchange that does exist
+is opt-in (the two-GPU Phi / Psi split of PAPER.md:167): exchange_halves of the binding, run
+here by two gloo processes on CPU tensors."""
 import json
 import os
 import subprocess
@@ -66,3 +68,40 @@ def test_timed_steps_stay_inside_the_schedule():
     import pytest
     with pytest.raises(ValueError):
         bench.timed_segments(8, 32, 1)
+
+
+SPLIT_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import torch, torch.distributed as dist
+import paper_2412_14104_b200 as t
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%%s" %% os.environ["PORT"],
+                        rank=int(os.environ["RANK"]), world_size=2)
+rank = dist.get_rank()
+ok = True
+for group in (None, dist.new_group([0, 1])):
+    n = 100003
+    full_phi = torch.arange(n, dtype=torch.float64) * 0.5 + 1.0      # what rank 0 contracted
+    full_psi = -torch.arange(n, dtype=torch.float64) / 3.0 - 2.0     # what rank 1 contracted
+    phi = full_phi.clone() if rank == 0 else torch.full((n,), float("nan"), dtype=torch.float64)
+    psi = full_psi.clone() if rank == 1 else torch.full((n,), float("nan"), dtype=torch.float64)
+    t.exchange_halves(phi, psi, rank, group)
+    ok = ok and torch.equal(phi, full_phi) and torch.equal(psi, full_psi)
+print(json.dumps({"rank": rank, "ok": bool(ok)}))
+dist.destroy_process_group()
+""" % ROOT
+
+
+def test_phi_psi_exchange_world2_gloo(tmp_path):
+    """After exchange_halves both processes hold both halves, bit for bit: rank 0's Phi, rank 1's Psi."""
+    script = tmp_path / "split_worker.py"
+    script.write_text(SPLIT_WORKER)
+    port = str(31500 + os.getpid() % 2000)
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), PORT=port)
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, text=True))
+    outs = [p.communicate(timeout=180)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs)
+    for out in outs:
+        assert json.loads(out.strip().splitlines()[-1])["ok"] is True
