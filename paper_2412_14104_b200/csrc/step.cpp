@@ -1458,6 +1458,11 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             auto orth = [&](double *Y, bool last) {
                 if (fast) {
                     if (last) {
+                        // wide lines (the paper's r = 7): r chi columns reach far down the spectrum of S and the
+                        // block is often too ill conditioned for two plain passes (the chain was rejected and the
+                        // isometry redone on the synchronous route, 25 ms each): a shifted pass first (shifted
+                        // Cholesky-QR3; the span, all that enters Gamma^triad, is unchanged), the check on the next
+                        if (kk > 64) cholqr_async(Y, n12, kk, 1, 1e-13, flag, nullptr, nullptr);
                         cholqr_async(Y, n12, kk, 2, 0.0, flag, ratio + 2 * nqr, nullptr);
                         ++nqr;
                     } else {
@@ -1517,7 +1522,7 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
             ritz_lam = ws_doubles(4LL * kk);
             ritz_flag = (int *)ws_alloc(4 * sizeof(int));
         }
-        if (!(c.routes & ROUTE_SEQUENTIAL_ISO) && kk <= 256 && q + 1 <= 8 && n12 >= (wide ? 2LL : 16LL) * kk) {   // the four isometries as concurrent chains
+        if (!(c.routes & ROUTE_SEQUENTIAL_ISO) && kk <= 256 && q + 1 <= 8 && n12 >= (wide ? 2LL : 4LL) * kk) {   // the four isometries as concurrent chains
             Fork fk(4);
             for (int i = 0; i < 4; ++i) {
                 fk.enter(i);
@@ -1529,7 +1534,10 @@ void do_coarse_grain(int direction, int chi, int r, int q, uint64_t seed, int mo
                 const IsoBack *bk = reinterpret_cast<IsoBack *>(fk.pinned(i));
                 bool ok = bk->flag == 0;
                 for (int j = 0; j < bk->pad; ++j) ok = ok && bk->ratio[2 * j] > 1e-5 * bk->ratio[2 * j + 1];
-                if (!ok) continue;   // ill conditioned block or no convergence: redone below
+                if (!ok) {           // ill conditioned block or no convergence: redone below
+                    if (getenv("TATRG_TRACE")) fprintf(stderr, "tatrg-trace isometry %d: chain rejected (flag %d), robust route\n", i, bk->flag);
+                    continue;
+                }
                 iso_kk = kk;
                 if (wide)
                     iso_lazy[i] = true;
