@@ -149,6 +149,14 @@ def test_r7_wide_internal_lines_chi20(tt):
     check(run_both(tt, 1 / 6.65, 0.0, 20, 7, 1, 5, 434343))
 
 
+@pytest.mark.parametrize("chi,r,n", [(12, 3, 10), (20, 2, 7)])
+def test_isometry_chains_at_widths_between_32_and_64(tt, chi, r, n):
+    """Oversampled lines that are neither 32 nor 64 wide on the concurrent isometry chains (fused Cholesky-QR of a
+    36- or 40-column block, the one-CTA Ritz solver at that width): chi = 12, r = 3 (r chi = 36 on 144 pair
+    states, the fewest rows per column the chains take) and chi = 20, r = 2 (r chi = 40 on 400 pair states)."""
+    check(run_both(tt, 1 / 6.65, 0.0, chi, r, 2, n, 20241219))
+
+
 def test_plain_atrg_parity(tt):
     """coarse_grain_atrg (Table 1: no triads, O(chi^9) contraction) against the oracle's
     mode='atrg' on the same seeded bond-swap sketches."""
