@@ -570,6 +570,52 @@ def run_gemm_micro(args):
     print(json.dumps({"gemm_micro": out}), flush=True)
 
 
+def run_split_two_gpus(args, cfg, name):
+    """--split under torchrun with exactly two processes: the real thing, one GPU each, the halves exchanged over
+    NCCL every step (enable_phi_psi_split).  One step of the pair = one coarse-graining step, so the value is
+    steps/s of the PAIR (strong scaling of one lattice, not replicas).  Not run in this project's environment
+    (one GPU per box): the single-process emulation below is what was measured."""
+    import torch
+    import torch.distributed as dist
+    import paper_2412_14104_b200 as tt
+    rank, local = int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0"))
+    if int(os.environ["WORLD_SIZE"]) != 2:
+        raise RuntimeError("--split needs exactly two processes (torchrun --nproc-per-node 2)")
+    torch.cuda.set_device(local)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
+    K, W, ramp = args.steps, max(args.warmup, 0), cfg["ramp"]
+    tt.set_workspace(chi=chi, r=r, device="cuda:%d" % local, atrg=bool(cfg.get("atrg")))
+    step_fn = tt.coarse_grain_atrg if cfg.get("atrg") else tt.coarse_grain
+    stream = torch.cuda.Stream()
+    tt.set_stream(stream)
+    tt.enable_phi_psi_split()
+    try:
+        tt.init_ising_tensor(1.0 / cfg["T"], cfg["h"])
+        with torch.cuda.stream(stream):
+            for m in range(ramp + W):
+                step_fn(m % 4 + 1, chi, r, q, seed)
+            dist.barrier()
+            torch.cuda.synchronize()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(stream)
+            for m in range(ramp + W, ramp + W + K):
+                step_fn(m % 4 + 1, chi, r, q, seed)
+            t1.record(stream)
+            dist.barrier()
+            torch.cuda.synchronize()
+        (ms,), _ = reduce_over_ranks([t0.elapsed_time(t1)], [0], dist, "cuda")
+        lnz = tt.log_Z_per_site()
+    finally:
+        tt.disable_phi_psi_split()
+    if rank == 0:
+        print(json.dumps({"mode": "Phi / Psi split over two GPUs (NCCL exchange every step)", "metric": METRIC,
+                          "value": K / (ms * 1e-3), "unit": UNIT, "n_gpus": 2, "steps": K, "warmup": W,
+                          "ms_per_step": ms / K, "scaling": "strong", "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": workload_name(name, cfg)}, "ln_Z_per_site": lnz}), flush=True)
+    dist.destroy_process_group()
+
+
 def run_split_emulation(args, cfg, name):
     """--split: what each of the two processes of the Phi / Psi split (tatrg_set_side_split; PAPER.md:167 'two GPUs
     are used') does per step, timed on ONE GPU by playing them one after the other: the whole
@@ -582,6 +628,9 @@ def run_split_emulation(args, cfg, name):
         raise RuntimeError("bench.py needs a CUDA device: libtatrg has no CPU fallback")
     chi, r, q, seed = cfg["chi"], cfg["r"], cfg["q"], cfg["seed"]
     K, W, ramp = args.steps, max(args.warmup, 0), cfg["ramp"]
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        return run_split_two_gpus(args, cfg, name)
     tt.set_workspace(chi=chi, r=r, atrg=bool(cfg.get("atrg")))
     step_fn = tt.coarse_grain_atrg if cfg.get("atrg") else tt.coarse_grain
     stream = torch.cuda.Stream()
