@@ -252,6 +252,8 @@ bool cholqr_fused(double *Y, long long m, int n, int passes, double shift_rel, i
     if (c.routes & ROUTE_UNFUSED_SQUEEZER) return false;
     if (n < 1 || n > CQ_B || passes < 1 || passes > 2 || m < CQ_ROWS) return false;
     if (n <= 32 && m >= 16384) return false;   // HBM-sized blocks of <= 32 columns: the streaming kernels of ts.cu (no padding)
+    if (m >= (1LL << 20)) return false;        // HBM-sized blocks of 33..64 columns (canonical form at chi > 32): compute-bound, the GEMM tiles
+                                               // on every SM are 1.2-1.6x faster than this grid of <= 128 CTAs (chi = 36..64: 4.1 -> 2.7 ... 32.2 -> 26.2 ms)
     const long long nchunks = (m + CQ_ROWS - 1) / CQ_ROWS;
     const int cap = c.sm_reserve > 0 ? c.sm_reserve : 128;   // resident: every CTA must find an SM
     const int grid = (int)std::min<long long>(nchunks, cap);
